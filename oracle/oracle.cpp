@@ -1,0 +1,952 @@
+/*
+ * oracle.cpp -- plain, slow, single-threaded CPU ORACLE of the gamma transport step loop.
+ *
+ * TEST INFRASTRUCTURE ONLY (see oracle.h).  Shares nothing with the CUDA path.
+ *
+ * Every function cites the passage it follows:
+ *   P:Lnn      = /root/reference/PAPER.md line nn   (Algorithm 1 = P:L55-76, Eq.1-9 = P:L78-150,
+ *                navigation problem statement = P:L120-127, Algorithm 2 = P:L133-144)
+ *   S:Cn       = SURVEY.md section 8(c) item Cn     (the readings of what the paper leaves silent)
+ *   D:...      = DESIGN.md "Readings" entry
+ *
+ * Arithmetic is the "canonical arithmetic" of S:C0: only + - * / sqrt, comparisons and |.| in
+ * navigation, evaluated left to right as written, compiled with -ffp-contract=off; explicit fma
+ * only in the affine transforms and in x + t*w.  Real = float | double per precision mode.
+ *
+ * Pins (tests/test_oracle_*.py): analytic box/tube distances, dense ray marching of the
+ * signed-distance field, brute-force locate with per-level transforms, chained steps vs. sorted
+ * analytic crossings, Klein-Nishina quadrature and k->0 limit, Compton energy-momentum
+ * conservation, chi^2 of sampled epsilon, slab transmission exp(-mu x), energy book-keeping,
+ * Philox vs. cuRAND's host generator, uniform end points.
+ * PARITY UNPINNED (defined only by SURVEY 8(c)/DESIGN.md, no independent truth exists):
+ *   sigma_PE0 normalisation, the capped Bethe-Heitler form, A values, source frame convention,
+ *   tolerances, tie-breaks, stuck guard, history hash.
+ */
+#include "oracle.h"
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#include <algorithm>
+
+namespace {
+
+/* ---- constants (S:C0) ---------------------------------------------------------------- */
+const double kMeC2 = 0.51099895;          /* MeV */
+const double kRe = 2.8179403262e-13;      /* cm  */
+const double kAlpha = 7.2973525693e-3;
+const double kNA = 6.02214076e23;
+const double kBarn = 1e-24;               /* cm^2 */
+const double kPi = 3.14159265358979323846;
+
+template <class R> inline R r_inf() { return std::numeric_limits<R>::infinity(); }
+template <class R> inline R r_fma(R a, R b, R c) { return std::fma(a, b, c); }
+template <class R> inline R r_abs(R a) { return std::fabs(a); }
+template <class R> inline R r_sqrt(R a) { return std::sqrt(a); }
+template <class R> inline R r_max(R a, R b) { return a > b ? a : b; }
+template <class R> inline R r_min(R a, R b) { return a < b ? a : b; }
+
+/* ---- geometry store ------------------------------------------------------------------- */
+struct SolidD {            /* as given (fp64) */
+    int type;
+    double a, b, c;        /* BOX: hx,hy,hz   TUBE: rmin,rmax,hz */
+    double sphi, dphi;
+    bool sector;
+    double cS, sS, cE, sE; /* host libm trig of sphi, sphi+dphi (S:C0) */
+};
+template <class R> struct SolidR {
+    int type; R a, b, c; bool sector; R cS, sS, cE, sE;
+};
+template <class R> struct XformR { R M[9]; R T[3]; };   /* global->local: p = M (x - T)  (S:C0) */
+
+struct Grid {              /* locate accelerator of one mother: uniform grid, padded lists */
+    int n[3]; double gmin[3], inv_w[3];
+    std::vector<int> start, cand;
+};
+
+struct MaterialD { double Z, A, rho; };
+template <class R> struct MaterialR { R aPE, aC, aP, capZ; };   /* D:"mu factorisation" */
+
+struct Geo {
+    std::vector<MaterialD> mats;
+    std::vector<SolidD> solids;
+    std::vector<int> parent, solid, material, xform_in;
+    std::vector<std::vector<int>> daughters;
+    std::vector<double> Rin, Tin;            /* input local->parent transforms per node (9,3) */
+    std::vector<XformR<double>> x64; std::vector<XformR<float>> x32;
+    std::vector<SolidR<double>> s64; std::vector<SolidR<float>> s32;
+    std::vector<MaterialR<double>> m64; std::vector<MaterialR<float>> m32;
+    std::vector<int> grid_of;                /* node -> index in grids or -1 */
+    std::vector<Grid> grids;
+    double tol64, tol32, sigma_pe0, e_cut; int stuck_limit, grid_min;
+};
+
+template <class R> struct Sel;
+template <> struct Sel<double> {
+    static const std::vector<XformR<double>>& x(const Geo& g) { return g.x64; }
+    static const std::vector<SolidR<double>>& s(const Geo& g) { return g.s64; }
+    static const std::vector<MaterialR<double>>& m(const Geo& g) { return g.m64; }
+    static double tol(const Geo& g) { return g.tol64; }
+};
+template <> struct Sel<float> {
+    static const std::vector<XformR<float>>& x(const Geo& g) { return g.x32; }
+    static const std::vector<SolidR<float>>& s(const Geo& g) { return g.s32; }
+    static const std::vector<MaterialR<float>>& m(const Geo& g) { return g.m32; }
+    static float tol(const Geo& g) { return (float)g.tol32; }
+};
+
+/* ---- solids (S:C2) -------------------------------------------------------------------- */
+enum { IN = 0, SURFACE = 1, OUT = 2 };
+
+template <class R> inline int classify(R D, R delta) {         /* S:C2 "Inside" */
+    if (D > delta) return OUT;
+    if (D >= -delta) return SURFACE;
+    return IN;
+}
+
+/* BOX: s_i = |p_i| - h_i */
+template <class R> int box_inside(const SolidR<R>& s, const R p[3], R delta) {
+    R D = r_max(r_max(r_abs(p[0]) - s.a, r_abs(p[1]) - s.b), r_abs(p[2]) - s.c);
+    return classify(D, delta);
+}
+
+/* one planar pair +-h along an axis, exit rule of S:C2: if moving outward and within the band -> 0,
+ * else candidate (sign(v) h - p)/v.  Returns false when the answer is 0. */
+template <class R> inline bool slab_out(R p, R v, R h, R delta, R& best) {
+    if (v > 0) {
+        if (p - h >= -delta) return false;
+        best = r_min(best, (h - p) / v);
+    } else if (v < 0) {
+        if (-p - h >= -delta) return false;
+        best = r_min(best, (-h - p) / v);
+    }
+    return true;
+}
+
+template <class R> R box_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R best = r_inf<R>();
+    if (!slab_out(p[0], v[0], s.a, delta, best)) return 0;
+    if (!slab_out(p[1], v[1], s.b, delta, best)) return 0;
+    if (!slab_out(p[2], v[2], s.c, delta, best)) return 0;
+    return r_max(best, (R)0);
+}
+
+/* S:C2 DistanceToIn BOX: slab method with tolerance */
+template <class R> R box_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    const R h[3] = {s.a, s.b, s.c};
+    R tmin = -r_inf<R>(), tmax = r_inf<R>();
+    for (int i = 0; i < 3; ++i) {
+        R si = r_abs(p[i]) - h[i];
+        if (si >= -delta && p[i] * v[i] >= 0) return r_inf<R>();
+        if (v[i] > 0) {
+            tmin = r_max(tmin, (-h[i] - p[i]) / v[i]);
+            tmax = r_min(tmax, (h[i] - p[i]) / v[i]);
+        } else if (v[i] < 0) {
+            tmin = r_max(tmin, (h[i] - p[i]) / v[i]);
+            tmax = r_min(tmax, (-h[i] - p[i]) / v[i]);
+        }
+    }
+    if (tmax <= tmin + delta) return r_inf<R>();
+    return tmin < delta ? (R)0 : tmin;
+}
+
+/* TUBE: rmin=a, rmax=b, hz=c; sector planes s_S = sS x - cS y, s_E = cE y - sE x */
+template <class R> int tube_inside(const SolidR<R>& s, const R p[3], R delta) {
+    R r = r_sqrt(p[0] * p[0] + p[1] * p[1]);
+    R D = r_abs(p[2]) - s.c;
+    D = r_max(D, r - s.b);
+    if (s.a > 0) D = r_max(D, s.a - r);
+    if (s.sector) {
+        D = r_max(D, s.sS * p[0] - s.cS * p[1]);
+        D = r_max(D, s.cE * p[1] - s.sE * p[0]);
+    }
+    return classify(D, delta);
+}
+
+template <class R> R tube_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R best = r_inf<R>();
+    if (!slab_out(p[2], v[2], s.c, delta, best)) return 0;           /* z planes */
+    R a = v[0] * v[0] + v[1] * v[1];
+    R b = p[0] * v[0] + p[1] * v[1];
+    R r2 = p[0] * p[0] + p[1] * p[1];
+    R r = r_sqrt(r2);
+    if (a > 0) {
+        /* outer cylinder: outward when b > 0; exit = larger root, stable form */
+        if (b > 0 && r - s.b >= -delta) return 0;
+        R c = r2 - s.b * s.b;
+        R Dq = r_max(b * b - a * c, (R)0);
+        R t = (b > 0) ? -c / (b + r_sqrt(Dq)) : (-b + r_sqrt(Dq)) / a;
+        best = r_min(best, t);
+        /* inner cylinder: outward (into the hole) when b < 0; hit = smaller root */
+        if (s.a > 0 && b < 0) {
+            if (s.a - r >= -delta) return 0;
+            R ci = r2 - s.a * s.a;
+            R Di = b * b - a * ci;
+            if (Di > 0) best = r_min(best, ci / (-b + r_sqrt(Di)));
+        }
+    }
+    if (s.sector) {
+        R sS = s.sS * p[0] - s.cS * p[1], dS = s.sS * v[0] - s.cS * v[1];
+        if (dS > 0) { if (sS >= -delta) return 0; best = r_min(best, -sS / dS); }
+        R sE = s.cE * p[1] - s.sE * p[0], dE = s.cE * v[1] - s.sE * v[0];
+        if (dE > 0) { if (sE >= -delta) return 0; best = r_min(best, -sE / dE); }
+    }
+    return r_max(best, (R)0);
+}
+
+template <class R> struct TubeHit {
+    const SolidR<R>& s; const R* p; const R* v; R delta;
+    R q[3];
+    void at(R t) { for (int i = 0; i < 3; ++i) q[i] = r_fma(t, v[i], p[i]); }
+    bool ok_z() const { return r_abs(q[2]) <= s.c + delta; }
+    bool ok_r() const {
+        R r = r_sqrt(q[0] * q[0] + q[1] * q[1]);
+        if (r > s.b + delta) return false;
+        if (s.a > 0 && r < s.a - delta) return false;
+        return true;
+    }
+    bool ok_phi() const {
+        if (!s.sector) return true;
+        return (s.sS * q[0] - s.cS * q[1] <= delta) && (s.cE * q[1] - s.sE * q[0] <= delta);
+    }
+};
+
+/* S:C2 DistanceToIn TUBE: minimum over validated candidates (i)-(iv) */
+template <class R> R tube_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R best = r_inf<R>();
+    TubeHit<R> h{s, p, v, delta, {0, 0, 0}};
+    R r2 = p[0] * p[0] + p[1] * p[1];
+    R r = r_sqrt(r2);
+    R a = v[0] * v[0] + v[1] * v[1];
+    R b = p[0] * v[0] + p[1] * v[1];
+    /* (i) z planes */
+    R sz = r_abs(p[2]) - s.c;
+    if (sz >= -delta) {
+        if (p[2] * v[2] >= 0) return r_inf<R>();
+        R t = r_max(sz / r_abs(v[2]), (R)0);
+        h.at(t);
+        if (h.ok_r() && h.ok_phi()) best = r_min(best, t);
+    }
+    /* (ii) outer cylinder from outside, must really penetrate the shrunken radius */
+    if (a > 0 && b < 0 && r >= s.b - delta) {
+        R rs = s.b - delta;
+        R cs = r2 - rs * rs;
+        if (b * b - a * cs > 0) {
+            R c = r2 - s.b * s.b;
+            R Dq = b * b - a * c;
+            R t = r_max(c / (-b + r_sqrt(Dq)), (R)0);
+            h.at(t);
+            if (h.ok_z() && h.ok_phi()) best = r_min(best, t);
+        }
+    }
+    /* (iii) inner cylinder: larger root = where the ray leaves the hole */
+    if (s.a > 0 && a > 0) {
+        R ci = r2 - s.a * s.a;
+        R Di = b * b - a * ci;
+        if (Di >= 0) {
+            R t = (b > 0) ? -ci / (b + r_sqrt(Di)) : (-b + r_sqrt(Di)) / a;
+            bool acc = (t >= 0);
+            if (!acc && r_abs(r - s.a) <= delta) { acc = true; }
+            if (acc) {
+                t = r_max(t, (R)0);
+                if (b + a * t > 0) {
+                    h.at(t);
+                    if (h.ok_z() && h.ok_phi()) best = r_min(best, t);
+                }
+            }
+        }
+    }
+    /* (iv) phi planes */
+    if (s.sector) {
+        for (int k = 0; k < 2; ++k) {
+            R c = k == 0 ? s.cS : s.cE, sn = k == 0 ? s.sS : s.sE;
+            R sp = k == 0 ? (s.sS * p[0] - s.cS * p[1]) : (s.cE * p[1] - s.sE * p[0]);
+            R dp = k == 0 ? (s.sS * v[0] - s.cS * v[1]) : (s.cE * v[1] - s.sE * v[0]);
+            if (sp >= -delta && dp < 0) {
+                R t = r_max(sp / (-dp), (R)0);
+                h.at(t);
+                if (!h.ok_z() || !h.ok_r()) continue;
+                if (h.q[0] * c + h.q[1] * sn < 0) continue;          /* correct half of the plane */
+                R so = k == 0 ? (s.cE * h.q[1] - s.sE * h.q[0]) : (s.sS * h.q[0] - s.cS * h.q[1]);
+                if (so > delta) continue;
+                best = r_min(best, t);
+            }
+        }
+    }
+    return best;
+}
+
+/* the "fork" on solid type */
+template <class R> int solid_inside(const SolidR<R>& s, const R p[3], R delta) {
+    return s.type == ORACLE_BOX ? box_inside(s, p, delta) : tube_inside(s, p, delta);
+}
+template <class R> R solid_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    return s.type == ORACLE_BOX ? box_dist_in(s, p, v, delta) : tube_dist_in(s, p, v, delta);
+}
+template <class R> R solid_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    return s.type == ORACLE_BOX ? box_dist_out(s, p, v, delta) : tube_dist_out(s, p, v, delta);
+}
+
+/* ---- navigator (S:C3, S:C4) ------------------------------------------------------------ */
+template <class R> struct Navigator {
+    const Geo& g; bool use_grid; R tol, delta;
+    const std::vector<XformR<R>>& X; const std::vector<SolidR<R>>& S;
+    Navigator(const Geo& geo, bool grid)
+        : g(geo), use_grid(grid), tol(Sel<R>::tol(geo)), delta(Sel<R>::tol(geo) / 2), X(Sel<R>::x(geo)), S(Sel<R>::s(geo)) {}
+
+    /* S:C0 affine transform with the explicit fma placement */
+    void local_point(int node, const R x[3], R p[3]) const {
+        const XformR<R>& t = X[node];
+        R d[3] = {x[0] - t.T[0], x[1] - t.T[1], x[2] - t.T[2]};
+        for (int k = 0; k < 3; ++k) p[k] = r_fma(t.M[3 * k + 2], d[2], r_fma(t.M[3 * k + 1], d[1], t.M[3 * k] * d[0]));
+    }
+    void local_dir(int node, const R w[3], R v[3]) const {
+        const XformR<R>& t = X[node];
+        for (int k = 0; k < 3; ++k) v[k] = r_fma(t.M[3 * k + 2], w[2], r_fma(t.M[3 * k + 1], w[1], t.M[3 * k] * w[0]));
+    }
+    /* S:C3 occupies */
+    bool occupies(int node, const R x[3], const R* w) const {
+        R p[3]; local_point(node, x, p);
+        const SolidR<R>& s = S[g.solid[node]];
+        int c = solid_inside(s, p, delta);
+        if (c == IN) return true;
+        if (c == OUT) return false;
+        if (!w) return true;
+        R v[3]; local_dir(node, w, v);
+        return solid_dist_out(s, p, v, delta) > 0;
+    }
+    /* descend from an occupied node through first-occupying daughters in index order (S:C3) */
+    int descend(int cur, const R x[3], const R* w) const {
+        for (;;) {
+            int found = -1;
+            int gi = use_grid ? g.grid_of[cur] : -1;
+            if (gi >= 0) {
+                /* accelerator: candidates of the grid cell holding the local point; padded lists are a
+                 * superset of every daughter that could occupy, kept in index order */
+                const Grid& G = g.grids[gi];
+                R p[3]; local_point(cur, x, p);
+                int c[3];
+                for (int k = 0; k < 3; ++k) {
+                    double f = std::floor(((double)p[k] - G.gmin[k]) * G.inv_w[k]);
+                    c[k] = (int)std::min(std::max(f, 0.0), (double)(G.n[k] - 1));
+                }
+                int cell = c[0] + G.n[0] * (c[1] + G.n[1] * c[2]);
+                for (int i = G.start[cell]; i < G.start[cell + 1]; ++i)
+                    if (occupies(G.cand[i], x, w)) { found = G.cand[i]; break; }
+            } else {
+                for (int d : g.daughters[cur]) if (occupies(d, x, w)) { found = d; break; }
+            }
+            if (found < 0) return cur;
+            cur = found;
+        }
+    }
+    int locate(const R x[3], const R* w) const {
+        if (!occupies(0, x, w)) return -1;
+        return descend(0, x, w);
+    }
+    /* S:C4 relocate: climb while not occupied, then descend */
+    int relocate(int X0, const R x[3], const R* w) const {
+        int cur = X0;
+        while (cur != -1 && !occupies(cur, x, w)) cur = g.parent[cur];
+        if (cur == -1) return -1;
+        return descend(cur, x, w);
+    }
+    /* S:C4 ComputeStep, plain definition: linear scan over all daughters */
+    void compute_step(int vol, const R x[3], const R w[3], R max_step, R& step, int& next) const {
+        if (vol < 0) { step = r_inf<R>(); next = -1; return; }
+        R p[3], v[3];
+        local_point(vol, x, p); local_dir(vol, w, v);
+        R best = solid_dist_out(S[g.solid[vol]], p, v, delta);
+        for (int d : g.daughters[vol]) {
+            local_point(d, x, p); local_dir(d, w, v);
+            R t = solid_dist_in(S[g.solid[d]], p, v, delta);
+            if (t < best) best = t;
+        }
+        if (best > max_step) { step = r_inf<R>(); next = vol; return; }
+        step = best;
+        R xn[3] = {r_fma(best, w[0], x[0]), r_fma(best, w[1], x[1]), r_fma(best, w[2], x[2])};
+        next = relocate(vol, xn, w);
+    }
+};
+
+/* ---- physics (S:C6) -------------------------------------------------------------------- */
+/* Klein-Nishina total cross-section per electron, cm^2 */
+double sigma_kn(double k) {
+    double l = std::log(1.0 + 2.0 * k);
+    double t1 = (1.0 + k) / (k * k) * (2.0 * (1.0 + k) / (1.0 + 2.0 * k) - l / k);
+    double t2 = l / (2.0 * k);
+    double t3 = (1.0 + 3.0 * k) / ((1.0 + 2.0 * k) * (1.0 + 2.0 * k));
+    return 2.0 * kPi * kRe * kRe * (t1 + t2 - t3);
+}
+double pair_cap(double Z) { return (28.0 / 9.0) * std::log(183.0 * std::pow(Z, -1.0 / 3.0)) - 2.0 / 27.0; }
+double sigma_pair(double k, double Z) {
+    if (!(k > 2.0)) return 0.0;
+    double P = std::min((28.0 / 9.0) * std::log(2.0 * k) - 218.0 / 27.0, pair_cap(Z));
+    return kAlpha * kRe * kRe * Z * Z * std::max(P, 0.0);
+}
+double sigma_pe(double E, double Z, double s0_barn) {
+    return s0_barn * kBarn * std::pow(Z / 82.0, 5.0) * std::pow(0.1 / E, 3.5);
+}
+
+/* D:"mu factorisation": energy factors are evaluated in fp64 from E and rounded once to Real;
+ * material factors are evaluated in fp64 at create time and rounded once to Real; the products and
+ * the sum are in Real.  In fp64 mode this is the closed form of S:C6 evaluated in a fixed order. */
+template <class R> struct EnergyFactors { R gPE, gKN, L2k; bool above_pair; };
+template <class R> EnergyFactors<R> energy_factors(R E) {
+    double e = (double)E, k = e / kMeC2;
+    EnergyFactors<R> f;
+    f.gPE = (R)std::pow(0.1 / e, 3.5);
+    f.gKN = (R)(sigma_kn(k) / (2.0 * kPi * kRe * kRe));
+    f.L2k = (R)std::log(2.0 * k);
+    f.above_pair = k > 2.0;
+    return f;
+}
+template <class R> void mu_partials(const MaterialR<R>& m, const EnergyFactors<R>& f, R mu[3]) {
+    mu[0] = m.aPE * f.gPE;
+    mu[1] = m.aC * f.gKN;
+    R P = r_min((R)(28.0 / 9.0) * f.L2k - (R)(218.0 / 27.0), m.capZ);
+    mu[2] = (f.above_pair && P > 0) ? m.aP * P : (R)0;
+}
+
+/* ---- RNG (S:C7) ------------------------------------------------------------------------ */
+void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        uint64_t p0 = (uint64_t)0xD2511F53u * c[0];
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c[2];
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c[1] ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c[3] ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c[0] = n0; c[1] = n1; c[2] = n2; c[3] = n3;
+    }
+}
+template <class R> R uniform_from_lane(uint64_t lane);
+template <> double uniform_from_lane<double>(uint64_t lane) { return (double)((lane >> 11) + 1) * 0x1p-53; }
+template <> float uniform_from_lane<float>(uint64_t lane) { return (float)((lane >> 40) + 1) * 0x1p-24f; }
+
+struct Stream {      /* draw j of photon id: lane (j mod 2) of block j/2 */
+    uint64_t seed, id; uint32_t j;
+    uint64_t lane() {
+        uint32_t c[4] = {(uint32_t)id, (uint32_t)(id >> 32), j >> 1, 0};
+        philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
+        uint64_t l = (j & 1) ? ((uint64_t)c[2] | ((uint64_t)c[3] << 32)) : ((uint64_t)c[0] | ((uint64_t)c[1] << 32));
+        ++j;
+        return l;
+    }
+    template <class R> R u() { return uniform_from_lane<R>(lane()); }
+};
+
+/* ---- sampling (S:C7) ------------------------------------------------------------------- */
+/* Klein-Nishina composition-rejection on eps = E'/E */
+template <class R> int kn_sample(R E, Stream& rng, R& eps, R& cost, R& sint2) {
+    R k = E / (R)kMeC2;
+    R eps0 = (R)1 / ((R)1 + (R)2 * k);
+    R a1 = -std::log(eps0);
+    R eps0sq = eps0 * eps0;
+    R a2 = ((R)1 - eps0sq) / (R)2;
+    int trials = 0;
+    for (;;) {
+        ++trials;
+        R u1 = rng.u<R>(), u2 = rng.u<R>(), u3 = rng.u<R>();
+        R e, e2;
+        if (u1 < a1 / (a1 + a2)) { e = std::exp(-a1 * u2); e2 = e * e; }
+        else { e2 = eps0sq + ((R)1 - eps0sq) * u2; e = r_sqrt(e2); }
+        R t = ((R)1 - e) / (k * e);
+        R s2 = t * ((R)2 - t);
+        if ((R)1 - e * s2 / ((R)1 + e2) >= u3) { eps = e; cost = (R)1 - t; sint2 = s2; return trials; }
+    }
+}
+/* direction update */
+template <class R> void rotate_dir(R w[3], R cost, R sint, R phi) {
+    R cp = std::cos(phi), sp = std::sin(phi);
+    R u = w[0], v = w[1], ww = w[2];
+    R s2 = u * u + v * v;
+    R n[3];
+    if (s2 >= (R)1e-10) {
+        R s = r_sqrt(s2);
+        n[0] = u * cost + sint * (u * ww * cp - v * sp) / s;
+        n[1] = v * cost + sint * (v * ww * cp + u * sp) / s;
+        n[2] = ww * cost - s * sint * cp;
+    } else {
+        n[0] = sint * cp; n[1] = sint * sp; n[2] = (ww < 0 ? -cost : cost);
+    }
+    R nn = r_sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+    w[0] = n[0] / nn; w[1] = n[1] / nn; w[2] = n[2] / nn;
+}
+
+/* ---- source (S:C8, D:"source frame") ---------------------------------------------------- */
+template <class R> struct SourceR {
+    int kind, energy_kind;
+    R o[3], a[3], e1[3], e2[3];
+    R sigma, cos_half, e0, ln_e0, ln_ratio;
+};
+template <class R> bool make_source(const oracle_source_t& s, SourceR<R>& o) {
+    double n = std::sqrt(s.axis[0] * s.axis[0] + s.axis[1] * s.axis[1] + s.axis[2] * s.axis[2]);
+    if (!(n > 0)) return false;
+    double a[3] = {s.axis[0] / n, s.axis[1] / n, s.axis[2] / n};
+    int m = 0;                                                       /* smallest |a_i|, ties x<y<z */
+    if (std::fabs(a[1]) < std::fabs(a[m])) m = 1;
+    if (std::fabs(a[2]) < std::fabs(a[m])) m = 2;
+    double h[3] = {0, 0, 0}; h[m] = 1;
+    double ha = a[m];
+    double e1[3] = {h[0] - ha * a[0], h[1] - ha * a[1], h[2] - ha * a[2]};
+    double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+    for (int i = 0; i < 3; ++i) e1[i] /= n1;
+    double e2[3] = {a[1] * e1[2] - a[2] * e1[1], a[2] * e1[0] - a[0] * e1[2], a[0] * e1[1] - a[1] * e1[0]};
+    o.kind = s.kind; o.energy_kind = s.energy_kind;
+    for (int i = 0; i < 3; ++i) { o.o[i] = (R)s.origin[i]; o.a[i] = (R)a[i]; o.e1[i] = (R)e1[i]; o.e2[i] = (R)e2[i]; }
+    o.sigma = (R)s.sigma; o.cos_half = (R)std::cos(s.half_angle);
+    o.e0 = (R)s.e0;
+    if (s.energy_kind == ORACLE_E_LOGUNIFORM) {
+        if (!(s.e0 > 0) || !(s.e1 >= s.e0)) return false;
+        o.ln_e0 = (R)std::log(s.e0); o.ln_ratio = (R)std::log(s.e1 / s.e0);
+    } else { o.ln_e0 = 0; o.ln_ratio = 0; }
+    return s.e0 > 0;
+}
+template <class R> void sample_source(const SourceR<R>& s, Stream& rng, R x[3], R w[3], R& E) {
+    const R twopi = (R)6.283185307179586;
+    for (int i = 0; i < 3; ++i) { x[i] = s.o[i]; w[i] = s.a[i]; }
+    if (s.kind == ORACLE_SRC_GAUSS_PENCIL) {
+        R u0 = rng.u<R>(), u1 = rng.u<R>();
+        R r = s.sigma * r_sqrt((R)-2 * std::log(u0));
+        R phi = twopi * u1;
+        R gx = r * std::cos(phi), gy = r * std::sin(phi);
+        for (int i = 0; i < 3; ++i) x[i] = s.o[i] + (gx * s.e1[i] + gy * s.e2[i]);
+    } else if (s.kind == ORACLE_SRC_CONE || s.kind == ORACLE_SRC_ISOTROPIC) {
+        R u0 = rng.u<R>(), u1 = rng.u<R>();
+        R ct = (s.kind == ORACLE_SRC_CONE) ? (R)1 - u0 * ((R)1 - s.cos_half) : (R)1 - (R)2 * u0;
+        R st = r_sqrt(r_max(((R)1 - ct) * ((R)1 + ct), (R)0));
+        R phi = twopi * u1;
+        R cx = st * std::cos(phi), cy = st * std::sin(phi);
+        R n[3];
+        for (int i = 0; i < 3; ++i) n[i] = (cx * s.e1[i] + cy * s.e2[i]) + ct * s.a[i];
+        R nn = r_sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+        for (int i = 0; i < 3; ++i) w[i] = n[i] / nn;
+    }
+    if (s.energy_kind == ORACLE_E_LOGUNIFORM) E = std::exp(s.ln_e0 + rng.u<R>() * s.ln_ratio);
+    else E = s.e0;
+}
+
+/* ---- transport loop (Algorithm 1 generalised, S:C9) ---------------------------- */
+inline void fnv_word(uint64_t& h, uint32_t w) {
+    for (int i = 0; i < 4; ++i) { h ^= (w >> (8 * i)) & 0xffu; h *= 0x100000001b3ull; }
+}
+enum { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
+
+template <class R>
+void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& src, uint64_t seed, uint64_t id,
+                      double* edep, oracle_stats_t& st, uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out) {
+    const std::vector<MaterialR<R>>& mats = Sel<R>::m(g);
+    const R twopi = (R)6.283185307179586;
+    Stream rng{seed, id, 0};
+    R x[3], w[3], E;
+    sample_source(src, rng, x, w, E);
+    st.n_photons++; st.e_source += (double)E;
+    uint64_t h = 0xcbf29ce484222325ull; uint32_t ns = 0;
+    int vol = nav.locate(x, w);
+    bool alive = true;
+    if (vol < 0) { st.n_escaped++; st.e_escaped += (double)E; alive = false; }
+    R Y = 0; EnergyFactors<R> ef{};
+    if (alive) { Y = -std::log(rng.u<R>()); ef = energy_factors(E); }           /* Alg.1 steps 1-2 */
+    int zero_steps = 0;
+    while (alive) {
+        R mu3[3]; mu_partials(mats[g.material[vol]], ef, mu3);
+        R mu = (mu3[0] + mu3[1]) + mu3[2];
+        R s_int = mu > 0 ? Y / mu : r_inf<R>();                                 /* Eq.7 remaining part */
+        R step; int next;
+        nav.compute_step(vol, x, w, s_int, step, next);                         /* "next intersection" P:L67 */
+        ++ns; st.n_steps++;
+        int vol_before = vol, ev; R len;
+        if (step == r_inf<R>()) {                                               /* S_j >= Y: interact here */
+            len = s_int;
+            for (int i = 0; i < 3; ++i) x[i] = r_fma(s_int, w[i], x[i]);
+            R t = rng.u<R>() * mu;
+            if (t < mu3[0]) {                                                   /* photoelectric */
+                edep[vol] += (double)E; st.e_deposited += (double)E; st.n_pe++; ev = EV_PE; alive = false;
+            } else if (t < mu3[0] + mu3[1] || !(mu3[2] > 0)) {                  /* Compton */
+                R eps, cost, s2; kn_sample(E, rng, eps, cost, s2);
+                R Ep = eps * E;
+                R phi = twopi * rng.u<R>();
+                rotate_dir(w, cost, r_sqrt(r_max(s2, (R)0)), phi);
+                R dep = E - Ep;
+                st.n_compton++; ev = EV_COMPTON;
+                E = Ep;
+                if (Ep < (R)g.e_cut) { dep = dep + Ep; st.n_cut++; ev = EV_CUT; alive = false; }
+                edep[vol] += (double)dep; st.e_deposited += (double)dep;
+                if (alive) { ef = energy_factors(E); Y = -std::log(rng.u<R>()); }
+            } else {                                                            /* pair: local deposit */
+                edep[vol] += (double)E; st.e_deposited += (double)E; st.n_pair++; ev = EV_PAIR; alive = false;
+            }
+        } else {                                                                /* boundary */
+            len = step;
+            for (int i = 0; i < 3; ++i) x[i] = r_fma(step, w[i], x[i]);
+            Y = r_max(Y - step * mu, (R)0);                                     /* S_j update */
+            vol = next;
+            if (vol < 0) { st.n_escaped++; st.e_escaped += (double)E; ev = EV_ESCAPE; alive = false; }
+            else ev = EV_BOUNDARY;
+        }
+        if (len <= nav.delta) ++zero_steps; else zero_steps = 0;
+        if (alive && zero_steps >= g.stuck_limit) { st.n_stuck++; st.e_stuck += (double)E; ev = EV_STUCK; alive = false; }
+        fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
+    }
+    if (hash_out) *hash_out = h;
+    if (nsteps_out) *nsteps_out = ns;
+    if (efinal_out) *efinal_out = (double)E;
+}
+
+/* ---- geometry construction -------------------------------------------------------------- */
+void mat3_mul(const double* A, const double* B, double* C) {
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j)
+        C[3 * i + j] = (A[3 * i] * B[j] + A[3 * i + 1] * B[3 + j]) + A[3 * i + 2] * B[6 + j];
+}
+
+/* tight AABB of a solid in its own frame */
+void solid_aabb(const SolidD& s, double lo[3], double hi[3]) {
+    if (s.type == ORACLE_BOX) { lo[0] = -s.a; hi[0] = s.a; lo[1] = -s.b; hi[1] = s.b; lo[2] = -s.c; hi[2] = s.c; return; }
+    lo[2] = -s.c; hi[2] = s.c;
+    if (!s.sector) { lo[0] = lo[1] = -s.b; hi[0] = hi[1] = s.b; return; }
+    double xs[16], ys[16]; int n = 0;
+    double ang[2] = {s.sphi, s.sphi + s.dphi}, rr[2] = {s.a, s.b};
+    for (int i = 0; i < 2; ++i) for (int j = 0; j < 2; ++j) { xs[n] = rr[j] * std::cos(ang[i]); ys[n] = rr[j] * std::sin(ang[i]); ++n; }
+    for (int k = -8; k <= 8; ++k) {
+        double th = k * (kPi / 2);
+        if (th >= ang[0] && th <= ang[1]) { xs[n] = s.b * std::cos(th); ys[n] = s.b * std::sin(th); ++n; }
+    }
+    lo[0] = hi[0] = xs[0]; lo[1] = hi[1] = ys[0];
+    for (int i = 1; i < n; ++i) { lo[0] = std::min(lo[0], xs[i]); hi[0] = std::max(hi[0], xs[i]); lo[1] = std::min(lo[1], ys[i]); hi[1] = std::max(hi[1], ys[i]); }
+}
+
+void build_grid(Geo& g, int mother) {
+    const std::vector<int>& ds = g.daughters[mother];
+    Grid G;
+    double mlo[3], mhi[3];
+    const SolidD& ms = g.solids[g.solid[mother]];
+    if (ms.type == ORACLE_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; mlo[2] = -ms.c; mhi[2] = ms.c; }
+    else { mlo[0] = mlo[1] = -ms.b; mhi[0] = mhi[1] = ms.b; mlo[2] = -ms.c; mhi[2] = ms.c; }
+    int nper = (int)std::ceil(std::cbrt((double)ds.size()));
+    nper = std::max(1, std::min(nper, 64));
+    double pad = 2.0 * std::max(g.tol32, g.tol64);
+    for (int k = 0; k < 3; ++k) { G.n[k] = nper; G.gmin[k] = mlo[k]; G.inv_w[k] = nper / (mhi[k] - mlo[k]); }
+    size_t ncell = (size_t)nper * nper * nper;
+    std::vector<std::vector<int>> lists(ncell);
+    for (int d : ds) {
+        double lo[3], hi[3]; solid_aabb(g.solids[g.solid[d]], lo, hi);
+        const double* Rm = &g.Rin[9 * d]; const double* T = &g.Tin[3 * d];
+        double alo[3] = {1e300, 1e300, 1e300}, ahi[3] = {-1e300, -1e300, -1e300};
+        for (int c = 0; c < 8; ++c) {
+            double q[3] = {(c & 1) ? hi[0] : lo[0], (c & 2) ? hi[1] : lo[1], (c & 4) ? hi[2] : lo[2]};
+            for (int k = 0; k < 3; ++k) {
+                double y = Rm[3 * k] * q[0] + Rm[3 * k + 1] * q[1] + Rm[3 * k + 2] * q[2] + T[k];
+                alo[k] = std::min(alo[k], y); ahi[k] = std::max(ahi[k], y);
+            }
+        }
+        int c0[3], c1[3];
+        for (int k = 0; k < 3; ++k) {
+            c0[k] = (int)std::min(std::max(std::floor((alo[k] - pad - G.gmin[k]) * G.inv_w[k]), 0.0), (double)(nper - 1));
+            c1[k] = (int)std::min(std::max(std::floor((ahi[k] + pad - G.gmin[k]) * G.inv_w[k]), 0.0), (double)(nper - 1));
+        }
+        for (int iz = c0[2]; iz <= c1[2]; ++iz) for (int iy = c0[1]; iy <= c1[1]; ++iy) for (int ix = c0[0]; ix <= c1[0]; ++ix)
+            lists[ix + (size_t)nper * (iy + (size_t)nper * iz)].push_back(d);   /* ds ascending -> lists ascending */
+    }
+    G.start.resize(ncell + 1); G.start[0] = 0;
+    for (size_t c = 0; c < ncell; ++c) G.start[c + 1] = G.start[c] + (int)lists[c].size();
+    G.cand.reserve(G.start[ncell]);
+    for (size_t c = 0; c < ncell; ++c) G.cand.insert(G.cand.end(), lists[c].begin(), lists[c].end());
+    g.grid_of[mother] = (int)g.grids.size();
+    g.grids.push_back(std::move(G));
+}
+
+template <class R> SolidR<R> round_solid(const SolidD& s) {
+    SolidR<R> o; o.type = s.type; o.a = (R)s.a; o.b = (R)s.b; o.c = (R)s.c; o.sector = s.sector;
+    o.cS = (R)s.cS; o.sS = (R)s.sS; o.cE = (R)s.cE; o.sE = (R)s.sE; return o;
+}
+template <class R> MaterialR<R> round_material(const MaterialD& m, double s0) {
+    double n = m.rho * kNA / m.A;                 /* atoms / cm^3;  mu[1/mm] = n sigma / 10 (S:C6) */
+    MaterialR<R> o;
+    o.aPE = (R)(n * (s0 * kBarn * std::pow(m.Z / 82.0, 5.0)) / 10.0);
+    o.aC = (R)(n * (m.Z * (2.0 * kPi * kRe * kRe)) / 10.0);
+    o.aP = (R)(n * (kAlpha * kRe * kRe * m.Z * m.Z) / 10.0);
+    o.capZ = (R)pair_cap(m.Z);
+    return o;
+}
+
+template <class R> int run_locate(const Geo& g, const void* pos, const void* dir, int64_t n, int32_t* out, bool grid) {
+    Navigator<R> nav(g, grid);
+    const R* P = (const R*)pos; const R* D = (const R*)dir;
+    for (int64_t i = 0; i < n; ++i) out[i] = nav.locate(P + 3 * i, D ? D + 3 * i : nullptr);
+    return ORACLE_OK;
+}
+template <class R> int run_step(const Geo& g, const void* pos, const void* dir, const int32_t* vol, const void* maxs,
+                                int64_t n, void* step_out, int32_t* next_out, bool grid) {
+    Navigator<R> nav(g, grid);
+    const R* P = (const R*)pos; const R* D = (const R*)dir; const R* Mx = (const R*)maxs; R* S = (R*)step_out;
+    for (int64_t i = 0; i < n; ++i) {
+        R st; int nx;
+        if (vol[i] >= (int32_t)g.parent.size()) return ORACLE_INVALID_ARGUMENT;
+        nav.compute_step(vol[i], P + 3 * i, D + 3 * i, Mx ? Mx[i] : r_inf<R>(), st, nx);
+        S[i] = st; next_out[i] = nx;
+    }
+    return ORACLE_OK;
+}
+template <class R> int run_transport(const Geo& g, const oracle_source_t* src, uint64_t seed, int64_t first, int64_t n,
+                                     double* edep, oracle_stats_t* st, uint64_t* hash, uint32_t* ns, double* ef, bool grid) {
+    SourceR<R> s;
+    if (!make_source(*src, s)) return ORACLE_INVALID_ARGUMENT;
+    Navigator<R> nav(g, grid);
+    oracle_stats_t local; std::memset(&local, 0, sizeof local);
+    for (int64_t i = 0; i < n; ++i)
+        transport_photon<R>(g, nav, s, seed, (uint64_t)(first + i), edep, local, hash ? hash + i : nullptr,
+                            ns ? ns + i : nullptr, ef ? ef + i : nullptr);
+    if (st) *st = local;
+    return ORACLE_OK;
+}
+
+template <class R> int run_solid_eval(const SolidD& sd, double tol, int what, const void* pos, const void* dir, int64_t n, void* out) {
+    SolidR<R> s = round_solid<R>(sd);
+    R delta = (R)tol / 2;
+    const R* P = (const R*)pos; const R* D = (const R*)dir; R* O = (R*)out;
+    for (int64_t i = 0; i < n; ++i) {
+        if (what == 0) O[i] = (R)solid_inside(s, P + 3 * i, delta);
+        else if (what == 1) O[i] = solid_dist_in(s, P + 3 * i, D + 3 * i, delta);
+        else O[i] = solid_dist_out(s, P + 3 * i, D + 3 * i, delta);
+    }
+    return ORACLE_OK;
+}
+
+int make_solid(int type, const double* p, SolidD& s) {
+    s.type = type; s.sector = false; s.cS = s.sS = s.cE = s.sE = 0; s.sphi = s.dphi = 0;
+    if (type == ORACLE_BOX) {
+        s.a = p[0]; s.b = p[1]; s.c = p[2];
+        if (!(s.a > 0 && s.b > 0 && s.c > 0)) return ORACLE_INVALID_ARGUMENT;
+        return ORACLE_OK;
+    }
+    if (type != ORACLE_TUBE) return ORACLE_UNSUPPORTED_SOLID;
+    s.a = p[0]; s.b = p[1]; s.c = p[2]; s.sphi = p[3]; s.dphi = p[4];
+    if (!(s.a >= 0 && s.b > s.a && s.c > 0)) return ORACLE_INVALID_ARGUMENT;
+    if (s.dphi >= 2 * kPi) return ORACLE_OK;
+    if (!(s.dphi > 0) || s.dphi > kPi) return ORACLE_UNSUPPORTED_SOLID;      /* convex sectors only (S:C2) */
+    s.sector = true;
+    s.cS = std::cos(s.sphi); s.sS = std::sin(s.sphi);
+    s.cE = std::cos(s.sphi + s.dphi); s.sE = std::sin(s.sphi + s.dphi);
+    return ORACLE_OK;
+}
+
+}  // namespace
+
+/* ======================================================================================== */
+extern "C" {
+
+int oracle_geometry_create(const double* materials, int32_t n_mats, const int32_t* solid_type, const double* solid_params,
+                           int32_t n_solids, const int32_t* placements, int32_t n_places, const double* transforms,
+                           int32_t n_transforms, const oracle_opts_t* opts, void** out) {
+    if (!materials || !solid_type || !solid_params || !placements || !transforms || !out) return ORACLE_INVALID_ARGUMENT;
+    if (n_mats <= 0 || n_solids <= 0 || n_places <= 0 || n_transforms <= 0) return ORACLE_INVALID_ARGUMENT;
+    Geo* g = new Geo();
+    for (int i = 0; i < n_mats; ++i) {
+        MaterialD m{materials[3 * i], materials[3 * i + 1], materials[3 * i + 2]};
+        if (!(m.Z > 0 && m.A > 0 && m.rho >= 0)) { delete g; return ORACLE_INVALID_ARGUMENT; }
+        g->mats.push_back(m);
+    }
+    for (int i = 0; i < n_solids; ++i) {
+        SolidD s; int rc = make_solid(solid_type[i], solid_params + 5 * i, s);
+        if (rc != ORACLE_OK) { delete g; return rc; }
+        g->solids.push_back(s);
+    }
+    g->parent.resize(n_places); g->solid.resize(n_places); g->material.resize(n_places); g->xform_in.resize(n_places);
+    g->daughters.resize(n_places); g->Rin.resize(9 * (size_t)n_places); g->Tin.resize(3 * (size_t)n_places);
+    g->x64.resize(n_places); g->x32.resize(n_places);
+    std::vector<double> Rg(9 * (size_t)n_places), Tg(3 * (size_t)n_places);
+    for (int i = 0; i < n_places; ++i) {
+        int p = placements[4 * i], s = placements[4 * i + 1], m = placements[4 * i + 2], t = placements[4 * i + 3];
+        if (s < 0 || s >= n_solids || m < 0 || m >= n_mats || t < 0 || t >= n_transforms) { delete g; return ORACLE_INVALID_ARGUMENT; }
+        if ((i == 0 && p != -1) || (i > 0 && (p < 0 || p >= i))) { delete g; return ORACLE_BAD_TREE; }
+        g->parent[i] = p; g->solid[i] = s; g->material[i] = m; g->xform_in[i] = t;
+        const double* Rl = transforms + 12 * (size_t)t; const double* Tl = Rl + 9;
+        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) {          /* orthonormality */
+            double dot = Rl[3 * a] * Rl[3 * b] + Rl[3 * a + 1] * Rl[3 * b + 1] + Rl[3 * a + 2] * Rl[3 * b + 2];
+            if (std::fabs(dot - (a == b ? 1.0 : 0.0)) > 1e-9) { delete g; return ORACLE_BAD_TREE; }
+        }
+        std::memcpy(&g->Rin[9 * (size_t)i], Rl, 9 * sizeof(double)); std::memcpy(&g->Tin[3 * (size_t)i], Tl, 3 * sizeof(double));
+        /* S:C0 composition root-down in fp64: Rg = Rg_parent R, Tg = Rg_parent T + Tg_parent */
+        double* R = &Rg[9 * (size_t)i]; double* T = &Tg[3 * (size_t)i];
+        if (p < 0) { std::memcpy(R, Rl, 9 * sizeof(double)); std::memcpy(T, Tl, 3 * sizeof(double)); }
+        else {
+            const double* Rp = &Rg[9 * (size_t)p]; const double* Tp = &Tg[3 * (size_t)p];
+            mat3_mul(Rp, Rl, R);
+            for (int a = 0; a < 3; ++a) T[a] = ((Rp[3 * a] * Tl[0] + Rp[3 * a + 1] * Tl[1]) + Rp[3 * a + 2] * Tl[2]) + Tp[a];
+            g->daughters[p].push_back(i);
+        }
+        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) {          /* M = Rg^T */
+            g->x64[i].M[3 * a + b] = R[3 * b + a]; g->x32[i].M[3 * a + b] = (float)R[3 * b + a];
+        }
+        for (int a = 0; a < 3; ++a) { g->x64[i].T[a] = T[a]; g->x32[i].T[a] = (float)T[a]; }
+    }
+    const SolidD& ws = g->solids[g->solid[0]];
+    double ext = ws.type == ORACLE_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : std::max(ws.b, ws.c);
+    g->tol64 = (opts && opts->tol64 > 0) ? opts->tol64 : 1e-9;
+    g->tol32 = (opts && opts->tol32 > 0) ? opts->tol32 : (double)(float)(ext * 0x1p-18);
+    g->sigma_pe0 = (opts && opts->sigma_pe0 > 0) ? opts->sigma_pe0 : 1750.0;
+    g->e_cut = (opts && opts->e_cut > 0) ? opts->e_cut : 0.010;
+    g->grid_min = (opts && opts->grid_min_daughters > 0) ? opts->grid_min_daughters : 8;
+    g->stuck_limit = (opts && opts->stuck_limit > 0) ? opts->stuck_limit : 8;
+    for (const SolidD& s : g->solids) { g->s64.push_back(round_solid<double>(s)); g->s32.push_back(round_solid<float>(s)); }
+    for (const MaterialD& m : g->mats) { g->m64.push_back(round_material<double>(m, g->sigma_pe0)); g->m32.push_back(round_material<float>(m, g->sigma_pe0)); }
+    g->grid_of.assign(n_places, -1);
+    for (int i = 0; i < n_places; ++i) if ((int)g->daughters[i].size() >= g->grid_min) build_grid(*g, i);
+    *out = g;
+    return ORACLE_OK;
+}
+
+int oracle_geometry_destroy(void* geo) { delete (Geo*)geo; return ORACLE_OK; }
+double oracle_geometry_tolerance(const void* geo, int precision) {
+    const Geo* g = (const Geo*)geo; return precision == 32 ? g->tol32 : g->tol64;
+}
+
+int oracle_nav_locate(const void* geo, int precision, const void* pos, const void* dir, int64_t n, int32_t* vol_out, int use_grid) {
+    if (!geo || (n > 0 && (!pos || !vol_out)) || n < 0) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    if (precision == 64) return run_locate<double>(g, pos, dir, n, vol_out, use_grid != 0);
+    if (precision == 32) return run_locate<float>(g, pos, dir, n, vol_out, use_grid != 0);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+/* Pin for locate (S:C3 "plain definition"): every node, hierarchical per-level transforms in fp64,
+ * surface counts as inside; answer = deepest node containing the point with all ancestors containing it. */
+int oracle_nav_locate_bruteforce(const void* geo, const double* pos, int64_t n, int32_t* vol_out) {
+    if (!geo || !pos || !vol_out) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    size_t V = g.parent.size();
+    std::vector<double> pl(3 * V); std::vector<char> in(V); std::vector<int> depth(V);
+    double delta = g.tol64 / 2;
+    for (int64_t q = 0; q < n; ++q) {
+        int best = -1, bestd = -1;
+        for (size_t i = 0; i < V; ++i) {
+            const double* Rl = &g.Rin[9 * i]; const double* Tl = &g.Tin[3 * i];
+            double x[3];
+            int p = g.parent[i];
+            if (p < 0) { x[0] = pos[3 * q]; x[1] = pos[3 * q + 1]; x[2] = pos[3 * q + 2]; depth[i] = 0; }
+            else { x[0] = pl[3 * p]; x[1] = pl[3 * p + 1]; x[2] = pl[3 * p + 2]; depth[i] = depth[p] + 1; }
+            double d[3] = {x[0] - Tl[0], x[1] - Tl[1], x[2] - Tl[2]};
+            for (int k = 0; k < 3; ++k) pl[3 * i + k] = Rl[k] * d[0] + Rl[3 + k] * d[1] + Rl[6 + k] * d[2];   /* R^T d */
+            bool anc = p < 0 ? true : (bool)in[p];
+            in[i] = anc && solid_inside(g.s64[g.solid[i]], &pl[3 * i], delta) != OUT;
+            if (in[i] && depth[i] > bestd) { best = (int)i; bestd = depth[i]; }
+        }
+        vol_out[q] = best;
+    }
+    return ORACLE_OK;
+}
+
+int oracle_nav_compute_step(const void* geo, int precision, const void* pos, const void* dir, const int32_t* vol_in,
+                            const void* max_step, int64_t n, void* step_out, int32_t* next_vol_out, int use_grid) {
+    if (!geo || n < 0 || (n > 0 && (!pos || !dir || !vol_in || !step_out || !next_vol_out))) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    if (precision == 64) return run_step<double>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, use_grid != 0);
+    if (precision == 32) return run_step<float>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, use_grid != 0);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+int oracle_transport_run(const void* geo, int precision, const oracle_source_t* src, uint64_t seed, int64_t first_id,
+                         int64_t n_photons, double* edep_out, oracle_stats_t* stats_out, uint64_t* hash_out,
+                         uint32_t* nsteps_out, double* efinal_out, int use_grid) {
+    if (!geo || !src || !edep_out || n_photons < 0 || first_id < 0) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    if (precision == 64) return run_transport<double>(g, src, seed, first_id, n_photons, edep_out, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
+    if (precision == 32) return run_transport<float>(g, src, seed, first_id, n_photons, edep_out, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+int oracle_solid_eval(int32_t type, const double* params5, double tol, int precision, int what, const void* pos,
+                      const void* dir, int64_t n, void* out) {
+    SolidD s; int rc = make_solid(type, params5, s);
+    if (rc != ORACLE_OK) return rc;
+    if (precision == 64) return run_solid_eval<double>(s, tol, what, pos, dir, n, out);
+    if (precision == 32) return run_solid_eval<float>(s, tol, what, pos, dir, n, out);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+double oracle_sigma_kn(double k) { return sigma_kn(k); }
+double oracle_sigma_pair(double k, double Z) { return sigma_pair(k, Z); }
+double oracle_sigma_pe(double E, double Z, double s0) { return sigma_pe(E, Z, s0); }
+
+int oracle_mu(const void* geo, int precision, int32_t material, double E, double* mu3) {
+    const Geo& g = *(const Geo*)geo;
+    if (material < 0 || material >= (int)g.mats.size()) return ORACLE_INVALID_ARGUMENT;
+    if (precision == 64) { double m[3]; mu_partials(g.m64[material], energy_factors<double>(E), m); mu3[0] = m[0]; mu3[1] = m[1]; mu3[2] = m[2]; }
+    else { float m[3]; mu_partials(g.m32[material], energy_factors<float>((float)E), m); mu3[0] = m[0]; mu3[1] = m[1]; mu3[2] = m[2]; }
+    return ORACLE_OK;
+}
+
+void oracle_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t* out4) {
+    uint32_t c[4] = {c0, c1, c2, c3}; philox4x32_10(c, k0, k1); std::memcpy(out4, c, sizeof c);
+}
+double oracle_uniform_from_lane(uint64_t lane, int precision) {
+    return precision == 32 ? (double)uniform_from_lane<float>(lane) : uniform_from_lane<double>(lane);
+}
+double oracle_draw(uint64_t seed, uint64_t id, uint32_t j, int precision) {
+    Stream s{seed, id, j};
+    return precision == 32 ? (double)s.u<float>() : s.u<double>();
+}
+
+int oracle_kn_sample(int precision, double E, uint64_t seed, int64_t first_id, int64_t n, double* eps_out, double* cost_out, int32_t* ntrials_out) {
+    for (int64_t i = 0; i < n; ++i) {
+        Stream s{seed, (uint64_t)(first_id + i), 0};
+        if (precision == 64) { double e, c, s2; int t = kn_sample<double>(E, s, e, c, s2); eps_out[i] = e; cost_out[i] = c; if (ntrials_out) ntrials_out[i] = t; }
+        else { float e, c, s2; int t = kn_sample<float>((float)E, s, e, c, s2); eps_out[i] = e; cost_out[i] = c; if (ntrials_out) ntrials_out[i] = t; }
+    }
+    return ORACLE_OK;
+}
+
+int oracle_rotate(int precision, const double* w, const double* cost, const double* phi, int64_t n, double* w_out) {
+    for (int64_t i = 0; i < n; ++i) {
+        if (precision == 64) {
+            double v[3] = {w[3 * i], w[3 * i + 1], w[3 * i + 2]};
+            double st = std::sqrt(std::max(0.0, 1.0 - cost[i] * cost[i]));
+            rotate_dir<double>(v, cost[i], st, phi[i]);
+            for (int k = 0; k < 3; ++k) w_out[3 * i + k] = v[k];
+        } else {
+            float v[3] = {(float)w[3 * i], (float)w[3 * i + 1], (float)w[3 * i + 2]};
+            float c = (float)cost[i]; float st = std::sqrt(std::max(0.0f, 1.0f - c * c));
+            rotate_dir<float>(v, c, st, (float)phi[i]);
+            for (int k = 0; k < 3; ++k) w_out[3 * i + k] = v[k];
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* S:C0 the canonical move x' = fma(t, w, x) */
+int oracle_move(int precision, const void* pos, const void* dir, const void* step, int64_t n, void* pos_out) {
+    if (precision == 64) {
+        const double* P = (const double*)pos; const double* D = (const double*)dir; const double* S = (const double*)step; double* O = (double*)pos_out;
+        for (int64_t i = 0; i < 3 * n; ++i) O[i] = std::fma(S[i / 3], D[i], P[i]);
+    } else if (precision == 32) {
+        const float* P = (const float*)pos; const float* D = (const float*)dir; const float* S = (const float*)step; float* O = (float*)pos_out;
+        for (int64_t i = 0; i < 3 * n; ++i) O[i] = std::fma(S[i / 3], D[i], P[i]);
+    } else return ORACLE_INVALID_ARGUMENT;
+    return ORACLE_OK;
+}
+
+int oracle_source_sample(int precision, const oracle_source_t* src, uint64_t seed, int64_t first_id, int64_t n,
+                         double* pos_out, double* dir_out, double* e_out, int32_t* ndraws_out) {
+    if (!src) return ORACLE_INVALID_ARGUMENT;
+    if (precision == 64) {
+        SourceR<double> s; if (!make_source(*src, s)) return ORACLE_INVALID_ARGUMENT;
+        for (int64_t i = 0; i < n; ++i) {
+            Stream r{seed, (uint64_t)(first_id + i), 0}; double x[3], w[3], E; sample_source(s, r, x, w, E);
+            for (int k = 0; k < 3; ++k) { pos_out[3 * i + k] = x[k]; dir_out[3 * i + k] = w[k]; }
+            e_out[i] = E; if (ndraws_out) ndraws_out[i] = (int32_t)r.j;
+        }
+    } else {
+        SourceR<float> s; if (!make_source(*src, s)) return ORACLE_INVALID_ARGUMENT;
+        for (int64_t i = 0; i < n; ++i) {
+            Stream r{seed, (uint64_t)(first_id + i), 0}; float x[3], w[3], E; sample_source(s, r, x, w, E);
+            for (int k = 0; k < 3; ++k) { pos_out[3 * i + k] = x[k]; dir_out[3 * i + k] = w[k]; }
+            e_out[i] = E; if (ndraws_out) ndraws_out[i] = (int32_t)r.j;
+        }
+    }
+    return ORACLE_OK;
+}
+
+}  // extern "C"
