@@ -1,0 +1,153 @@
+/*
+ * gammanav.h -- C ABI of the B200-native gamma transport / Geant4-style navigation library
+ * (libgammanav.so, hand-written CUDA for sm_100a; no CPU fallback).
+ *
+ * The four entry points follow the paper's statement of the problem:
+ *   - "Load the geometry and transfer it to GPU memory"            PAPER.md L139 (Algorithm 2, phase 1)  -> gn_geometry_create
+ *   - "If a particle is in point A, inside which ... volumes is it?" PAPER.md L124                        -> gn_nav_locate
+ *   - "Will the particle hit a volume boundary ... on its way to point B? If so, where"  PAPER.md L125   -> gn_nav_compute_step
+ *   - Algorithm 1 run for N particles in parallel (Algorithm 2 phase 5, L143),
+ *     generalised to Compton / photoelectric / pair sampling with a per-volume energy tally
+ *     (BASELINE.json north_star)                                                   -> gn_transport_run
+ *
+ * Conventions: lengths mm, energies MeV, densities g/cm3.  `precision` is 32 or 64 and selects the
+ * element type (float / double) of every `void*` Real buffer and the arithmetic of the kernels.
+ * Pointers named h_* are HOST memory, d_* are DEVICE memory (caller-owned, never retained).
+ * Positions / directions at the ABI are row-major n x 3 (x0 y0 z0 x1 ...).
+ * Every function returns GN_OK (0) or a negative gn_status; nothing throws or aborts, and outputs are
+ * untouched on failure.  gn_last_error() gives a human-readable string for the calling thread's last failure.
+ * All nav calls are asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream);
+ * gn_transport_run synchronises the stream before it fills the host stats.
+ */
+#ifndef GAMMANAV_H
+#define GAMMANAV_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GN_OK = 0,
+    GN_INVALID_ARGUMENT = -1,   /* NULL / negative sizes / bad precision / index out of range */
+    GN_UNSUPPORTED_SOLID = -2,  /* unknown type, or tube with pi < dphi < 2 pi (non-convex sector) */
+    GN_BAD_TREE = -3,           /* node 0 not the world, parent >= child, R not orthonormal (1e-9) */
+    GN_OUT_OF_MEMORY = -4,
+    GN_CUDA_ERROR = -5
+} gn_status;
+
+enum { GN_BOX = 0, GN_TUBE = 1 };
+enum { GN_SRC_PENCIL = 0, GN_SRC_GAUSS_PENCIL = 1, GN_SRC_CONE = 2, GN_SRC_ISOTROPIC = 3 };
+enum { GN_E_MONO = 0, GN_E_LOGUNIFORM = 1 };
+
+typedef struct gn_geometry gn_geometry;   /* opaque; owns all device allocations of one geometry */
+
+/* Options (all fields: <= 0 selects the default).  SURVEY 8(c) C0, C5, C6, C9. */
+typedef struct {
+    double tol64;              /* surface tolerance in fp64 mode [mm]; default 1e-9 */
+    double tol32;              /* surface tolerance in fp32 mode [mm]; default (largest world half-extent) * 2^-18 */
+    double sigma_pe0;          /* photoelectric cross-section of Z = 82 at 0.1 MeV [barn/atom]; default 1750 */
+    double e_cut;              /* photons below this energy are absorbed locally [MeV]; default 0.010 */
+    int32_t voxel_min_daughters; /* mothers with at least this many daughters get a voxel grid; default 8 */
+    int32_t stuck_limit;       /* consecutive steps of length <= tol/2 before a photon is killed; default 8 */
+    int32_t steps_per_pass;    /* K: steps a photon takes per wavefront pass before it is re-queued; default 16 */
+    int32_t reserved;
+} gn_opts;
+
+/* Photon source.  axis need not be normalised. */
+typedef struct {
+    int32_t kind;              /* GN_SRC_* */
+    int32_t energy_kind;       /* GN_E_*   */
+    double origin[3];          /* mm */
+    double axis[3];
+    double sigma;              /* GN_SRC_GAUSS_PENCIL: lateral Gaussian sigma [mm] */
+    double half_angle;         /* GN_SRC_CONE: half opening angle [rad], uniform in solid angle */
+    double e0, e1;             /* MONO: e0; LOGUNIFORM: uniform in ln E over [e0, e1] */
+} gn_source;
+
+/* Run statistics (host).  n_steps = number of ComputeStep calls = the "photon steps" of BASELINE.json's metric. */
+typedef struct {
+    uint64_t n_steps, n_compton, n_pe, n_pair, n_cut, n_escaped, n_stuck, n_photons;
+    double e_escaped, e_stuck, e_source, e_deposited;
+    uint64_t n_passes;         /* wavefront passes (kernel launches of the step kernel) */
+    uint64_t n_kernel_launches;/* all kernels launched by the call */
+} gn_run_stats;
+
+/*
+ * gn_geometry_create -- PAPER.md L139 / L127 (volumes hierarchy, solids, per-material density).
+ *   h_materials    n_mats x 3 doubles: Z, A [g/mol], rho [g/cm3]
+ *   h_solid_type   n_solids int32: GN_BOX | GN_TUBE
+ *   h_solid_params n_solids x 5 doubles: BOX hx,hy,hz,-,- ; TUBE rmin,rmax,hz,sphi,dphi  (C2; dphi >= 2 pi
+ *                  = full tube, 0 < dphi <= pi = convex sector)
+ *   h_placements   n_places x 4 int32: parent (-1 for node 0 = world, parent < child), solid, material,
+ *                  transform index.  Every node is its own touchable: volume index = node index (C1).
+ *   h_transforms   n_transforms x 12 doubles: R row-major (local -> parent) then T [mm]   (C0)
+ *   h_opts         NULL = defaults
+ * All input arrays are host memory, copied during the call.  The handle owns its device memory
+ * (structure-of-arrays store: node records, composed global->local affine transforms in fp32 and fp64,
+ * solids, material factors, flattened voxel grids) until gn_geometry_destroy.
+ * Overlapping / protruding daughters are not detected (Geant4 convention).
+ */
+int gn_geometry_create(const double* h_materials, int32_t n_mats,
+                       const int32_t* h_solid_type, const double* h_solid_params, int32_t n_solids,
+                       const int32_t* h_placements, int32_t n_places,
+                       const double* h_transforms, int32_t n_transforms,
+                       const gn_opts* h_opts, gn_geometry** out);
+int gn_geometry_destroy(gn_geometry* geo);
+
+/* geometry queries (host side, cheap) */
+int32_t gn_geometry_num_places(const gn_geometry* geo);
+double gn_geometry_tolerance(const gn_geometry* geo, int precision);
+/* voxel store summary: info[0] = number of voxelised mothers, [1] = total cells, [2] = total candidate
+ * references, [3] = bytes of device memory held by the geometry */
+int gn_geometry_voxel_info(const gn_geometry* geo, int64_t info[4]);
+
+/*
+ * gn_nav_locate -- PAPER.md L124; SURVEY 8(c) C3.
+ *   d_pos n x 3 Real, d_dir n x 3 Real or NULL (NULL: a point on a surface counts as inside),
+ *   d_vol_out n int32: deepest volume occupied, -1 = outside the world.
+ */
+int gn_nav_locate(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir,
+                  int64_t n, int32_t* d_vol_out, void* cuda_stream);
+
+/*
+ * gn_nav_compute_step -- PAPER.md L125; SURVEY 8(c) C4.
+ *   d_vol_in n int32 (as returned by gn_nav_locate; -1 gives (+inf, -1)),
+ *   d_max_step n Real or NULL (= +inf): if the nearest boundary is farther than max_step the result is
+ *   (+inf, vol_in),
+ *   d_step_out n Real: distance to the nearest boundary (DistanceToOut of the current solid, DistanceToIn of
+ *   its daughters via the voxel grid), d_next_vol_out n int32: the volume occupied just after the boundary
+ *   (-1 = left the world).
+ */
+int gn_nav_compute_step(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir,
+                        const int32_t* d_vol_in, const void* d_max_step, int64_t n,
+                        void* d_step_out, int32_t* d_next_vol_out, void* cuda_stream);
+
+/*
+ * gn_transport_run -- PAPER.md Algorithm 1 (L55-76) for photons first_photon_id .. first_photon_id + n - 1,
+ * each with its own Philox4x32-10 stream keyed by (seed, photon id).
+ *   d_edep_out    gn_geometry_num_places doubles [MeV]; ZEROED by the callee, then accumulated (fp64 atomics)
+ *   h_stats_out   host, may be NULL
+ *   d_hash_out    n uint64 history hashes (FNV-1a-64 over (volume, event) per step), or NULL
+ *   d_nsteps_out  n uint32 steps per photon, or NULL
+ *   d_efinal_out  n doubles: photon energy when it terminated, or NULL
+ * Scratch (two photon-state queues, 2 x n x 48 B in fp32 / 80 B in fp64, plus counters) is allocated from
+ * the CUDA stream-ordered pool and released before return.
+ */
+int gn_transport_run(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
+                     int64_t first_photon_id, int64_t n_photons,
+                     double* d_edep_out, gn_run_stats* h_stats_out,
+                     uint64_t* d_hash_out, uint32_t* d_nsteps_out, double* d_efinal_out, void* cuda_stream);
+
+/* Host-buffer convenience wrappers (the "end to end" path: copies host<->device inside the call). */
+int gn_nav_query_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, int64_t n,
+                      int32_t* h_vol_out, void* h_step_out, int32_t* h_next_vol_out);
+int gn_transport_run_host(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
+                          int64_t first_photon_id, int64_t n_photons, double* h_edep_out, gn_run_stats* h_stats_out);
+
+const char* gn_last_error(void);
+const char* gn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,330 @@
+// geometry.cu -- gn_geometry_create / destroy: validate the placement tree, compose the affine transforms
+// root-down in fp64, build the flattened voxel grids (C5) and upload the
+// structure-of-arrays store (store.h) in both precisions.  Host code only; "Load the geometry
+// and transfer it to GPU memory".
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <vector>
+#include "geometry.h"
+
+namespace gn {
+
+static thread_local std::string g_last_error;
+void set_error(const std::string& msg) { g_last_error = msg; }
+int fail(int code, const std::string& msg) { g_last_error = msg; return code; }
+const char* last_error_cstr() { return g_last_error.c_str(); }
+
+namespace {
+
+const double kRe = 2.8179403262e-13, kAlpha = 7.2973525693e-3, kNA = 6.02214076e23, kBarn = 1e-24;
+const double kPi = 3.14159265358979323846;
+
+struct HostSolid { int type; double a, b, c, sphi, dphi; bool sector; double cS, sS, cE, sE; };
+
+struct Uploader {
+    gn_geometry* geo; bool ok = true; std::string err;
+    template <class T> const T* put(const std::vector<T>& v) {
+        if (!ok) return nullptr;
+        void* d = nullptr;
+        size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(T);
+        cudaError_t e = cudaMalloc(&d, bytes);
+        if (e != cudaSuccess) { ok = false; err = std::string("cudaMalloc: ") + cudaGetErrorString(e); return nullptr; }
+        geo->allocations.push_back(d); geo->device_bytes += (int64_t)bytes;
+        if (!v.empty()) {
+            e = cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { ok = false; err = std::string("cudaMemcpy: ") + cudaGetErrorString(e); return nullptr; }
+        }
+        return static_cast<const T*>(d);
+    }
+};
+
+// axis-aligned bounds of an annular sector r in [r0, r1], phi in [p0, p1]
+void sector_bounds(double r0, double r1, double p0, double p1, double lo[2], double hi[2]) {
+    double xs[12], ys[12]; int n = 0;
+    const double ang[2] = {p0, p1}, rr[2] = {r0, r1};
+    for (int i = 0; i < 2; ++i) for (int j = 0; j < 2; ++j) { xs[n] = rr[j] * std::cos(ang[i]); ys[n] = rr[j] * std::sin(ang[i]); ++n; }
+    int k0 = (int)std::ceil(p0 / (kPi / 2) - 1e-12), k1 = (int)std::floor(p1 / (kPi / 2) + 1e-12);
+    for (int k = k0; k <= k1 && n < 12; ++k) { xs[n] = r1 * std::cos(k * (kPi / 2)); ys[n] = r1 * std::sin(k * (kPi / 2)); ++n; }
+    lo[0] = hi[0] = xs[0]; lo[1] = hi[1] = ys[0];
+    for (int i = 1; i < n; ++i) { lo[0] = std::min(lo[0], xs[i]); hi[0] = std::max(hi[0], xs[i]); lo[1] = std::min(lo[1], ys[i]); hi[1] = std::max(hi[1], ys[i]); }
+    double pad = 1e-9 * r1;
+    lo[0] -= pad; lo[1] -= pad; hi[0] += pad; hi[1] += pad;
+}
+
+// bounds of a placed daughter in its mother's frame (R, T: local -> mother)
+void daughter_bounds(const HostSolid& s, const double* R, const double* T, double lo[3], double hi[3]) {
+    if (s.type == GN_TUBE && s.sector && std::fabs(R[8] - 1.0) < 1e-12 && std::fabs(R[0] * R[4] - R[1] * R[3] - 1.0) < 1e-9) {
+        // rotation about z: the sector stays a sector, shifted in angle -- exact bounds
+        double th = std::atan2(R[3], R[0]);
+        double l2[2], h2[2];
+        sector_bounds(s.a, s.b, s.sphi + th, s.sphi + s.dphi + th, l2, h2);
+        lo[0] = l2[0] + T[0]; hi[0] = h2[0] + T[0]; lo[1] = l2[1] + T[1]; hi[1] = h2[1] + T[1];
+        lo[2] = T[2] - s.c; hi[2] = T[2] + s.c;
+        return;
+    }
+    double l[3], h[3];
+    if (s.type == GN_BOX) { l[0] = -s.a; h[0] = s.a; l[1] = -s.b; h[1] = s.b; l[2] = -s.c; h[2] = s.c; }
+    else {
+        l[2] = -s.c; h[2] = s.c;
+        if (s.sector) sector_bounds(s.a, s.b, s.sphi, s.sphi + s.dphi, l, h);
+        else { l[0] = l[1] = -s.b; h[0] = h[1] = s.b; }
+    }
+    for (int k = 0; k < 3; ++k) { lo[k] = 1e300; hi[k] = -1e300; }
+    for (int c = 0; c < 8; ++c) {
+        double q[3] = {(c & 1) ? h[0] : l[0], (c & 2) ? h[1] : l[1], (c & 4) ? h[2] : l[2]};
+        for (int k = 0; k < 3; ++k) {
+            double y = R[3 * k] * q[0] + R[3 * k + 1] * q[1] + R[3 * k + 2] * q[2] + T[k];
+            lo[k] = std::min(lo[k], y); hi[k] = std::max(hi[k], y);
+        }
+    }
+}
+
+template <class R> SolidRec<R> make_solid_rec(const HostSolid& s) {
+    SolidRec<R> o;
+    o.a = (R)s.a; o.b = (R)s.b; o.c = (R)s.c; o.cS = (R)s.cS; o.sS = (R)s.sS; o.cE = (R)s.cE; o.sE = (R)s.sE;
+    o.type = s.type == GN_BOX ? SOLID_BOX : SOLID_TUBE;
+    o.flags = 0;
+    if (s.type == GN_TUBE) { if (s.sector) o.flags |= TUBE_SECTOR; if (o.a > 0) o.flags |= TUBE_HOLE; }
+    return o;
+}
+
+template <class R> MatRec<R> make_mat_rec(double Z, double A, double rho, double s0) {
+    double n = rho * kNA / A;                        // atoms / cm^3; mu [1/mm] = n sigma / 10
+    MatRec<R> o;
+    o.aPE = (R)(n * (s0 * kBarn * std::pow(Z / 82.0, 5.0)) / 10.0);
+    o.aC = (R)(n * (Z * (2.0 * kPi * kRe * kRe)) / 10.0);
+    o.aP = (R)(n * (kAlpha * kRe * kRe * Z * Z) / 10.0);
+    o.capZ = (R)((28.0 / 9.0) * std::log(183.0 * std::pow(Z, -1.0 / 3.0)) - 2.0 / 27.0);
+    return o;
+}
+
+struct HostGrid { int n[3]; double gmin[3], w[3]; int cell_base; };
+
+}  // namespace
+}  // namespace gn
+
+using namespace gn;
+
+extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, const int32_t* h_solid_type,
+                                  const double* h_solid_params, int32_t n_solids, const int32_t* h_placements,
+                                  int32_t n_places, const double* h_transforms, int32_t n_transforms,
+                                  const gn_opts* h_opts, gn_geometry** out) {
+    if (!h_materials || !h_solid_type || !h_solid_params || !h_placements || !h_transforms || !out)
+        return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: NULL argument");
+    if (n_mats <= 0 || n_solids <= 0 || n_places <= 0 || n_transforms <= 0)
+        return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: empty table");
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) {
+        cudaGetLastError();
+        return fail(GN_CUDA_ERROR, "gn_geometry_create: no CUDA device (this library has no CPU fallback)");
+    }
+    for (int i = 0; i < n_mats; ++i) {
+        double Z = h_materials[3 * i], A = h_materials[3 * i + 1], rho = h_materials[3 * i + 2];
+        if (!(Z > 0 && A > 0 && rho >= 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: material needs Z > 0, A > 0, rho >= 0");
+    }
+    std::vector<HostSolid> solids(n_solids);
+    for (int i = 0; i < n_solids; ++i) {
+        const double* p = h_solid_params + 5 * (size_t)i;
+        HostSolid& s = solids[i];
+        s.type = h_solid_type[i]; s.sector = false; s.cS = s.sS = s.cE = s.sE = 0; s.sphi = s.dphi = 0;
+        s.a = p[0]; s.b = p[1]; s.c = p[2];
+        if (s.type == GN_BOX) {
+            if (!(s.a > 0 && s.b > 0 && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: box half-lengths must be positive");
+        } else if (s.type == GN_TUBE) {
+            s.sphi = p[3]; s.dphi = p[4];
+            if (!(s.a >= 0 && s.b > s.a && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: tube needs 0 <= rmin < rmax, hz > 0");
+            if (s.dphi < 2 * kPi) {
+                if (!(s.dphi > 0) || s.dphi > kPi) return fail(GN_UNSUPPORTED_SOLID, "gn_geometry_create: tube sector must have 0 < dphi <= pi (or a full tube)");
+                s.sector = true;
+                s.cS = std::cos(s.sphi); s.sS = std::sin(s.sphi);
+                s.cE = std::cos(s.sphi + s.dphi); s.sE = std::sin(s.sphi + s.dphi);
+            }
+        } else return fail(GN_UNSUPPORTED_SOLID, "gn_geometry_create: unknown solid type");
+    }
+    const size_t V = (size_t)n_places;
+    std::vector<int4> node(V);
+    std::vector<double> Rg(9 * V), Tg(3 * V);
+    std::vector<int> kid_count(V, 0);
+    for (size_t i = 0; i < V; ++i) {
+        int p = h_placements[4 * i], s = h_placements[4 * i + 1], m = h_placements[4 * i + 2], t = h_placements[4 * i + 3];
+        if (s < 0 || s >= n_solids || m < 0 || m >= n_mats || t < 0 || t >= n_transforms)
+            return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: placement index out of range");
+        if ((i == 0 && p != -1) || (i > 0 && (p < 0 || (size_t)p >= i)))
+            return fail(GN_BAD_TREE, "gn_geometry_create: node 0 must be the world and parent < child");
+        const double* Rl = h_transforms + 12 * (size_t)t; const double* Tl = Rl + 9;
+        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) {
+            double dot = Rl[3 * a] * Rl[3 * b] + Rl[3 * a + 1] * Rl[3 * b + 1] + Rl[3 * a + 2] * Rl[3 * b + 2];
+            if (std::fabs(dot - (a == b ? 1.0 : 0.0)) > 1e-9) return fail(GN_BAD_TREE, "gn_geometry_create: rotation not orthonormal");
+        }
+        node[i] = make_int4(p, s, m, -1);
+        double* R = &Rg[9 * i]; double* T = &Tg[3 * i];
+        if (p < 0) { std::memcpy(R, Rl, 9 * sizeof(double)); std::memcpy(T, Tl, 3 * sizeof(double)); }
+        else {
+            // C0: Rg = Rg_parent R, Tg = Rg_parent T + Tg_parent, left to right, fp64
+            const double* Rp = &Rg[9 * (size_t)p]; const double* Tp = &Tg[3 * (size_t)p];
+            for (int a = 0; a < 3; ++a) {
+                for (int b = 0; b < 3; ++b) R[3 * a + b] = (Rp[3 * a] * Rl[b] + Rp[3 * a + 1] * Rl[3 + b]) + Rp[3 * a + 2] * Rl[6 + b];
+                T[a] = ((Rp[3 * a] * Tl[0] + Rp[3 * a + 1] * Tl[1]) + Rp[3 * a + 2] * Tl[2]) + Tp[a];
+            }
+            kid_count[p]++;
+        }
+    }
+    // daughters in index order (CSR)
+    std::vector<int2> kids(V);
+    std::vector<int> dlist(V > 1 ? V - 1 : 0);
+    { int acc = 0; for (size_t i = 0; i < V; ++i) { kids[i] = make_int2(acc, 0); acc += kid_count[i]; } }
+    for (size_t i = 1; i < V; ++i) { int p = node[i].x; dlist[kids[p].x + kids[p].y] = (int)i; kids[p].y++; }
+
+    gn_geometry* geo = new gn_geometry();
+    geo->n_places = n_places; geo->n_solids = n_solids; geo->n_mats = n_mats;
+    cudaGetDevice(&geo->device);
+    gn_opts o{}; if (h_opts) o = *h_opts;
+    const HostSolid& ws = solids[node[0].y];
+    double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : std::max(ws.b, ws.c);
+    geo->tol64 = o.tol64 > 0 ? o.tol64 : 1e-9;
+    geo->tol32 = o.tol32 > 0 ? o.tol32 : (double)(float)(ext * 0x1p-18);
+    if (!(o.sigma_pe0 > 0)) o.sigma_pe0 = 1750.0;
+    if (!(o.e_cut > 0)) o.e_cut = 0.010;
+    if (o.voxel_min_daughters <= 0) o.voxel_min_daughters = 8;
+    if (o.stuck_limit <= 0) o.stuck_limit = 8;
+    if (o.steps_per_pass <= 0) o.steps_per_pass = 16;
+    o.tol64 = geo->tol64; o.tol32 = geo->tol32;
+    geo->opts = o;
+
+    // ---- voxel grids (C5): one uniform 3-D grid per mother = three nested levels of uniform slices, flattened
+    std::vector<HostGrid> grids;
+    std::vector<int> cell_start(1, 0), cand;
+    const double shrink = geo->tol64 / 8;
+    for (size_t mth = 0; mth < V; ++mth) {
+        int nd = kids[mth].y;
+        if (nd < o.voxel_min_daughters) continue;
+        const HostSolid& ms = solids[node[mth].y];
+        double mlo[3], mhi[3];
+        if (ms.type == GN_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; }
+        else { mlo[0] = mlo[1] = -ms.b; mhi[0] = mhi[1] = ms.b; }
+        mlo[2] = -ms.c; mhi[2] = ms.c;
+        std::vector<double> blo(3 * (size_t)nd), bhi(3 * (size_t)nd);
+        double minext[3] = {1e300, 1e300, 1e300};
+        for (int j = 0; j < nd; ++j) {
+            int d = dlist[kids[mth].x + j];
+            int t = h_placements[4 * (size_t)d + 3];
+            const double* Rl = h_transforms + 12 * (size_t)t;
+            daughter_bounds(solids[node[d].y], Rl, Rl + 9, &blo[3 * (size_t)j], &bhi[3 * (size_t)j]);
+            for (int k = 0; k < 3; ++k) minext[k] = std::min(minext[k], bhi[3 * (size_t)j + k] - blo[3 * (size_t)j + k]);
+        }
+        HostGrid G;
+        double budget = std::max(8.0 * nd, 4096.0);
+        for (int k = 0; k < 3; ++k) {
+            double L = mhi[k] - mlo[k];
+            double f = std::floor(L / std::max(minext[k], L / 1024.0) + 1e-9);
+            G.n[k] = (int)std::min(std::max(f, 1.0), 1024.0);
+        }
+        while ((double)G.n[0] * G.n[1] * G.n[2] > budget) {
+            int k = (G.n[0] >= G.n[1] && G.n[0] >= G.n[2]) ? 0 : (G.n[1] >= G.n[2] ? 1 : 2);
+            G.n[k] = (G.n[k] + 1) / 2;
+        }
+        for (int k = 0; k < 3; ++k) { G.gmin[k] = mlo[k]; G.w[k] = (mhi[k] - mlo[k]) / G.n[k]; }
+        size_t ncell = (size_t)G.n[0] * G.n[1] * G.n[2];
+        G.cell_base = (int)cell_start.size() - 1;
+        std::vector<int> count(ncell, 0);
+        std::vector<int> c0(3 * (size_t)nd), c1(3 * (size_t)nd);
+        for (int j = 0; j < nd; ++j) {
+            for (int k = 0; k < 3; ++k) {
+                double top = G.n[k] - 1.0;
+                double a = std::floor((blo[3 * (size_t)j + k] + shrink - G.gmin[k]) / G.w[k]);
+                double b = std::floor((bhi[3 * (size_t)j + k] - shrink - G.gmin[k]) / G.w[k]);
+                a = std::min(std::max(a, 0.0), top); b = std::min(std::max(b, 0.0), top);
+                if (b < a) b = a;
+                c0[3 * (size_t)j + k] = (int)a; c1[3 * (size_t)j + k] = (int)b;
+            }
+            for (int iz = c0[3 * (size_t)j + 2]; iz <= c1[3 * (size_t)j + 2]; ++iz)
+                for (int iy = c0[3 * (size_t)j + 1]; iy <= c1[3 * (size_t)j + 1]; ++iy)
+                    for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
+                        count[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++;
+        }
+        size_t base = cand.size();
+        std::vector<size_t> pos(ncell);
+        { size_t acc = base; for (size_t c = 0; c < ncell; ++c) { pos[c] = acc; acc += count[c]; cell_start.push_back((int)acc); } cand.resize(acc); }
+        for (int j = 0; j < nd; ++j) {           // j ascending = daughter index ascending -> lists stay sorted
+            int d = dlist[kids[mth].x + j];
+            for (int iz = c0[3 * (size_t)j + 2]; iz <= c1[3 * (size_t)j + 2]; ++iz)
+                for (int iy = c0[3 * (size_t)j + 1]; iy <= c1[3 * (size_t)j + 1]; ++iy)
+                    for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
+                        cand[pos[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++] = d;
+        }
+        node[mth].w = (int)grids.size();
+        grids.push_back(G);
+        geo->n_cells += (int64_t)ncell;
+    }
+    geo->n_grids = (int64_t)grids.size(); geo->n_cand = (int64_t)cand.size();
+
+    // ---- per-precision tables
+    std::vector<float> xf32(12 * V); std::vector<double> xf64(12 * V);
+    for (size_t i = 0; i < V; ++i) {
+        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) {            // M = Rg^T
+            xf64[12 * i + 3 * a + b] = Rg[9 * i + 3 * b + a]; xf32[12 * i + 3 * a + b] = (float)Rg[9 * i + 3 * b + a];
+        }
+        for (int a = 0; a < 3; ++a) { xf64[12 * i + 9 + a] = Tg[3 * i + a]; xf32[12 * i + 9 + a] = (float)Tg[3 * i + a]; }
+    }
+    std::vector<SolidRec<float>> s32; std::vector<SolidRec<double>> s64;
+    for (const HostSolid& s : solids) { s32.push_back(make_solid_rec<float>(s)); s64.push_back(make_solid_rec<double>(s)); }
+    std::vector<MatRec<float>> m32; std::vector<MatRec<double>> m64;
+    for (int i = 0; i < n_mats; ++i) {
+        m32.push_back(make_mat_rec<float>(h_materials[3 * i], h_materials[3 * i + 1], h_materials[3 * i + 2], o.sigma_pe0));
+        m64.push_back(make_mat_rec<double>(h_materials[3 * i], h_materials[3 * i + 1], h_materials[3 * i + 2], o.sigma_pe0));
+    }
+    std::vector<GridRec<float>> g32; std::vector<GridRec<double>> g64;
+    for (const HostGrid& G : grids) {
+        GridRec<float> a; GridRec<double> b;
+        for (int k = 0; k < 3; ++k) {
+            a.gmin[k] = (float)G.gmin[k]; a.w[k] = (float)G.w[k]; a.inv_w[k] = (float)(1.0 / G.w[k]); a.n[k] = G.n[k];
+            b.gmin[k] = G.gmin[k]; b.w[k] = G.w[k]; b.inv_w[k] = 1.0 / G.w[k]; b.n[k] = G.n[k];
+        }
+        a.cell_base = b.cell_base = G.cell_base;
+        g32.push_back(a); g64.push_back(b);
+    }
+
+    Uploader up{geo};
+    const int4* d_node = up.put(node); const int2* d_kids = up.put(kids); const int* d_dlist = up.put(dlist);
+    const int* d_cs = up.put(cell_start); const int* d_cand = up.put(cand);
+    GeoView<float>& a = geo->v32; GeoView<double>& b = geo->v64;
+    a.node = b.node = d_node; a.kids = b.kids = d_kids; a.dlist = b.dlist = d_dlist; a.cell_start = b.cell_start = d_cs; a.cand = b.cand = d_cand;
+    a.xf = up.put(xf32); b.xf = up.put(xf64);
+    a.solids = up.put(s32); b.solids = up.put(s64);
+    a.mats = up.put(m32); b.mats = up.put(m64);
+    a.grids = up.put(g32); b.grids = up.put(g64);
+    a.tol = (float)geo->tol32; a.delta = a.tol / 2; a.probe = std::max(a.tol, (float)(ext * 0x1p-18)); a.e_cut = (float)o.e_cut;
+    b.tol = geo->tol64; b.delta = b.tol / 2; b.probe = b.tol; b.e_cut = o.e_cut;
+    a.n_nodes = b.n_nodes = n_places; a.n_solids = b.n_solids = n_solids; a.n_mats = b.n_mats = n_mats;
+    a.stuck_limit = b.stuck_limit = o.stuck_limit;
+    if (!up.ok) {
+        std::string e = up.err;
+        gn_geometry_destroy(geo);
+        return fail(e.find("cudaMalloc") == 0 ? GN_OUT_OF_MEMORY : GN_CUDA_ERROR, "gn_geometry_create: " + e);
+    }
+    *out = geo;
+    return GN_OK;
+}
+
+extern "C" int gn_geometry_destroy(gn_geometry* geo) {
+    if (!geo) return GN_OK;
+    for (void* p : geo->allocations) cudaFree(p);
+    delete geo;
+    return GN_OK;
+}
+
+extern "C" int32_t gn_geometry_num_places(const gn_geometry* geo) { return geo ? geo->n_places : 0; }
+extern "C" double gn_geometry_tolerance(const gn_geometry* geo, int precision) {
+    if (!geo) return 0.0;
+    return precision == 32 ? geo->tol32 : geo->tol64;
+}
+extern "C" int gn_geometry_voxel_info(const gn_geometry* geo, int64_t info[4]) {
+    if (!geo || !info) return fail(GN_INVALID_ARGUMENT, "gn_geometry_voxel_info: NULL argument");
+    info[0] = geo->n_grids; info[1] = geo->n_cells; info[2] = geo->n_cand; info[3] = geo->device_bytes;
+    return GN_OK;
+}
+namespace gn { const char* last_error_cstr(); }
+extern "C" const char* gn_last_error(void) { return gn::last_error_cstr(); }
+extern "C" const char* gn_version(void) { return "gammanav 0.1 (sm_100a)"; }

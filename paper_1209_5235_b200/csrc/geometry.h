@@ -1,0 +1,22 @@
+// geometry.h -- the opaque gn_geometry handle (host side) shared by geometry.cu and kernels.cu
+#pragma once
+#include <string>
+#include <vector>
+#include "store.h"
+#include "../../include/gammanav.h"
+
+struct gn_geometry {
+    gn::GeoView<float> v32{};
+    gn::GeoView<double> v64{};
+    std::vector<void*> allocations;      // every cudaMalloc owned by the handle
+    int32_t n_places = 0, n_solids = 0, n_mats = 0;
+    double tol32 = 0, tol64 = 0;
+    gn_opts opts{};
+    int64_t n_grids = 0, n_cells = 0, n_cand = 0, device_bytes = 0;
+    int device = 0;
+};
+
+namespace gn {
+void set_error(const std::string& msg);
+int fail(int code, const std::string& msg);
+}
