@@ -1,0 +1,320 @@
+"""bench.py -- BASELINE.json's metric on its named workload, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3|1|2|4|5]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one gn_transport_run of the
+workload (config 3 by default: 64^3 voxel phantom, 1e7 photons of 6 MeV from a 5-degree cone, fp32 -- the
+configuration BASELINE.json's north_star quotes the target on), or for config 5 one gn_nav_locate +
+gn_nav_compute_step over the query batch.  metric = transported photon steps/s (ComputeStep queries/s for
+config 5).  Multi-GPU (torchrun, one rank per GPU): weak scaling, every rank transports its own contiguous
+photon-id range of the same size on a replicated geometry; the per-volume tally is all-reduced (NCCL) at the
+end of each step, inside the timed region.
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+ALGO_BYTES = {("transport", 32): 96.0, ("transport", 64): 160.0, ("nav", 32): 64.0, ("nav", 64): 116.0}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        self.lines, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def workload(k):
+    from paper_1209_5235_b200 import workloads as W
+    wl = W.config(k)
+    precision = 32 if 32 in wl.precisions else 64
+    return wl, precision
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def _oracle_worker(args):
+    k, precision, first, count = args
+    import oracle
+    from paper_1209_5235_b200 import workloads as W
+    wl = W.config(k)
+    og = oracle.OracleGeometry(wl.geometry)
+    t = time.perf_counter()
+    if wl.source is not None:
+        r = og.transport(wl.source, wl.seed, count, precision, first_id=first)
+        units = r["stats"]["n_steps"]
+    else:
+        R = np.float32 if precision == 32 else np.float64
+        pos, dirs = W.nav_queries(wl.geometry, count, seed=wl.seed, dtype=R, first=first)
+        t = time.perf_counter()
+        vol = og.locate(pos, dirs, precision); og.compute_step(pos, dirs, vol, None, precision)
+        units = count
+    return units, time.perf_counter() - t
+
+
+def oracle_rate(k, precision, sample, cores=1):
+    """units/s of the oracle as it stands on `cores` host cores (independent workers over disjoint id ranges,
+    as the paper's OpenMP-over-particles version)."""
+    if cores == 1:
+        units, dt = _oracle_worker((k, precision, 0, sample))
+        return units / dt, units, dt
+    import multiprocessing as mp
+    per = sample // cores
+    with mp.get_context("spawn").Pool(cores) as pool:
+        t = time.perf_counter()
+        res = pool.map(_oracle_worker, [(k, precision, i * per, per) for i in range(cores)])
+        wall = time.perf_counter() - t
+    units = sum(u for u, _ in res)
+    dt = max(d for _, d in res)            # excludes geometry construction, like the GPU side
+    return units / dt, units, wall
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl, precision = workload(args.config)
+    sample = {1: 10000, 2: 20000, 3: 100000, 4: 50000, 5: 300000}[args.config]
+    _oracle_worker((args.config, precision, 0, max(1, sample // 10)))          # page in, build lib
+    times, units = [], 0
+    for _ in range(args.warmup):
+        _oracle_worker((args.config, precision, 0, max(1, sample // 10)))
+    for s in range(args.steps):
+        u, dt = _oracle_worker((args.config, precision, s * sample, sample))
+        units += u; times.append(dt)
+    total = sum(times)
+    value = units / total
+    unit = "photon-steps/s" if wl.source is not None else "ComputeStep queries/s"
+    line = {"impl": "reference", "metric": "transported photon steps/s" if wl.source is not None else "ComputeStep queries/s",
+            "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if precision == 32 else "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "precision": precision, "sample_per_step": sample},
+            "cpu_baseline": {"value": value, "unit": unit, "cores": 1, "kind": "oracle",
+                             "sample": f"{sample} of {wl.n} {'photons' if wl.source is not None else 'queries'} per step, single thread"},
+            "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1209_5235_b200 import binding as B, build as lib_build, workloads as W
+    from paper_1209_5235_b200.sharding import allreduce_tally
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        lib_build.build()
+    if world > 1:
+        dist.barrier()
+    wl, precision = workload(args.config)
+    if args.precision:
+        precision = args.precision
+    n = int(wl.n * args.scale)
+    geo = B.Geometry(wl.geometry, **({"steps_per_pass": args.steps_per_pass} if args.steps_per_pass else {}))
+    transport = wl.source is not None
+    first_id = rank * n                                       # weak scaling: same work per GPU, disjoint ids
+    dev = torch.device("cuda", local)
+    if transport:
+        edep = torch.empty(geo.n_places, dtype=torch.float64, device=dev)
+
+        def step():
+            r = B.transport_run(geo, wl.source, wl.seed, n, precision, first_photon_id=first_id, edep=edep)
+            st = r["stats"]
+            if world > 1:
+                allreduce_tally(edep, st)
+            return st["n_steps"], st["n_kernel_launches"], st["kernel_ms"]
+    else:
+        rdt = torch.float32 if precision == 32 else torch.float64
+        pos, dirs = W.nav_queries_torch(wl.geometry, n, wl.seed + 1000 * rank, rdt, dev)
+        vol = torch.empty(n, dtype=torch.int32, device=dev)
+        out = (torch.empty(n, dtype=rdt, device=dev), torch.empty(n, dtype=torch.int32, device=dev))
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+
+        def step():
+            ev[0].record()
+            B.nav_locate(geo, pos, dirs, out=vol)
+            B.nav_compute_step(geo, pos, dirs, vol, out=out)
+            ev[1].record(); ev[1].synchronize()
+            return n, 2, ev[0].elapsed_time(ev[1])
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3) if not args.allow_short_warmup else args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    units = launches = 0; kernel_ms = 0.0
+    e0.record()
+    for _ in range(args.steps):
+        u, l, km = step()
+        units += u; launches += l; kernel_ms += km
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    t = torch.tensor([ms, float(units), float(launches), kernel_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, units, launches = tmax[0].item(), tsum[1].item(), tsum[2].item()
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- end to end through the host-buffer C-ABI call (H2D / D2H inside the timed region)
+    e2e = None
+    if transport:
+        cs_bytes = 88
+        t0 = time.perf_counter(); u2 = 0
+        for _ in range(max(1, args.steps // 2)):
+            r = B.transport_run_host(geo, wl.source, wl.seed, n, precision, first_photon_id=first_id)
+            u2 += r["stats"]["n_steps"]
+        dt = time.perf_counter() - t0
+        e2e_val = torch.tensor([u2 / dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(e2e_val, op=dist.ReduceOp.SUM)
+        e2e = {"value": e2e_val.item(), "unit": "photon-steps/s", "h2d_bytes_per_step": cs_bytes, "d2h_bytes_per_step": geo.n_places * 8 + 136,
+               "note": "inputs of a run are the source description and the seed; the per-volume tally and stats come back to the host"}
+    else:
+        m = min(n, 1 << 24)
+        R = np.float32 if precision == 32 else np.float64
+        hp = torch.empty((m, 3), dtype=rdt).pin_memory(); hd = torch.empty((m, 3), dtype=rdt).pin_memory()
+        hp.copy_(pos[:m]); hd.copy_(dirs[:m])
+        B.nav_query_host(geo, hp.numpy()[:1024], hd.numpy()[:1024], precision)
+        t0 = time.perf_counter()
+        B.nav_query_host(geo, hp.numpy(), hd.numpy(), precision)
+        dt = time.perf_counter() - t0
+        rs = 4 if precision == 32 else 8
+        e2e = {"value": world * m / dt, "unit": "ComputeStep queries/s", "h2d_bytes_per_step": 6 * rs * m, "d2h_bytes_per_step": (8 + rs) * m,
+               "note": f"{m} queries from pinned host memory per call"}
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        kind = "transport" if transport else "nav"
+        abytes = ALGO_BYTES[(kind, precision)]
+        # dominant kernel = transport_pass (the only kernel of the step); its launch durations are measured with CUDA
+        # events on the launching stream inside gn_transport_run (stats.kernel_ms), summed over the step's launches
+        achieved = (units / world) * abytes / (kernel_ms * 1e-3) / 1e9 if kernel_ms > 0 else None
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(f"{wl.name}_fp{precision}")
+            except Exception:
+                traffic = None
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
+                    "traffic": traffic, "peak_source": peak_src, "kernel": "transport_pass" if transport else "locate_kernel+step_kernel",
+                    "algorithmic_bytes_per_unit": abytes, "kernel_ms_per_step": kernel_ms / args.steps,
+                    "note": "achieved = steps x algorithmic bytes / summed kernel launch time (all passes of a step); traffic = ncu dram bytes per step"}
+        cpu = None
+        if not args.no_cpu_baseline:
+            sample = {1: 10000, 2: 100000, 3: 300000, 4: 200000, 5: 1500000}[args.config]
+            v1, u1, d1 = oracle_rate(args.config, precision, sample, 1)
+            cpu = {"value": v1, "unit": "photon-steps/s" if transport else "ComputeStep queries/s", "cores": 1, "kind": "oracle",
+                   "sample": f"first {sample} of {wl.n} {'photons' if transport else 'queries'} of {wl.name}, fp{precision}, {d1:.1f} s"}
+            if args.cpu_all_cores:
+                nc = os.cpu_count() or 1
+                vN, uN, dN = oracle_rate(args.config, precision, sample * min(nc, 8), nc)
+                cpu["all_cores"] = {"value": vN, "cores": nc, "wall_s": dN}
+        line = {"metric": "transported photon steps/s" if transport else "ComputeStep queries/s",
+                "value": units / (ms * 1e-3), "unit": "photon-steps/s" if transport else "ComputeStep queries/s",
+                "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if precision == 32 else "f64", "data": "synthetic",
+                "config": {"workload": wl.name, "precision": precision, ("photons_per_gpu" if transport else "queries_per_gpu"): n,
+                           "volumes": geo.n_places, "l2": "photon state queues (2 x %d MB) exceed the 126 MB L2; no explicit flush" % (n * (48 if precision == 32 else 80) // 10 ** 6)
+                           if transport else "query arrays (%d MB) exceed the 126 MB L2" % (n * 6 * (4 if precision == 32 else 8) // 10 ** 6),
+                           "parallelism": f"dp{world} (photon-id ranges, replicated geometry)"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+                "units_per_step": units / args.steps / world}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier(); dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--precision", type=int, default=0, choices=[0, 32, 64])
+    ap.add_argument("--scale", type=float, default=1.0, help="fraction of the workload's photons/queries (diagnostics only)")
+    ap.add_argument("--steps-per-pass", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-all-cores", action="store_true")
+    ap.add_argument("--allow-short-warmup", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -70,6 +70,7 @@ typedef struct {
     double e_escaped, e_stuck, e_source, e_deposited;
     uint64_t n_passes;         /* wavefront passes (kernel launches of the step kernel) */
     uint64_t n_kernel_launches;/* all kernels launched by the call */
+    double kernel_ms;          /* sum of the step-kernel launch durations, CUDA events on the launching stream */
 } gn_run_stats;
 
 /*

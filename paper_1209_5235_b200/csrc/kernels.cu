@@ -342,7 +342,10 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     uint32_t* h_count = nullptr;
     int rc = GN_OK;
     uint64_t passes = 0, launches = 0;
-    auto cleanup = [&]() { if (h_count) cudaFreeHost(h_count); cudaFreeAsync(scratch, s); };
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    double kernel_ms = 0.0;
+    auto cleanup = [&]() { if (h_count) cudaFreeHost(h_count); if (ev0) cudaEventDestroy(ev0); if (ev1) cudaEventDestroy(ev1); cudaFreeAsync(scratch, s); };
+    if (cudaEventCreate(&ev0) != cudaSuccess || cudaEventCreate(&ev1) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_CUDA_ERROR, "gn_transport_run: event create"); }
     if (cudaMallocHost((void**)&h_count, 64) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_OUT_OF_MEMORY, "gn_transport_run: pinned alloc"); }
     cudaMemsetAsync(d_stats, 0, 512, s);
     const GeoView<R>& g = view<R>(geo);
@@ -354,6 +357,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         while (n_in > 0) {
             cudaMemsetAsync(d_count, 0, 4, s);
             unsigned blocks = (n_in + TR_THREADS - 1) / TR_THREADS;
+            cudaEventRecord(ev0, s);
             if (first) {
                 if (track) transport_pass<R, true, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
                 else transport_pass<R, true, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
@@ -363,9 +367,11 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             }
             ++passes; ++launches;
             e = cudaGetLastError();
+            cudaEventRecord(ev1, s);
             if (e == cudaSuccess) e = cudaMemcpyAsync(h_count, d_count, 4, cudaMemcpyDeviceToHost, s);
             if (e == cudaSuccess) e = cudaStreamSynchronize(s);
             if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pass"); break; }
+            { float ms = 0.f; if (cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
             n_in = *h_count;
             first = false;
             Queue<R> t = in; in = out; out = t;
@@ -380,7 +386,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             h_stats->n_steps = hs.n_steps; h_stats->n_compton = hs.n_compton; h_stats->n_pe = hs.n_pe; h_stats->n_pair = hs.n_pair;
             h_stats->n_cut = hs.n_cut; h_stats->n_escaped = hs.n_escaped; h_stats->n_stuck = hs.n_stuck; h_stats->n_photons = hs.n_photons;
             h_stats->e_escaped = hs.e_escaped; h_stats->e_stuck = hs.e_stuck; h_stats->e_source = hs.e_source; h_stats->e_deposited = hs.e_deposited;
-            h_stats->n_passes = passes; h_stats->n_kernel_launches = launches;
+            h_stats->n_passes = passes; h_stats->n_kernel_launches = launches; h_stats->kernel_ms = kernel_ms;
         }
     }
     cleanup();
