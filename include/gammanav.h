@@ -50,7 +50,7 @@ typedef struct {
     int32_t voxel_min_daughters; /* mothers with at least this many daughters get a voxel grid; default 8 */
     int32_t stuck_limit;       /* consecutive steps of length <= tol/2 before a photon is killed; default 8 */
     int32_t steps_per_pass;    /* K: steps a photon takes per wavefront pass before it is re-queued; default 16 */
-    int32_t reserved;
+    int32_t first_pass_steps;  /* K0: steps in the pass that also generates the photons (sheds photons that miss early); default 4 */
 } gn_opts;
 
 /* Photon source.  axis need not be normalised. */

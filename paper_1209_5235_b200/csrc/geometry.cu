@@ -278,19 +278,35 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     std::vector<GridRec<float>> g32; std::vector<GridRec<double>> g64;
     for (const HostGrid& G : grids) {
         GridRec<float> a; GridRec<double> b;
+        const double probe32 = std::max(geo->tol32, (double)(float)(ext * 0x1p-18)), probe64 = geo->tol64;
         for (int k = 0; k < 3; ++k) {
             a.gmin[k] = (float)G.gmin[k]; a.w[k] = (float)G.w[k]; a.inv_w[k] = (float)(1.0 / G.w[k]); a.n[k] = G.n[k];
             b.gmin[k] = G.gmin[k]; b.w[k] = G.w[k]; b.inv_w[k] = 1.0 / G.w[k]; b.n[k] = G.n[k];
+            // probe half-width in cell units, 1.5 x for the rounding of the index arithmetic itself
+            a.eps[k] = (float)(1.5 * probe32 / G.w[k]); b.eps[k] = 1.5 * probe64 / G.w[k];
         }
         a.cell_base = b.cell_base = G.cell_base;
         g32.push_back(a); g64.push_back(b);
     }
 
+    // device encodings (store.h): node {parent, solid | flags, material, n daughters}, kids {first, grid}, cells {x, count}
+    std::vector<int4> dev_node(V); std::vector<int2> dev_kids(V);
+    for (size_t i = 0; i < V; ++i) {
+        const double* R = &Rg[9 * i];
+        bool ident = R[0] == 1.0 && R[4] == 1.0 && R[8] == 1.0 && R[1] == 0.0 && R[2] == 0.0 && R[3] == 0.0 && R[5] == 0.0 && R[6] == 0.0 && R[7] == 0.0;
+        dev_node[i] = make_int4(node[i].x, node[i].y | (ident ? NODE_IDENTITY : 0), node[i].z, kids[i].y);
+        dev_kids[i] = make_int2(kids[i].x, node[i].w);
+    }
+    std::vector<int2> cells(cell_start.size() - 1);
+    for (size_t c = 0; c + 1 < cell_start.size(); ++c) {
+        int cnt = cell_start[c + 1] - cell_start[c];
+        cells[c] = make_int2(cnt == 1 ? cand[cell_start[c]] : cell_start[c], cnt);
+    }
     Uploader up{geo};
-    const int4* d_node = up.put(node); const int2* d_kids = up.put(kids); const int* d_dlist = up.put(dlist);
-    const int* d_cs = up.put(cell_start); const int* d_cand = up.put(cand);
+    const int4* d_node = up.put(dev_node); const int2* d_kids = up.put(dev_kids); const int* d_dlist = up.put(dlist);
+    const int2* d_cells = up.put(cells); const int* d_cand = up.put(cand);
     GeoView<float>& a = geo->v32; GeoView<double>& b = geo->v64;
-    a.node = b.node = d_node; a.kids = b.kids = d_kids; a.dlist = b.dlist = d_dlist; a.cell_start = b.cell_start = d_cs; a.cand = b.cand = d_cand;
+    a.node = b.node = d_node; a.kids = b.kids = d_kids; a.dlist = b.dlist = d_dlist; a.cells = b.cells = d_cells; a.cand = b.cand = d_cand;
     a.xf = up.put(xf32); b.xf = up.put(xf64);
     a.solids = up.put(s32); b.solids = up.put(s64);
     a.mats = up.put(m32); b.mats = up.put(m64);

@@ -2,13 +2,18 @@
 //
 // transport_run design (B200-first; the paper's one-thread-runs-Algorithm-1-to-completion kernel, PAPER.md
 // L143, and its CUDPP compaction experiment, L195, are the prior art):
-//   * photon state lives in two structure-of-arrays queues in HBM (48 B / photon in fp32, 80 B in fp64);
-//   * one wavefront pass = one launch of transport_pass: every thread loads one live photon (coalesced SoA
-//     loads), advances it by up to K steps (Algorithm 1 loop body: mu, s_int, ComputeStep, move / interact),
-//     and survivors are compacted into the other queue with a ballot + block-aggregated atomic cursor;
-//     pass 0 generates the photons from the source instead of loading them;
+//   * photon state lives in two queues in HBM, one 16-byte-aligned record per photon (64 B in fp32, 112 B in
+//     fp64: position, direction, E, remaining optical depth Y, the three energy factors of mu, volume, photon
+//     index, Philox draw counter, step counters), moved with 16-byte vector loads / stores;
+//   * one wavefront pass = one launch of transport_pass: every thread loads one live photon, advances it by up
+//     to K steps (Algorithm 1 loop body: mu, s_int, ComputeStep, move / interact) keeping the navigation cursor
+//     (node record + frame of the current volume) in registers, and survivors are compacted into the other queue
+//     with a ballot + block-aggregated atomic cursor; pass 0 generates the photons from the source instead of
+//     loading them and uses a short K so that photons that miss everything leave the warps early;
 //   * energy deposits are reduced across the warp per distinct volume (shuffle tree) before the fp64 atomic;
-//   * solids and material factors are staged in shared memory; transforms and voxel lists stay in L2.
+//   * rare physics (Klein-Nishina sampling, energy factors in fp64) is kept out of line so that the hot
+//     navigation loop stays small in registers and instruction cache;
+//   * solids and material factors are staged in shared memory; transforms and voxel cells stay in L2.
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -42,7 +47,8 @@ __global__ void __launch_bounds__(NAV_THREADS) locate_kernel(GeoView<R> g, const
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{0, 0, 0};
         if (HAS_DIR) { w.x = dir[3 * i]; w.y = dir[3 * i + 1]; w.z = dir[3 * i + 2]; }
-        vol_out[i] = nav.locate(x, w);
+        Cursor<R> c;
+        vol_out[i] = nav.locate(x, w, c);
     }
 }
 
@@ -58,9 +64,13 @@ __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
         int vol = vol_in[i];
-        R step; int next;
-        if (vol >= g.n_nodes) { step = rinf<R>(); next = -1; }
-        else nav.compute_step(vol, x, w, max_step ? max_step[i] : rinf<R>(), step, next);
+        R step = rinf<R>(); int next = -1;
+        if (vol >= 0 && vol < g.n_nodes) {
+            Cursor<R> c; nav.load_cursor(vol, c);
+            V3<R> xn;
+            nav.compute_step(c, x, w, max_step ? max_step[i] : rinf<R>(), step, xn);
+            next = c.vol;
+        }
         step_out[i] = step; next_out[i] = next;
     }
 }
@@ -68,7 +78,7 @@ __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R
 // -------------------------------------------------------------------------------------------------------
 // transport
 // -------------------------------------------------------------------------------------------------------
-constexpr int TR_THREADS = 256;
+constexpr int TR_THREADS = 128;
 enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
 
 struct DevStats {
@@ -76,11 +86,26 @@ struct DevStats {
     double e_escaped, e_stuck, e_source, e_deposited;
 };
 
-template <class R> struct Queue {          // SoA photon state, capacity n
-    R *x, *y, *z, *wx, *wy, *wz, *E, *Y;
-    int32_t* vol; uint32_t* idx; uint32_t* ctr; uint32_t* misc;   // misc = zero_steps | nsteps << 8
-    uint64_t* hash;                                                // only when histories are tracked
+// one photon in the queue; sizeof = 64 (float) / 112 (double), moved as 16-byte words
+template <class R> struct alignas(16) PhotonRec {
+    R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k;
+    int32_t vol; uint32_t idx, ctr, misc;        // misc = zero_steps | nsteps << 8
+    uint32_t pad[sizeof(R) == 4 ? 1 : 2];
 };
+static_assert(sizeof(PhotonRec<float>) == 64 && sizeof(PhotonRec<double>) == 112, "photon record layout");
+
+template <class R> __device__ __forceinline__ void load_rec(const PhotonRec<R>* q, unsigned i, PhotonRec<R>& r) {
+    const uint4* s = reinterpret_cast<const uint4*>(q + i);
+    uint4* d = reinterpret_cast<uint4*>(&r);
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(PhotonRec<R>) / 16); ++k) d[k] = __ldcs(s + k);      // streamed: read once
+}
+template <class R> __device__ __forceinline__ void store_rec(PhotonRec<R>* q, unsigned i, const PhotonRec<R>& r) {
+    uint4* d = reinterpret_cast<uint4*>(q + i);
+    const uint4* s = reinterpret_cast<const uint4*>(&r);
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(PhotonRec<R>) / 16); ++k) __stcs(d + k, s[k]);
+}
 
 struct PerPhotonOut { uint64_t* hash; uint32_t* nsteps; double* efinal; };
 
@@ -90,7 +115,7 @@ __device__ __forceinline__ void fnv_word(uint64_t& h, uint32_t w) {
 }
 
 // warp-aggregated tally: one fp64 atomic per distinct volume per warp
-__device__ __forceinline__ void warp_tally(double* __restrict__ edep, int vol, double dep, bool has) {
+__device__ __noinline__ void warp_tally(double* __restrict__ edep, int vol, double dep, bool has) {
     unsigned pending = __ballot_sync(0xffffffffu, has);
     const int lane = threadIdx.x & 31;
     while (pending) {
@@ -116,10 +141,24 @@ template <class T> __device__ __forceinline__ T warp_sum(T v) {
     return v;
 }
 
+// Compton scattering of one photon (C6/C7), out of line: rare (well under 1 % of steps)
+template <class R>
+__device__ __noinline__ void compton(R& E, V3<R>& w, PhiloxStream& rng, R& dep) {
+    R eps, cost, s2;
+    kn_sample(E, rng, eps, cost, s2);
+    R Ep = eps * E;
+    R phi = (R)6.283185307179586 * draw<R>(rng);
+    rotate_direction(w, cost, rsqrt_(rmax(s2, (R)0)), phi);
+    dep = E - Ep;
+    E = Ep;
+}
+template <class R> __device__ __noinline__ void energy_factors_ool(R E, EnergyFactors<R>& ef) { ef = energy_factors(E); }
+
 template <class R, bool FROM_SOURCE, bool TRACK>
 __global__ void __launch_bounds__(TR_THREADS)
-transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_in, Queue<R> qin, Queue<R> qout,
-               uint32_t* __restrict__ out_count, double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K) {
+transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_in, const PhotonRec<R>* __restrict__ qin,
+               PhotonRec<R>* __restrict__ qout, uint32_t* __restrict__ out_count, double* __restrict__ edep, DevStats* __restrict__ stats,
+               PerPhotonOut pp, int K) {
     __shared__ SolidRec<R> sh_solids[MAX_SMEM_SOLIDS];
     __shared__ MatRec<R> sh_mats[MAX_SMEM_MATS];
     __shared__ unsigned sh_warp_count[TR_THREADS / 32];
@@ -133,14 +172,14 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
     Navigator<R, true> nav(g, solids);
-    const R twopi = (R)6.283185307179586;
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     bool alive = i < n_in;
-    V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0; int vol = -1; uint32_t idx = 0, misc = 0; uint64_t h = 0xcbf29ce484222325ull;
+    V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0; uint32_t idx = 0, misc = 0; uint64_t h = 0xcbf29ce484222325ull;
+    EnergyFactors<R> ef{}; ef.above_pair = 0;
+    Cursor<R> cur; cur.vol = -1; cur.nd = make_int4(-1, 0, 0, 0);
     PhiloxStream rng; rng.init(seed, 0, 0);
-    // per-thread statistics of this pass
     unsigned c_steps = 0, c_compton = 0, c_pe = 0, c_pair = 0, c_cut = 0, c_esc = 0, c_stuck = 0, c_phot = 0;
     double e_esc = 0, e_stuck = 0, e_src = 0, e_dep = 0;
 
@@ -150,63 +189,58 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             rng.init(seed, first_id + i, 0);
             sample_source(src, rng, x, w, E);
             c_phot = 1; e_src = (double)E;
-            vol = nav.locate(x, w);
-            if (vol < 0) {
+            if (nav.locate(x, w, cur) < 0) {
                 c_esc = 1; e_esc = (double)E; alive = false;
-                if (TRACK) { if (pp.hash) pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = 0; if (pp.efinal) pp.efinal[idx] = (double)E; }
+                if (TRACK) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = 0; if (pp.efinal) pp.efinal[idx] = (double)E; }
             } else {
                 Y = -rlog(draw<R>(rng));                       // Algorithm 1 steps 1-2
+                energy_factors_ool(E, ef);
             }
         } else {
-            x.x = qin.x[i]; x.y = qin.y[i]; x.z = qin.z[i]; w.x = qin.wx[i]; w.y = qin.wy[i]; w.z = qin.wz[i];
-            E = qin.E[i]; Y = qin.Y[i]; vol = qin.vol[i]; idx = qin.idx[i]; misc = qin.misc[i];
-            rng.init(seed, first_id + idx, qin.ctr[i]);
-            if (TRACK) h = qin.hash[i];
+            PhotonRec<R> r; load_rec(qin, i, r);
+            x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
+            ef.gPE = r.gPE; ef.gKN = r.gKN; ef.L2k = r.L2k; ef.above_pair = ((double)E / GN_ME_C2) > 2.0;
+            idx = r.idx; misc = r.misc;
+            rng.init(seed, first_id + idx, r.ctr);
+            nav.load_cursor(r.vol, cur);
+            if (TRACK) h = pp.hash[idx];
         }
     }
-    EnergyFactors<R> ef{};
-    if (alive) ef = energy_factors(E);
 
     for (int k = 0; k < K; ++k) {
         if (!__any_sync(0xffffffffu, alive)) break;
         bool has_dep = false; double dep_d = 0.0; int dep_vol = 0;
         if (alive) {
-            int4 nd = __ldg(&g.node[vol]);
-            R muPE, muC, muP; mu_partials(mats[nd.z], ef, muPE, muC, muP);
+            R muPE, muC, muP; mu_partials(mats[cur.nd.z], ef, muPE, muC, muP);
             R mu = (muPE + muC) + muP;
             R s_int = mu > 0 ? Y / mu : rinf<R>();                         // remaining part of Eq. 7
-            R step; int next;
-            nav.compute_step(vol, x, w, s_int, step, next);                // "next intersection"
+            const int vol_before = cur.vol;
+            R step; V3<R> xn;
+            nav.compute_step(cur, x, w, s_int, step, xn);                  // "next intersection"
             ++c_steps; misc += 0x100u;
-            const int vol_before = vol; int ev; R len;
+            int ev; R len;
             if (step == rinf<R>()) {                                       // S_j >= Y: the photon interacts in vol
                 len = s_int;
                 x = advance(x, w, s_int);
                 R t = draw<R>(rng) * mu;
-                has_dep = true; dep_vol = vol;
+                has_dep = true; dep_vol = vol_before;
                 if (t < muPE) {
                     dep_d = (double)E; ++c_pe; ev = EV_PE; alive = false;
                 } else if (t < muPE + muC || !(muP > 0)) {
-                    R eps, cost, s2; kn_sample(E, rng, eps, cost, s2);
-                    R Ep = eps * E;
-                    R phi = twopi * draw<R>(rng);
-                    rotate_direction(w, cost, rsqrt_(rmax(s2, (R)0)), phi);
-                    R dep = E - Ep;
+                    R dep; compton(E, w, rng, dep);
                     ++c_compton; ev = EV_COMPTON;
-                    E = Ep;
-                    if (Ep < g.e_cut) { dep = dep + Ep; ++c_cut; ev = EV_CUT; alive = false; }
+                    if (E < g.e_cut) { dep = dep + E; ++c_cut; ev = EV_CUT; alive = false; }
                     dep_d = (double)dep;
-                    if (alive) { ef = energy_factors(E); Y = -rlog(draw<R>(rng)); }
+                    if (alive) { energy_factors_ool(E, ef); Y = -rlog(draw<R>(rng)); }
                 } else {
                     dep_d = (double)E; ++c_pair; ev = EV_PAIR; alive = false;
                 }
                 e_dep += dep_d;
             } else {                                                       // boundary: S_j update
                 len = step;
-                x = advance(x, w, step);
+                x = xn;
                 Y = rmax(Y - step * mu, (R)0);
-                vol = next;
-                if (vol < 0) { ++c_esc; e_esc += (double)E; ev = EV_ESCAPE; alive = false; } else ev = EV_BOUNDARY;
+                if (cur.vol < 0) { ++c_esc; e_esc += (double)E; ev = EV_ESCAPE; alive = false; } else ev = EV_BOUNDARY;
             }
             uint32_t zs = misc & 0xffu;
             zs = (len <= g.delta) ? zs + 1 : 0;
@@ -214,7 +248,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             misc = (misc & ~0xffu) | (zs & 0xffu);
             if (TRACK) {
                 fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
-                if (!alive) { if (pp.hash) pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = misc >> 8; if (pp.efinal) pp.efinal[idx] = (double)E; }
+                if (!alive) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = misc >> 8; if (pp.efinal) pp.efinal[idx] = (double)E; }
             }
         }
         if (__any_sync(0xffffffffu, has_dep)) warp_tally(edep, dep_vol, dep_d, has_dep);
@@ -232,9 +266,13 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     __syncthreads();
     if (alive) {
         unsigned o = sh_base + sh_warp_count[warp] + __popc(bal & ((1u << lane) - 1u));
-        qout.x[o] = x.x; qout.y[o] = x.y; qout.z[o] = x.z; qout.wx[o] = w.x; qout.wy[o] = w.y; qout.wz[o] = w.z;
-        qout.E[o] = E; qout.Y[o] = Y; qout.vol[o] = vol; qout.idx[o] = idx; qout.ctr[o] = rng.j; qout.misc[o] = misc;
-        if (TRACK) qout.hash[o] = h;
+        PhotonRec<R> r;
+        r.x = x.x; r.y = x.y; r.z = x.z; r.wx = w.x; r.wy = w.y; r.wz = w.z; r.E = E; r.Y = Y;
+        r.gPE = ef.gPE; r.gKN = ef.gKN; r.L2k = ef.L2k; r.vol = cur.vol; r.idx = idx; r.ctr = rng.j; r.misc = misc;
+#pragma unroll
+        for (int q = 0; q < (int)(sizeof(r.pad) / 4); ++q) r.pad[q] = 0;
+        store_rec(qout, o, r);
+        if (TRACK) pp.hash[idx] = h;
     }
     // ---- statistics: warp tree, shared atomics, one global atomic per counter per block -----------------------
     unsigned long long cs[8] = {c_steps, c_compton, c_pe, c_pair, c_cut, c_esc, c_stuck, c_phot};
@@ -306,22 +344,7 @@ template <class R> bool make_source(const gn_source& s, SourceDev<R>& o) {
     return s.kind >= GN_SRC_PENCIL && s.kind <= GN_SRC_ISOTROPIC;
 }
 
-template <class R> size_t queue_bytes(size_t cap, bool track) {
-    size_t b = cap * (8 * sizeof(R) + 4 * 4);
-    if (track) b += cap * 8;
-    return b + 256;
-}
-template <class R> Queue<R> carve_queue(char* base, size_t cap, bool track) {
-    Queue<R> q{};
-    char* p = base;
-    if (track) { q.hash = (uint64_t*)p; p += cap * 8; }       // 8-byte aligned first
-    R** f[8] = {&q.x, &q.y, &q.z, &q.wx, &q.wy, &q.wz, &q.E, &q.Y};
-    for (int i = 0; i < 8; ++i) { *f[i] = (R*)p; p += cap * sizeof(R); }
-    q.vol = (int32_t*)p; p += cap * 4; q.idx = (uint32_t*)p; p += cap * 4; q.ctr = (uint32_t*)p; p += cap * 4; q.misc = (uint32_t*)p;
-    return q;
-}
-
-constexpr int64_t TR_BATCH = 1ll << 24;     // photons per batch (bounds scratch at 2 x 16.8 M x 48 B = 1.6 GB in fp32)
+constexpr int64_t TR_BATCH = 1ll << 24;     // photons per batch (bounds scratch at 2 x 16.8 M x 64 B = 2.1 GB in fp32)
 
 template <class R>
 int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed, int64_t first_id, int64_t n_photons,
@@ -330,37 +353,40 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     if (!make_source(*h_src, src)) return fail(GN_INVALID_ARGUMENT, "gn_transport_run: bad source (axis, energies or kind)");
     const bool track = d_hash || d_nsteps || d_efinal;
     const int K = geo->opts.steps_per_pass;
+    const int K0 = std::min(K, geo->opts.first_pass_steps > 0 ? geo->opts.first_pass_steps : 4);      // first pass: short, sheds photons that miss
     const size_t cap = (size_t)std::min<int64_t>(std::max<int64_t>(n_photons, 1), TR_BATCH);
-    const size_t qb = queue_bytes<R>(cap, track);
+    const size_t qb = cap * sizeof(PhotonRec<R>);
+    const size_t hb = (track && !d_hash) ? cap * 8 : 0;       // the hash array doubles as per-photon state between passes
     char* scratch = nullptr;
     GN_CUDA(cudaMemsetAsync(d_edep, 0, sizeof(double) * (size_t)geo->n_places, s), "gn_transport_run memset edep");
-    cudaError_t e = cudaMallocAsync((void**)&scratch, 2 * qb + 512, s);
+    cudaError_t e = cudaMallocAsync((void**)&scratch, 2 * qb + hb + 512, s);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, std::string("gn_transport_run scratch: ") + cudaGetErrorString(e)); }
-    Queue<R> qa = carve_queue<R>(scratch, cap, track), qb_ = carve_queue<R>(scratch + qb, cap, track);
-    DevStats* d_stats = (DevStats*)(scratch + 2 * qb);
-    uint32_t* d_count = (uint32_t*)(scratch + 2 * qb + 256);
+    PhotonRec<R>* qa = (PhotonRec<R>*)scratch; PhotonRec<R>* qb_ = (PhotonRec<R>*)(scratch + qb);
+    uint64_t* tmp_hash = hb ? (uint64_t*)(scratch + 2 * qb) : nullptr;
+    DevStats* d_stats = (DevStats*)(scratch + 2 * qb + hb);
+    uint32_t* d_count = (uint32_t*)(scratch + 2 * qb + hb + 256);
     uint32_t* h_count = nullptr;
     int rc = GN_OK;
     uint64_t passes = 0, launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     double kernel_ms = 0.0;
     auto cleanup = [&]() { if (h_count) cudaFreeHost(h_count); if (ev0) cudaEventDestroy(ev0); if (ev1) cudaEventDestroy(ev1); cudaFreeAsync(scratch, s); };
-    if (cudaEventCreate(&ev0) != cudaSuccess || cudaEventCreate(&ev1) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_CUDA_ERROR, "gn_transport_run: event create"); }
     if (cudaMallocHost((void**)&h_count, 64) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_OUT_OF_MEMORY, "gn_transport_run: pinned alloc"); }
+    if (cudaEventCreate(&ev0) != cudaSuccess || cudaEventCreate(&ev1) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_CUDA_ERROR, "gn_transport_run: event create"); }
     cudaMemsetAsync(d_stats, 0, 512, s);
     const GeoView<R>& g = view<R>(geo);
     for (int64_t done = 0; done < n_photons && rc == GN_OK; done += (int64_t)cap) {
         uint32_t n_in = (uint32_t)std::min<int64_t>((int64_t)cap, n_photons - done);
-        PerPhotonOut pp{d_hash ? d_hash + done : nullptr, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
-        Queue<R> in = qb_, out = qa;
+        PerPhotonOut pp{d_hash ? d_hash + done : tmp_hash, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
+        PhotonRec<R>* in = qb_; PhotonRec<R>* out = qa;
         bool first = true;
         while (n_in > 0) {
             cudaMemsetAsync(d_count, 0, 4, s);
             unsigned blocks = (n_in + TR_THREADS - 1) / TR_THREADS;
             cudaEventRecord(ev0, s);
             if (first) {
-                if (track) transport_pass<R, true, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
-                else transport_pass<R, true, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
+                if (track) transport_pass<R, true, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K0);
+                else transport_pass<R, true, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K0);
             } else {
                 if (track) transport_pass<R, false, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
                 else transport_pass<R, false, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
@@ -374,7 +400,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             { float ms = 0.f; if (cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
             n_in = *h_count;
             first = false;
-            Queue<R> t = in; in = out; out = t;
+            PhotonRec<R>* t = in; in = out; out = t;
         }
     }
     if (rc == GN_OK) {
