@@ -50,7 +50,9 @@ typedef struct {
     int32_t voxel_min_daughters; /* mothers with at least this many daughters get a voxel grid; default 8 */
     int32_t stuck_limit;       /* consecutive steps of length <= tol/2 before a photon is killed; default 8 */
     int32_t steps_per_pass;    /* K: steps a photon takes per wavefront pass before it is re-queued; default 16 */
-    int32_t first_pass_steps;  /* K0: steps in the pass that also generates the photons (sheds photons that miss early); default 4 */
+    int32_t first_pass_steps;  /* K0: steps in the pass that also generates the photons (sheds photons that miss early); default 1 */
+    int32_t tail_photons;      /* once at most this many photons are left, one last pass runs them to completion; default 148 * 512 */
+    int32_t reserved;          /* must be 0 */
 } gn_opts;
 
 /* Photon source.  axis need not be normalised. */
@@ -131,8 +133,9 @@ int gn_nav_compute_step(const gn_geometry* geo, int precision, const void* d_pos
  *   d_hash_out    n uint64 history hashes (FNV-1a-64 over (volume, event) per step), or NULL
  *   d_nsteps_out  n uint32 steps per photon, or NULL
  *   d_efinal_out  n doubles: photon energy when it terminated, or NULL
- * Scratch (two photon-state queues, 2 x n x 48 B in fp32 / 80 B in fp64, plus counters) is allocated from
- * the CUDA stream-ordered pool and released before return.
+ * Scratch (two photon-state queues, 2 x min(n, 2^24) x 64 B in fp32 / 112 B in fp64, plus counters) belongs to
+ * the geometry handle: grown on demand, reused by later runs, released by gn_geometry_destroy.  Runs on one
+ * handle are serialised (internal mutex); use one handle per stream for concurrent runs.
  */
 int gn_transport_run(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
                      int64_t first_photon_id, int64_t n_photons,

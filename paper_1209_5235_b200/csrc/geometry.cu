@@ -190,6 +190,8 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     if (o.voxel_min_daughters <= 0) o.voxel_min_daughters = 8;
     if (o.stuck_limit <= 0) o.stuck_limit = 8;
     if (o.steps_per_pass <= 0) o.steps_per_pass = 16;
+    if (o.first_pass_steps <= 0) o.first_pass_steps = 1;
+    if (o.tail_photons <= 0) o.tail_photons = 148 * 512;
     o.tol64 = geo->tol64; o.tol32 = geo->tol32;
     geo->opts = o;
 
@@ -260,13 +262,24 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     }
     geo->n_grids = (int64_t)grids.size(); geo->n_cand = (int64_t)cand.size();
 
-    // ---- per-precision tables
-    std::vector<float> xf32(12 * V); std::vector<double> xf64(12 * V);
+    // ---- per-precision tables (store.h): node records with Tg inline, padded rotations
+    std::vector<NodeRec<float>> n32(V); std::vector<NodeRec<double>> n64(V);
+    std::vector<float> rot32((size_t)RotStride<float>::value * V, 0.f); std::vector<double> rot64((size_t)RotStride<double>::value * V, 0.0);
     for (size_t i = 0; i < V; ++i) {
+        const double* R = &Rg[9 * i];
+        bool ident = R[0] == 1.0 && R[4] == 1.0 && R[8] == 1.0 && R[1] == 0.0 && R[2] == 0.0 && R[3] == 0.0 && R[5] == 0.0 && R[6] == 0.0 && R[7] == 0.0;
         for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) {            // M = Rg^T
-            xf64[12 * i + 3 * a + b] = Rg[9 * i + 3 * b + a]; xf32[12 * i + 3 * a + b] = (float)Rg[9 * i + 3 * b + a];
+            rot64[RotStride<double>::value * i + 3 * a + b] = Rg[9 * i + 3 * b + a];
+            rot32[RotStride<float>::value * i + 3 * a + b] = (float)Rg[9 * i + 3 * b + a];
         }
-        for (int a = 0; a < 3; ++a) { xf64[12 * i + 9 + a] = Tg[3 * i + a]; xf32[12 * i + 9 + a] = (float)Tg[3 * i + a]; }
+        NodeRec<float>& a = n32[i]; NodeRec<double>& b = n64[i];
+        a.parent = b.parent = node[i].x;
+        a.info = b.info = node[i].y | (ident ? NODE_IDENTITY : 0);
+        a.mat = b.mat = node[i].z;
+        a.ndau = b.ndau = kids[i].y;
+        a.link = b.link = node[i].w >= 0 ? ~node[i].w : kids[i].x;        // voxelised mother: ~grid id
+        b.pad = 0;
+        for (int k = 0; k < 3; ++k) { b.t[k] = Tg[3 * i + k]; a.t[k] = (float)Tg[3 * i + k]; }
     }
     std::vector<SolidRec<float>> s32; std::vector<SolidRec<double>> s64;
     for (const HostSolid& s : solids) { s32.push_back(make_solid_rec<float>(s)); s64.push_back(make_solid_rec<double>(s)); }
@@ -288,29 +301,22 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         a.cell_base = b.cell_base = G.cell_base;
         g32.push_back(a); g64.push_back(b);
     }
-
-    // device encodings (store.h): node {parent, solid | flags, material, n daughters}, kids {first, grid}, cells {x, count}
-    std::vector<int4> dev_node(V); std::vector<int2> dev_kids(V);
-    for (size_t i = 0; i < V; ++i) {
-        const double* R = &Rg[9 * i];
-        bool ident = R[0] == 1.0 && R[4] == 1.0 && R[8] == 1.0 && R[1] == 0.0 && R[2] == 0.0 && R[3] == 0.0 && R[5] == 0.0 && R[6] == 0.0 && R[7] == 0.0;
-        dev_node[i] = make_int4(node[i].x, node[i].y | (ident ? NODE_IDENTITY : 0), node[i].z, kids[i].y);
-        dev_kids[i] = make_int2(kids[i].x, node[i].w);
-    }
     std::vector<int2> cells(cell_start.size() - 1);
     for (size_t c = 0; c + 1 < cell_start.size(); ++c) {
         int cnt = cell_start[c + 1] - cell_start[c];
         cells[c] = make_int2(cnt == 1 ? cand[cell_start[c]] : cell_start[c], cnt);
     }
     Uploader up{geo};
-    const int4* d_node = up.put(dev_node); const int2* d_kids = up.put(dev_kids); const int* d_dlist = up.put(dlist);
+    const int* d_dlist = up.put(dlist);
     const int2* d_cells = up.put(cells); const int* d_cand = up.put(cand);
     GeoView<float>& a = geo->v32; GeoView<double>& b = geo->v64;
-    a.node = b.node = d_node; a.kids = b.kids = d_kids; a.dlist = b.dlist = d_dlist; a.cells = b.cells = d_cells; a.cand = b.cand = d_cand;
-    a.xf = up.put(xf32); b.xf = up.put(xf64);
+    a.dlist = b.dlist = d_dlist; a.cells = b.cells = d_cells; a.cand = b.cand = d_cand;
+    a.node = up.put(n32); b.node = up.put(n64);
+    a.rot = up.put(rot32); b.rot = up.put(rot64);
     a.solids = up.put(s32); b.solids = up.put(s64);
     a.mats = up.put(m32); b.mats = up.put(m64);
     a.grids = up.put(g32); b.grids = up.put(g64);
+    a.n_grids = b.n_grids = (int)grids.size();
     a.tol = (float)geo->tol32; a.delta = a.tol / 2; a.probe = std::max(a.tol, (float)(ext * 0x1p-18)); a.e_cut = (float)o.e_cut;
     b.tol = geo->tol64; b.delta = b.tol / 2; b.probe = b.tol; b.e_cut = o.e_cut;
     a.n_nodes = b.n_nodes = n_places; a.n_solids = b.n_solids = n_solids; a.n_mats = b.n_mats = n_mats;
@@ -327,6 +333,9 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
 extern "C" int gn_geometry_destroy(gn_geometry* geo) {
     if (!geo) return GN_OK;
     for (void* p : geo->allocations) cudaFree(p);
+    if (geo->ws_scratch) cudaFree(geo->ws_scratch);
+    if (geo->ws_pinned) cudaFreeHost(geo->ws_pinned);
+    if (geo->ws_events_ok) for (cudaEvent_t e : geo->ws_events) if (e) cudaEventDestroy(e);
     delete geo;
     return GN_OK;
 }

@@ -1,5 +1,6 @@
 // geometry.h -- the opaque gn_geometry handle (host side) shared by geometry.cu and kernels.cu
 #pragma once
+#include <mutex>
 #include <string>
 #include <vector>
 #include "store.h"
@@ -14,6 +15,14 @@ struct gn_geometry {
     gn_opts opts{};
     int64_t n_grids = 0, n_cells = 0, n_cand = 0, device_bytes = 0;
     int device = 0;
+    // transport workspace (photon queues, counters, pinned read-back, events): grown on demand, reused by every
+    // gn_transport_run on this handle, released by gn_geometry_destroy; runs on one handle are serialised
+    mutable std::mutex ws_mutex;
+    mutable char* ws_scratch = nullptr;
+    mutable size_t ws_bytes = 0;
+    mutable void* ws_pinned = nullptr;
+    mutable cudaEvent_t ws_events[8] = {};
+    mutable bool ws_events_ok = false;
 };
 
 namespace gn {

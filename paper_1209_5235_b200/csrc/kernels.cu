@@ -1,4 +1,4 @@
-// kernels.cu -- navigation kernels, the wavefront transport kernels and the C entry points that launch them.
+// kernels.cu -- navigation kernels, the wavefront transport kernel and the C entry points that launch them.
 //
 // transport_run design (B200-first; the paper's one-thread-runs-Algorithm-1-to-completion kernel, PAPER.md
 // L143, and its CUDPP compaction experiment, L195, are the prior art):
@@ -6,16 +6,23 @@
 //     fp64: position, direction, E, remaining optical depth Y, the three energy factors of mu, volume, photon
 //     index, Philox draw counter, step counters), moved with 16-byte vector loads / stores;
 //   * one wavefront pass = one launch of transport_pass: every thread loads one live photon, advances it by up
-//     to K steps (Algorithm 1 loop body: mu, s_int, ComputeStep, move / interact) keeping the navigation cursor
-//     (node record + frame of the current volume) in registers, and survivors are compacted into the other queue
-//     with a ballot + block-aggregated atomic cursor; pass 0 generates the photons from the source instead of
-//     loading them and uses a short K so that photons that miss everything leave the warps early;
+//     to K steps (Algorithm 1 loop body: mu, s_int, ComputeStep, move / interact) keeping the node record of the
+//     current volume in registers, and survivors are compacted into the other queue with a ballot + block-
+//     aggregated atomic cursor, partitioned by a 1-bit key (solid type of the current volume) to the front /
+//     back of the queue; pass 0 generates the photons from the source and takes one step, so photons that miss
+//     everything leave the warps at once;
+//   * passes are chained on the device: a pass reads its input count from the counter its predecessor
+//     incremented, so the host enqueues passes back to back and only looks at counts that are two passes old;
+//     once few photons are left, one last pass runs them to completion;
 //   * energy deposits are reduced across the warp per distinct volume (shuffle tree) before the fp64 atomic;
-//   * rare physics (Klein-Nishina sampling, energy factors in fp64) is kept out of line so that the hot
-//     navigation loop stays small in registers and instruction cache;
-//   * solids and material factors are staged in shared memory; transforms and voxel cells stay in L2.
+//   * rare physics (Philox rounds, Klein-Nishina sampling, energy factors in fp64) and bulky geometry (tube
+//     distances, daughter scans, voxel walk) are out of line, one copy each, so that the hot navigation loop is
+//     small in registers and instruction cache;
+//   * solids, voxel-grid headers and material factors are staged in shared memory; node records and voxel
+//     cells stay in L2.
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include "geometry.h"
 #include "nav.cuh"
@@ -23,32 +30,43 @@
 
 namespace gn {
 
+constexpr int NAV_THREADS = 256;
+constexpr int MAX_SMEM_SOLIDS = 32;
+constexpr int MAX_SMEM_GRIDS = 8;
+constexpr int MAX_SMEM_MATS = 32;
+
+// per-block copies of the small tables + the pointer block the out-of-line navigation helpers read
+template <class R> struct BlockTables {
+    SolidRec<R> solids[MAX_SMEM_SOLIDS];
+    GridRec<R> grids[MAX_SMEM_GRIDS];
+    NavCtx<R> ctx;
+};
+template <class R> __device__ __forceinline__ void stage_tables(const GeoView<R>& g, BlockTables<R>& t) {
+    const bool ss = g.n_solids <= MAX_SMEM_SOLIDS, sg = g.n_grids <= MAX_SMEM_GRIDS;
+    if (ss) for (int i = threadIdx.x; i < g.n_solids; i += blockDim.x) t.solids[i] = g.solids[i];
+    if (sg) for (int i = threadIdx.x; i < g.n_grids; i += blockDim.x) t.grids[i] = g.grids[i];
+    if (threadIdx.x == 0) {
+        t.ctx.node = g.node; t.ctx.rot = g.rot; t.ctx.dlist = g.dlist; t.ctx.cells = g.cells; t.ctx.cand = g.cand;
+        t.ctx.solids = ss ? t.solids : g.solids; t.ctx.grids = sg ? t.grids : g.grids; t.ctx.delta = g.delta;
+    }
+}
+
 // -------------------------------------------------------------------------------------------------------
 // navigation kernels: pure maps over queries
 // -------------------------------------------------------------------------------------------------------
-constexpr int NAV_THREADS = 256;
-constexpr int MAX_SMEM_SOLIDS = 64;
-constexpr int MAX_SMEM_MATS = 32;
-
-template <class R> __device__ __forceinline__ const SolidRec<R>* stage_solids(const GeoView<R>& g, SolidRec<R>* sh) {
-    if (g.n_solids > MAX_SMEM_SOLIDS) return g.solids;
-    for (int i = threadIdx.x; i < g.n_solids; i += blockDim.x) sh[i] = g.solids[i];
-    return sh;
-}
-
 template <class R, bool HAS_DIR>
 __global__ void __launch_bounds__(NAV_THREADS) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                              int64_t n, int32_t* __restrict__ vol_out) {
-    __shared__ SolidRec<R> sh_solids[MAX_SMEM_SOLIDS];
-    const SolidRec<R>* solids = stage_solids(g, sh_solids);
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
     __syncthreads();
-    Navigator<R, HAS_DIR> nav(g, solids);
+    Navigator<R, HAS_DIR> nav(g, &tab.ctx);
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{0, 0, 0};
         if (HAS_DIR) { w.x = dir[3 * i]; w.y = dir[3 * i + 1]; w.z = dir[3 * i + 2]; }
-        Cursor<R> c;
-        vol_out[i] = nav.locate(x, w, c);
+        NodeRec<R> nd;
+        vol_out[i] = nav.locate(x, w, nd);
     }
 }
 
@@ -56,20 +74,20 @@ template <class R>
 __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                            const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
                                                            int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out) {
-    __shared__ SolidRec<R> sh_solids[MAX_SMEM_SOLIDS];
-    const SolidRec<R>* solids = stage_solids(g, sh_solids);
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
     __syncthreads();
-    Navigator<R, true> nav(g, solids);
+    Navigator<R, true> nav(g, &tab.ctx);
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
         int vol = vol_in[i];
         R step = rinf<R>(); int next = -1;
         if (vol >= 0 && vol < g.n_nodes) {
-            Cursor<R> c; nav.load_cursor(vol, c);
+            NodeRec<R> nd = nav.node(vol);
             V3<R> xn;
-            nav.compute_step(c, x, w, max_step ? max_step[i] : rinf<R>(), step, xn);
-            next = c.vol;
+            nav.compute_step(vol, nd, x, w, max_step ? max_step[i] : rinf<R>(), step, xn);
+            next = vol;
         }
         step_out[i] = step; next_out[i] = next;
     }
@@ -79,18 +97,25 @@ __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R
 // transport
 // -------------------------------------------------------------------------------------------------------
 constexpr int TR_THREADS = 128;
+constexpr int TR_WARPS = TR_THREADS / 32;
+constexpr int INTERACT_BATCH = 8;     // parked lanes that trigger a warp's interaction phase
 enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
+enum : int { FATE_ALIVE = 0, FATE_ABSORBED = 1, FATE_ESCAPED = 2, FATE_STUCK = 3, FATE_NONE = 4 };
+enum : int { ST_STEPS = 0, ST_COMPTON, ST_PE, ST_PAIR, ST_CUT, ST_ESCAPED, ST_STUCK, ST_PHOTONS };
+enum : int { EN_ESCAPED = 0, EN_STUCK, EN_SOURCE, EN_DEPOSITED };
 
 struct DevStats {
-    unsigned long long n_steps, n_compton, n_pe, n_pair, n_cut, n_escaped, n_stuck, n_photons;
-    double e_escaped, e_stuck, e_source, e_deposited;
+    unsigned long long cnt[8];       // ST_*
+    double en[4];                    // EN_*
 };
+// survivors of a pass: key-0 photons fill the output queue from the front, key-1 photons from the back
+struct PassCounters { unsigned front, back; };
 
 // one photon in the queue; sizeof = 64 (float) / 112 (double), moved as 16-byte words
 template <class R> struct alignas(16) PhotonRec {
     R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k;
     int32_t vol; uint32_t idx, ctr, misc;        // misc = zero_steps | nsteps << 8
-    uint32_t pad[sizeof(R) == 4 ? 1 : 2];
+    uint32_t tail[sizeof(R) == 4 ? 1 : 2];       // tail[0] = E above the pair threshold (k > 2); rest padding
 };
 static_assert(sizeof(PhotonRec<float>) == 64 && sizeof(PhotonRec<double>) == 112, "photon record layout");
 
@@ -114,8 +139,14 @@ __device__ __forceinline__ void fnv_word(uint64_t& h, uint32_t w) {
     for (int i = 0; i < 4; ++i) { h ^= (w >> (8 * i)) & 0xffu; h *= 0x100000001b3ull; }
 }
 
+template <class T> __device__ __forceinline__ T warp_sum(T v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
 // warp-aggregated tally: one fp64 atomic per distinct volume per warp
-__device__ __noinline__ void warp_tally(double* __restrict__ edep, int vol, double dep, bool has) {
+__device__ __noinline__ void warp_tally(double* __restrict__ edep, double* sh_dep_total, int vol, double dep, bool has) {
     unsigned pending = __ballot_sync(0xffffffffu, has);
     const int lane = threadIdx.x & 31;
     while (pending) {
@@ -123,167 +154,245 @@ __device__ __noinline__ void warp_tally(double* __restrict__ edep, int vol, doub
         int v = __shfl_sync(0xffffffffu, vol, leader);
         bool same = has && vol == v;
         unsigned grp = __ballot_sync(0xffffffffu, same);
-        if (grp == (1u << leader)) {
-            if (lane == leader) atomicAdd(&edep[v], dep);
-        } else {
-            double s = same ? dep : 0.0;
+        double s = dep;
+        if (grp != (1u << leader)) {
+            s = same ? dep : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-            if (lane == leader) atomicAdd(&edep[v], s);
         }
+        if (lane == leader) { atomicAdd(&edep[v], s); atomicAdd(sh_dep_total, s); }
         pending &= ~grp;
     }
 }
 
-template <class T> __device__ __forceinline__ T warp_sum(T v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+// One interaction (C6 / C7), out of line: process choice, Klein-Nishina sampling, new direction, new energy
+// factors, new optical depth.  State goes through a short-lived record so that the caller's registers never
+// have their address taken.
+template <class R> struct InteractIO {
+    R E, wx, wy, wz, Y, gPE, gKN, L2k, dep;
+    uint32_t j; int above, ev;
+};
+template <class R>
+__device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R mu, R e_cut, uint64_t seed, uint64_t id) {
+    PhiloxStream rng; rng.init(seed, id, io->j);
+    R E = io->E;
+    R t = draw<R>(rng) * mu;
+    if (t < muPE) { io->dep = E; io->ev = EV_PE; }
+    else if (t < muPE + muC || !(muP > 0)) {
+        R eps, cost, s2;
+        kn_sample(E, rng, eps, cost, s2);
+        R Ep = eps * E;
+        R phi = (R)6.283185307179586 * draw<R>(rng);
+        V3<R> w{io->wx, io->wy, io->wz};
+        rotate_direction(w, cost, rsqrt_(rmax(s2, (R)0)), phi);
+        io->wx = w.x; io->wy = w.y; io->wz = w.z;
+        R dep = E - Ep;
+        io->E = Ep; io->ev = EV_COMPTON;
+        if (Ep < e_cut) { dep = dep + Ep; io->ev = EV_CUT; }
+        else {
+            EnergyFactors<R> ef = energy_factors(Ep);
+            io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
+            io->Y = -rlog(draw<R>(rng));
+        }
+        io->dep = dep;
+    } else { io->dep = E; io->ev = EV_PAIR; }
+    io->j = rng.j;
 }
 
-// Compton scattering of one photon (C6/C7), out of line: rare (well under 1 % of steps)
+// photon birth (C8, Algorithm 1 steps 1-2), out of line: source sampling, energy factors, first optical depth
+template <class R> struct BirthIO { R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k; uint32_t j; int above; };
 template <class R>
-__device__ __noinline__ void compton(R& E, V3<R>& w, PhiloxStream& rng, R& dep) {
-    R eps, cost, s2;
-    kn_sample(E, rng, eps, cost, s2);
-    R Ep = eps * E;
-    R phi = (R)6.283185307179586 * draw<R>(rng);
-    rotate_direction(w, cost, rsqrt_(rmax(s2, (R)0)), phi);
-    dep = E - Ep;
-    E = Ep;
+__device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, uint64_t seed, uint64_t id) {
+    PhiloxStream rng; rng.init(seed, id, 0);
+    V3<R> x, w; R E;
+    sample_source(*src, rng, x, w, E);
+    io->x = x.x; io->y = x.y; io->z = x.z; io->wx = w.x; io->wy = w.y; io->wz = w.z; io->E = E;
+    io->Y = -rlog(draw<R>(rng));                       // Algorithm 1 steps 1-2
+    EnergyFactors<R> ef = energy_factors(E);
+    io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
+    io->j = rng.j;
 }
-template <class R> __device__ __noinline__ void energy_factors_ool(R E, EnergyFactors<R>& ef) { ef = energy_factors(E); }
 
 template <class R, bool FROM_SOURCE, bool TRACK>
 __global__ void __launch_bounds__(TR_THREADS)
-transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_in, const PhotonRec<R>* __restrict__ qin,
-               PhotonRec<R>* __restrict__ qout, uint32_t* __restrict__ out_count, double* __restrict__ edep, DevStats* __restrict__ stats,
-               PerPhotonOut pp, int K) {
-    __shared__ SolidRec<R> sh_solids[MAX_SMEM_SOLIDS];
+transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
+               PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
+               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K) {
+    // input: pass 0 generates n_src photons; later passes read the survivors of the previous pass, whose count is
+    // known only on the device (front + back of cin)
+    unsigned n_front = n_src, n_in = n_src;
+    if (!FROM_SOURCE) { n_front = cin->front; n_in = n_front + cin->back; }
+    if (blockIdx.x * TR_THREADS >= n_in) return;
+
+    __shared__ BlockTables<R> tab;
     __shared__ MatRec<R> sh_mats[MAX_SMEM_MATS];
-    __shared__ unsigned sh_warp_count[TR_THREADS / 32];
-    __shared__ unsigned sh_base;
+    __shared__ SourceDev<R> sh_src;
+    __shared__ unsigned sh_wcount[2][TR_WARPS];
+    __shared__ unsigned sh_base[2];
     __shared__ unsigned long long sh_cnt[8];
     __shared__ double sh_en[4];
-    const SolidRec<R>* solids = stage_solids(g, sh_solids);
+    stage_tables(g, tab);
     const MatRec<R>* mats = g.mats;
     if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
+    if (FROM_SOURCE && threadIdx.x == 0) sh_src = src;
     if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
-    Navigator<R, true> nav(g, solids);
-    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    Navigator<R, true> nav(g, &tab.ctx);
+    const unsigned i = blockIdx.x * TR_THREADS + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    bool alive = i < n_in;
-    V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0; uint32_t idx = 0, misc = 0; uint64_t h = 0xcbf29ce484222325ull;
-    EnergyFactors<R> ef{}; ef.above_pair = 0;
-    Cursor<R> cur; cur.vol = -1; cur.nd = make_int4(-1, 0, 0, 0);
-    PhiloxStream rng; rng.init(seed, 0, 0);
-    unsigned c_steps = 0, c_compton = 0, c_pe = 0, c_pair = 0, c_cut = 0, c_esc = 0, c_stuck = 0, c_phot = 0;
-    double e_esc = 0, e_stuck = 0, e_src = 0, e_dep = 0;
+    int fate = i < n_in ? FATE_ALIVE : FATE_NONE;
+    V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0, gPE = 0, gKN = 0, L2k = 0;
+    uint32_t idx = 0, misc = 0, ctr = 0; int above = 0;
+    uint64_t h = 0xcbf29ce484222325ull;
+    int vol = -1; NodeRec<R> nd = {};
+    unsigned c_steps = 0;
 
-    if (alive) {
-        if (FROM_SOURCE) {
+    if (FROM_SOURCE) {
+        unsigned c_phot = 0; double e_src = 0.0;
+        if (fate == FATE_ALIVE) {
             idx = i;
-            rng.init(seed, first_id + i, 0);
-            sample_source(src, rng, x, w, E);
+            BirthIO<R> b;
+            birth(&b, &sh_src, seed, first_id + i);
+            x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
+            gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
             c_phot = 1; e_src = (double)E;
-            if (nav.locate(x, w, cur) < 0) {
-                c_esc = 1; e_esc = (double)E; alive = false;
+            vol = nav.locate(x, w, nd);
+            if (vol < 0) {
+                fate = FATE_ESCAPED;
                 if (TRACK) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = 0; if (pp.efinal) pp.efinal[idx] = (double)E; }
-            } else {
-                Y = -rlog(draw<R>(rng));                       // Algorithm 1 steps 1-2
-                energy_factors_ool(E, ef);
             }
-        } else {
-            PhotonRec<R> r; load_rec(qin, i, r);
-            x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
-            ef.gPE = r.gPE; ef.gKN = r.gKN; ef.L2k = r.L2k; ef.above_pair = ((double)E / GN_ME_C2) > 2.0;
-            idx = r.idx; misc = r.misc;
-            rng.init(seed, first_id + idx, r.ctr);
-            nav.load_cursor(r.vol, cur);
-            if (TRACK) h = pp.hash[idx];
         }
+        c_phot = warp_sum(c_phot); e_src = warp_sum(e_src);
+        if (lane == 0) { atomicAdd(&sh_cnt[ST_PHOTONS], (unsigned long long)c_phot); atomicAdd(&sh_en[EN_SOURCE], e_src); }
+    } else if (fate == FATE_ALIVE) {
+        PhotonRec<R> r; load_rec(qin, i < n_front ? i : cap - 1u - (i - n_front), r);
+        x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
+        gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = (int)r.tail[0];
+        idx = r.idx; misc = r.misc; ctr = r.ctr; vol = r.vol;
+        nd = nav.node(vol);
+        if (TRACK) h = pp.hash[idx];
     }
 
-    for (int k = 0; k < K; ++k) {
-        if (!__any_sync(0xffffffffu, alive)) break;
-        bool has_dep = false; double dep_d = 0.0; int dep_vol = 0;
-        if (alive) {
-            R muPE, muC, muP; mu_partials(mats[cur.nd.z], ef, muPE, muC, muP);
-            R mu = (muPE + muC) + muP;
-            R s_int = mu > 0 ? Y / mu : rinf<R>();                         // remaining part of Eq. 7
-            const int vol_before = cur.vol;
-            R step; V3<R> xn;
-            nav.compute_step(cur, x, w, s_int, step, xn);                  // "next intersection"
-            ++c_steps; misc += 0x100u;
-            int ev; R len;
-            if (step == rinf<R>()) {                                       // S_j >= Y: the photon interacts in vol
-                len = s_int;
-                x = advance(x, w, s_int);
-                R t = draw<R>(rng) * mu;
-                has_dep = true; dep_vol = vol_before;
-                if (t < muPE) {
-                    dep_d = (double)E; ++c_pe; ev = EV_PE; alive = false;
-                } else if (t < muPE + muC || !(muP > 0)) {
-                    R dep; compton(E, w, rng, dep);
-                    ++c_compton; ev = EV_COMPTON;
-                    if (E < g.e_cut) { dep = dep + E; ++c_cut; ev = EV_CUT; alive = false; }
-                    dep_d = (double)dep;
-                    if (alive) { energy_factors_ool(E, ef); Y = -rlog(draw<R>(rng)); }
+    // A lane whose photon reaches its interaction point parks there (pending) instead of running the rare, long
+    // physics alone with 31 lanes idle; the warp runs one interaction phase for all parked lanes once
+    // INTERACT_BATCH of them wait, or when nothing else is left to do (group by event type).
+    bool pending = false;
+    auto finish_step = [&](int ev, int vol_before) {          // stuck guard (C9) + history hash; after the step's event
+        if (fate == FATE_ALIVE && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; fate = FATE_STUCK; }
+        if (TRACK) {
+            fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
+            if (fate != FATE_ALIVE) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = misc >> 8; if (pp.efinal) pp.efinal[idx] = (double)E; }
+        }
+    };
+#pragma unroll 1
+    for (int k = 0;;) {
+        const unsigned pen = __ballot_sync(0xffffffffu, pending);
+        const unsigned act = __ballot_sync(0xffffffffu, fate == FATE_ALIVE && !pending);
+        const bool budget = k < K;
+        if (pen && (act == 0 || !budget || __popc(pen) >= INTERACT_BATCH)) {
+            // ---- interaction phase (A6-A9) ----------------------------------------------------------------------
+            double dep_d = 0.0;
+            if (pending) {
+                const MatRec<R> m = mats[nd.mat];
+                const R muPE = m.aPE * gPE, muC = m.aC * gKN;
+                const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
+                const R muP = (above && P > 0) ? m.aP * P : (R)0;
+                const R mu = (muPE + muC) + muP;
+                InteractIO<R> io;
+                io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
+                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + idx);
+                const int ev = io.ev; ctr = io.j;
+                dep_d = (double)io.dep;
+                if (ev == EV_COMPTON || ev == EV_CUT) {
+                    E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
+                    atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
+                    if (ev == EV_CUT) { atomicAdd(&sh_cnt[ST_CUT], 1ull); fate = FATE_ABSORBED; }
+                    else { Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above; }
                 } else {
-                    dep_d = (double)E; ++c_pair; ev = EV_PAIR; alive = false;
+                    atomicAdd(&sh_cnt[ev == EV_PE ? ST_PE : ST_PAIR], 1ull);
+                    fate = FATE_ABSORBED;
                 }
-                e_dep += dep_d;
-            } else {                                                       // boundary: S_j update
-                len = step;
-                x = xn;
-                Y = rmax(Y - step * mu, (R)0);
-                if (cur.vol < 0) { ++c_esc; e_esc += (double)E; ev = EV_ESCAPE; alive = false; } else ev = EV_BOUNDARY;
+                finish_step(ev, vol);
             }
+            warp_tally(edep, &sh_en[EN_DEPOSITED], vol, dep_d, pending);
+            pending = false;
+            continue;
+        }
+        if (act == 0 || !budget) break;
+        ++k;
+        if (fate == FATE_ALIVE && !pending) {
+            const MatRec<R> m = mats[nd.mat];
+            const R muPE = m.aPE * gPE, muC = m.aC * gKN;
+            const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
+            const R muP = (above && P > 0) ? m.aP * P : (R)0;
+            const R mu = (muPE + muC) + muP;
+            const R s_int = mu > 0 ? rdiv(Y, mu) : rinf<R>();                  // remaining part of Eq. 7
+            const int vol_before = vol;
+            R step; V3<R> xn;
+            nav.compute_step(vol, nd, x, w, s_int, step, xn);                  // "next intersection"
+            ++c_steps; misc += 0x100u;
+            const bool inter = step == rinf<R>();                              // S_j >= Y: the photon interacts in vol
+            const R len = inter ? s_int : step;
             uint32_t zs = misc & 0xffu;
             zs = (len <= g.delta) ? zs + 1 : 0;
-            if (alive && zs >= (uint32_t)g.stuck_limit) { ++c_stuck; e_stuck += (double)E; ev = EV_STUCK; alive = false; }
             misc = (misc & ~0xffu) | (zs & 0xffu);
-            if (TRACK) {
-                fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
-                if (!alive) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = misc >> 8; if (pp.efinal) pp.efinal[idx] = (double)E; }
+            if (inter) {
+                x = advance(x, w, s_int);
+                pending = true;
+            } else {                                                           // boundary: S_j update
+                x = xn;
+                Y = rmax(Y - step * mu, (R)0);
+                int ev = EV_BOUNDARY;
+                if (vol < 0) { ev = EV_ESCAPE; fate = FATE_ESCAPED; }
+                finish_step(ev, vol_before);
             }
         }
-        if (__any_sync(0xffffffffu, has_dep)) warp_tally(edep, dep_vol, dep_d, has_dep);
     }
 
-    // ---- compaction of survivors into the other queue ------------------------------------
-    unsigned bal = __ballot_sync(0xffffffffu, alive);
-    if (lane == 0) sh_warp_count[warp] = __popc(bal);
+    // ---- compaction of survivors into the other queue, partitioned by key -------------------
+    const bool alive = fate == FATE_ALIVE;
+    const bool key1 = alive && nav.solid_of(nd).type != SOLID_BOX;
+    const unsigned bal0 = __ballot_sync(0xffffffffu, alive && !key1), bal1 = __ballot_sync(0xffffffffu, key1);
+    if (lane == 0) { sh_wcount[0][warp] = __popc(bal0); sh_wcount[1][warp] = __popc(bal1); }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x < 2) {
         unsigned tot = 0;
-        for (int q = 0; q < TR_THREADS / 32; ++q) { unsigned c = sh_warp_count[q]; sh_warp_count[q] = tot; tot += c; }
-        sh_base = tot ? atomicAdd(out_count, tot) : 0u;
+        for (int q = 0; q < TR_WARPS; ++q) { unsigned c = sh_wcount[threadIdx.x][q]; sh_wcount[threadIdx.x][q] = tot; tot += c; }
+        sh_base[threadIdx.x] = tot ? atomicAdd(threadIdx.x == 0 ? &cout->front : &cout->back, tot) : 0u;
     }
     __syncthreads();
     if (alive) {
-        unsigned o = sh_base + sh_warp_count[warp] + __popc(bal & ((1u << lane) - 1u));
+        const unsigned below = (1u << lane) - 1u;
+        unsigned o = key1 ? cap - 1u - (sh_base[1] + sh_wcount[1][warp] + __popc(bal1 & below))
+                          : sh_base[0] + sh_wcount[0][warp] + __popc(bal0 & below);
         PhotonRec<R> r;
         r.x = x.x; r.y = x.y; r.z = x.z; r.wx = w.x; r.wy = w.y; r.wz = w.z; r.E = E; r.Y = Y;
-        r.gPE = ef.gPE; r.gKN = ef.gKN; r.L2k = ef.L2k; r.vol = cur.vol; r.idx = idx; r.ctr = rng.j; r.misc = misc;
+        r.gPE = gPE; r.gKN = gKN; r.L2k = L2k; r.vol = vol; r.idx = idx; r.ctr = ctr; r.misc = misc;
 #pragma unroll
-        for (int q = 0; q < (int)(sizeof(r.pad) / 4); ++q) r.pad[q] = 0;
+        for (int q = 0; q < (int)(sizeof(r.tail) / 4); ++q) r.tail[q] = 0;
+        r.tail[0] = (uint32_t)above;
         store_rec(qout, o, r);
         if (TRACK) pp.hash[idx] = h;
     }
     // ---- statistics: warp tree, shared atomics, one global atomic per counter per block -----------------------
-    unsigned long long cs[8] = {c_steps, c_compton, c_pe, c_pair, c_cut, c_esc, c_stuck, c_phot};
-    double es[4] = {e_esc, e_stuck, e_src, e_dep};
-#pragma unroll
-    for (int q = 0; q < 8; ++q) { unsigned long long v = warp_sum(cs[q]); if (lane == 0 && v) atomicAdd(&sh_cnt[q], v); }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { double v = warp_sum(es[q]); if (lane == 0 && v != 0.0) atomicAdd(&sh_en[q], v); }
+    {
+        unsigned s = warp_sum(c_steps);
+        unsigned ne = warp_sum(fate == FATE_ESCAPED ? 1u : 0u), ns = warp_sum(fate == FATE_STUCK ? 1u : 0u);
+        double ee = warp_sum(fate == FATE_ESCAPED ? (double)E : 0.0);
+        if (lane == 0) {
+            if (s) atomicAdd(&sh_cnt[ST_STEPS], (unsigned long long)s);
+            if (ne) { atomicAdd(&sh_cnt[ST_ESCAPED], (unsigned long long)ne); atomicAdd(&sh_en[EN_ESCAPED], ee); }
+        }
+        if (ns) {                                                           // warp-uniform, rare
+            double es = warp_sum(fate == FATE_STUCK ? (double)E : 0.0);
+            if (lane == 0) { atomicAdd(&sh_cnt[ST_STUCK], (unsigned long long)ns); atomicAdd(&sh_en[EN_STUCK], es); }
+        }
+    }
     __syncthreads();
-    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&(&stats->n_steps)[threadIdx.x], sh_cnt[threadIdx.x]);
-    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&(&stats->e_escaped)[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
 }
 
 // -------------------------------------------------------------------------------------------------------
@@ -345,6 +454,17 @@ template <class R> bool make_source(const gn_source& s, SourceDev<R>& o) {
 }
 
 constexpr int64_t TR_BATCH = 1ll << 24;     // photons per batch (bounds scratch at 2 x 16.8 M x 64 B = 2.1 GB in fp32)
+constexpr int TR_MAX_PASSES = 4096;         // device counters per batch; the last one always runs to completion
+constexpr int TR_LAG = 2;                   // the host looks at survivor counts that are this many passes old
+constexpr int K_UNLIMITED = 0x7fffffff;
+
+template <class R, bool SRC>
+static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
+                        uint32_t n_src, const PassCounters* cin, PassCounters* cout, const PhotonRec<R>* qin, PhotonRec<R>* qout, uint32_t cap,
+                        double* edep, DevStats* stats, PerPhotonOut pp, int K) {
+    if (track) transport_pass<R, SRC, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
+    else transport_pass<R, SRC, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
+}
 
 template <class R>
 int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed, int64_t first_id, int64_t n_photons,
@@ -353,55 +473,78 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     if (!make_source(*h_src, src)) return fail(GN_INVALID_ARGUMENT, "gn_transport_run: bad source (axis, energies or kind)");
     const bool track = d_hash || d_nsteps || d_efinal;
     const int K = geo->opts.steps_per_pass;
-    const int K0 = std::min(K, geo->opts.first_pass_steps > 0 ? geo->opts.first_pass_steps : 4);      // first pass: short, sheds photons that miss
+    const int K0 = std::min(K, geo->opts.first_pass_steps);      // first pass: short, sheds photons that miss
     const size_t cap = (size_t)std::min<int64_t>(std::max<int64_t>(n_photons, 1), TR_BATCH);
     const size_t qb = cap * sizeof(PhotonRec<R>);
     const size_t hb = (track && !d_hash) ? cap * 8 : 0;       // the hash array doubles as per-photon state between passes
-    char* scratch = nullptr;
+    const size_t cb = sizeof(PassCounters) * (TR_MAX_PASSES + 2);
+    const size_t need = 2 * qb + hb + 512 + cb;
+    std::lock_guard<std::mutex> lock(geo->ws_mutex);          // one run at a time per handle: the workspace is shared
     GN_CUDA(cudaMemsetAsync(d_edep, 0, sizeof(double) * (size_t)geo->n_places, s), "gn_transport_run memset edep");
-    cudaError_t e = cudaMallocAsync((void**)&scratch, 2 * qb + hb + 512, s);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, std::string("gn_transport_run scratch: ") + cudaGetErrorString(e)); }
+    if (geo->ws_bytes < need) {
+        if (geo->ws_scratch) { cudaStreamSynchronize(s); cudaFree(geo->ws_scratch); geo->ws_scratch = nullptr; geo->ws_bytes = 0; }
+        cudaError_t e = cudaMalloc((void**)&geo->ws_scratch, need);
+        if (e != cudaSuccess) { cudaGetLastError(); geo->ws_scratch = nullptr; return fail(GN_OUT_OF_MEMORY, std::string("gn_transport_run scratch: ") + cudaGetErrorString(e)); }
+        geo->ws_bytes = need;
+    }
+    if (!geo->ws_pinned && cudaMallocHost(&geo->ws_pinned, cb) != cudaSuccess) { cudaGetLastError(); geo->ws_pinned = nullptr; return fail(GN_OUT_OF_MEMORY, "gn_transport_run: pinned alloc"); }
+    if (!geo->ws_events_ok) {
+        bool ok = cudaEventCreate(&geo->ws_events[0]) == cudaSuccess && cudaEventCreate(&geo->ws_events[1]) == cudaSuccess;
+        for (int q = 0; q <= TR_LAG; ++q) ok = ok && cudaEventCreateWithFlags(&geo->ws_events[2 + q], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) { cudaGetLastError(); return fail(GN_CUDA_ERROR, "gn_transport_run: event create"); }
+        geo->ws_events_ok = true;
+    }
+    char* scratch = geo->ws_scratch;
     PhotonRec<R>* qa = (PhotonRec<R>*)scratch; PhotonRec<R>* qb_ = (PhotonRec<R>*)(scratch + qb);
     uint64_t* tmp_hash = hb ? (uint64_t*)(scratch + 2 * qb) : nullptr;
     DevStats* d_stats = (DevStats*)(scratch + 2 * qb + hb);
-    uint32_t* d_count = (uint32_t*)(scratch + 2 * qb + hb + 256);
-    uint32_t* h_count = nullptr;
+    PassCounters* d_ctr = (PassCounters*)(scratch + 2 * qb + hb + 512);
+    PassCounters* h_ctr = (PassCounters*)geo->ws_pinned;
     int rc = GN_OK;
     uint64_t passes = 0, launches = 0;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t ev0 = geo->ws_events[0], ev1 = geo->ws_events[1];
+    cudaEvent_t* ring = &geo->ws_events[2];
     double kernel_ms = 0.0;
-    auto cleanup = [&]() { if (h_count) cudaFreeHost(h_count); if (ev0) cudaEventDestroy(ev0); if (ev1) cudaEventDestroy(ev1); cudaFreeAsync(scratch, s); };
-    if (cudaMallocHost((void**)&h_count, 64) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_OUT_OF_MEMORY, "gn_transport_run: pinned alloc"); }
-    if (cudaEventCreate(&ev0) != cudaSuccess || cudaEventCreate(&ev1) != cudaSuccess) { cudaGetLastError(); cleanup(); return fail(GN_CUDA_ERROR, "gn_transport_run: event create"); }
+    cudaError_t e = cudaSuccess;
+    const unsigned tail = (unsigned)geo->opts.tail_photons;
     cudaMemsetAsync(d_stats, 0, 512, s);
     const GeoView<R>& g = view<R>(geo);
     for (int64_t done = 0; done < n_photons && rc == GN_OK; done += (int64_t)cap) {
-        uint32_t n_in = (uint32_t)std::min<int64_t>((int64_t)cap, n_photons - done);
+        const uint32_t n0 = (uint32_t)std::min<int64_t>((int64_t)cap, n_photons - done);
+        const uint64_t fid = (uint64_t)(first_id + done);
         PerPhotonOut pp{d_hash ? d_hash + done : tmp_hash, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
         PhotonRec<R>* in = qb_; PhotonRec<R>* out = qa;
-        bool first = true;
-        while (n_in > 0) {
-            cudaMemsetAsync(d_count, 0, 4, s);
-            unsigned blocks = (n_in + TR_THREADS - 1) / TR_THREADS;
-            cudaEventRecord(ev0, s);
-            if (first) {
-                if (track) transport_pass<R, true, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K0);
-                else transport_pass<R, true, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K0);
-            } else {
-                if (track) transport_pass<R, false, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
-                else transport_pass<R, false, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, (uint64_t)(first_id + done), n_in, in, out, d_count, d_edep, d_stats, pp, K);
+        cudaMemsetAsync(d_ctr, 0, cb, s);
+        cudaEventRecord(ev0, s);
+        // pass p reads counter p and adds to counter p + 1; the host enqueues passes back to back and learns the
+        // survivor counts TR_LAG passes late (upper bound for the grid; blocks past the true count return at once)
+        unsigned ub = n0;
+        bool finished = false;
+        for (int p = 0; !finished; ++p) {
+            if (p > TR_LAG) {
+                e = cudaEventSynchronize(ring[(p - TR_LAG) % (TR_LAG + 1)]);
+                if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pass"); break; }
+                ub = h_ctr[p - TR_LAG].front + h_ctr[p - TR_LAG].back;        // input count of pass p - TR_LAG >= that of pass p
+                if (ub == 0) break;
             }
+            const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
+            const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
+            if (p == 0) launch_pass<R, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0);
+            else launch_pass<R, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, last ? K_UNLIMITED : K);
             ++passes; ++launches;
             e = cudaGetLastError();
-            cudaEventRecord(ev1, s);
-            if (e == cudaSuccess) e = cudaMemcpyAsync(h_count, d_count, 4, cudaMemcpyDeviceToHost, s);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+            if (e == cudaSuccess && !last) {
+                e = cudaMemcpyAsync(&h_ctr[p + 1], d_ctr + p + 1, sizeof(PassCounters), cudaMemcpyDeviceToHost, s);
+                if (e == cudaSuccess) e = cudaEventRecord(ring[(p + 1) % (TR_LAG + 1)], s);
+            }
             if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pass"); break; }
-            { float ms = 0.f; if (cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
-            n_in = *h_count;
-            first = false;
+            finished = last;
             PhotonRec<R>* t = in; in = out; out = t;
         }
+        cudaEventRecord(ev1, s);
+        e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess && rc == GN_OK) rc = cuda_fail(e, "gn_transport_run batch");
+        { float ms = 0.f; if (rc == GN_OK && cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
     }
     if (rc == GN_OK) {
         DevStats hs;
@@ -409,13 +552,12 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) rc = cuda_fail(e, "gn_transport_run stats");
         else if (h_stats) {
-            h_stats->n_steps = hs.n_steps; h_stats->n_compton = hs.n_compton; h_stats->n_pe = hs.n_pe; h_stats->n_pair = hs.n_pair;
-            h_stats->n_cut = hs.n_cut; h_stats->n_escaped = hs.n_escaped; h_stats->n_stuck = hs.n_stuck; h_stats->n_photons = hs.n_photons;
-            h_stats->e_escaped = hs.e_escaped; h_stats->e_stuck = hs.e_stuck; h_stats->e_source = hs.e_source; h_stats->e_deposited = hs.e_deposited;
+            h_stats->n_steps = hs.cnt[ST_STEPS]; h_stats->n_compton = hs.cnt[ST_COMPTON]; h_stats->n_pe = hs.cnt[ST_PE]; h_stats->n_pair = hs.cnt[ST_PAIR];
+            h_stats->n_cut = hs.cnt[ST_CUT]; h_stats->n_escaped = hs.cnt[ST_ESCAPED]; h_stats->n_stuck = hs.cnt[ST_STUCK]; h_stats->n_photons = hs.cnt[ST_PHOTONS];
+            h_stats->e_escaped = hs.en[EN_ESCAPED]; h_stats->e_stuck = hs.en[EN_STUCK]; h_stats->e_source = hs.en[EN_SOURCE]; h_stats->e_deposited = hs.en[EN_DEPOSITED];
             h_stats->n_passes = passes; h_stats->n_kernel_launches = launches; h_stats->kernel_ms = kernel_ms;
         }
     }
-    cleanup();
     return rc;
 }
 

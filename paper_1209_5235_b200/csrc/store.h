@@ -1,16 +1,16 @@
-// store.h -- device-resident structure-of-arrays geometry store (what the kernels see).
+// store.h -- device-resident geometry store (what the kernels see).
 //
 // One GeoView<Real> per precision; built once by gn_geometry_create (geometry.cu) and passed to the
 // kernels by value.  Layout (all arrays in HBM, L2-resident for every BASELINE.json config):
-//   node[i]   int4  {parent, solid | flags, material, number of daughters}      16 B / node
+//   node[i]   NodeRec: everything a visit to node i needs in ONE 32-byte sector (fp32; 48 B in fp64):
+//               parent, solid | flags, material, number of daughters, link, Tg[3]
+//             link >= 0: first index into dlist (daughters in index order); link < 0: ~(voxel grid id)
 //             flag NODE_IDENTITY: the composed rotation is exactly the identity, so p_local = x - Tg and
 //             v_local = w (the general fma chain gives the same values; only the sign of zeros can differ,
-//             which no comparison in the navigator can see)
-//   kids[i]   int2  {first index into dlist (daughters in index order), voxel grid id or -1}
-//   xf[i]     12 Real: M (row-major, global->local rotation) then Tg; p_local = M (x - Tg)
-//             48 B (fp32, three 16-byte loads) / 96 B (fp64, six 16-byte loads); Tg sits in the last 16 / 32 B
-//   solids, mats: tiny tables (staged to shared memory by every kernel)
-//   grids[g]  header of the voxel grid of one mother
+//             which no comparison in the navigator can see) and `rot` is never read for this node
+//   rot[i]    M (row-major, global->local rotation), 9 Real padded to 12 (fp32, three 16-byte loads) /
+//             10 (fp64, five 16-byte loads);  p_local = M (x - Tg)
+//   solids, mats, grids: small tables (staged to shared memory by every kernel)
 //   cells[c]  int2 {x, count}: count == 1 -> x is the candidate daughter itself; else x = offset into cand
 #pragma once
 #include <cstdint>
@@ -30,6 +30,14 @@ template <class R> struct SolidRec {
 
 template <class R> struct MatRec { R aPE, aC, aP, capZ; };
 
+template <class R> struct NodeRec;
+template <> struct alignas(16) NodeRec<float> { int parent, info, mat, ndau; int link; float t[3]; };
+template <> struct alignas(16) NodeRec<double> { int parent, info, mat, ndau; int link, pad; double t[3]; };
+static_assert(sizeof(NodeRec<float>) == 32 && sizeof(NodeRec<double>) == 48, "node record layout");
+template <class R> struct RotStride;
+template <> struct RotStride<float> { static constexpr int value = 12; };
+template <> struct RotStride<double> { static constexpr int value = 10; };
+
 template <class R> struct GridRec {
     R gmin[3], inv_w[3], w[3], eps[3];   // eps = probe half-width in cell units (padded)
     int n[3];
@@ -37,10 +45,9 @@ template <class R> struct GridRec {
 };
 
 template <class R> struct GeoView {
-    const int4* node;
-    const int2* kids;
+    const NodeRec<R>* node;
+    const R* rot;
     const int* dlist;
-    const R* xf;
     const SolidRec<R>* solids;
     const MatRec<R>* mats;
     const GridRec<R>* grids;
@@ -48,7 +55,7 @@ template <class R> struct GeoView {
     const int* cand;
     R tol, delta, probe;  // surface tolerance, tol/2, voxel probe half-width
     R e_cut;
-    int n_nodes, n_solids, n_mats, stuck_limit;
+    int n_nodes, n_solids, n_mats, n_grids, stuck_limit;
 };
 
 }  // namespace gn

@@ -218,11 +218,14 @@ def test_transport_is_independent_of_steps_per_pass_and_sharding(B):
     import torch
     geom, src, n, seed = TRANSPORT_CASES["phantom16"]()
     runs = []
-    for K in (1, 7, 64):
-        g = B.Geometry(geom, steps_per_pass=K)
+    # tail_photons=1: no run-to-completion pass before a single photon is left, so the wavefront passes, the
+    # compaction and the front/back partition of the queues are all exercised; the default (one tail pass after
+    # the first, since n is small) must give the same histories
+    for K, tail in ((1, 1), (7, 1), (64, 1), (16, 0)):
+        g = B.Geometry(geom, steps_per_pass=K, tail_photons=tail)
         r = B.transport_run(g, src, seed, n, 64, per_photon=True)
         runs.append((r["hash"].cpu().numpy(), r["edep"].cpu().numpy(), r["stats"]))
-        assert r["stats"]["n_passes"] >= (2 if K == 64 else 8)
+        assert r["stats"]["n_passes"] >= (2 if (K == 64 or tail == 0) else 8)
     for h, e, s in runs[1:]:
         assert np.array_equal(h, runs[0][0]) and np.allclose(e, runs[0][1], rtol=1e-12, atol=1e-12)
         assert s["n_steps"] == runs[0][2]["n_steps"]
