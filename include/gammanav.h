@@ -148,6 +148,15 @@ int gn_nav_query_host(const gn_geometry* geo, int precision, const void* h_pos, 
 int gn_transport_run_host(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
                           int64_t first_photon_id, int64_t n_photons, double* h_edep_out, gn_run_stats* h_stats_out);
 
+/*
+ * gn_selftest_arith -- device self-test of the library's in-line correctly rounded fp32 division and square root
+ * (SURVEY 8(c) C0 "canonical arithmetic": navigation may only use correctly rounded + - x / sqrt) against the
+ * toolchain's IEEE intrinsics, bit for bit: all 2^32 square-root arguments and n_div_pairs pseudo-random /
+ * structured division pairs.  h_out[0] = sqrt mismatches, [1] = division mismatches, [2] / [3] = smallest failing
+ * argument index of each (all ones when none).  Synchronous; default stream.
+ */
+int gn_selftest_arith(int64_t n_div_pairs, uint64_t h_out[4]);
+
 const char* gn_last_error(void);
 const char* gn_version(void);
 

@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",
            "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_transport_run", "gn_nav_query_host",
-           "gn_transport_run_host", "gn_last_error", "gn_version")
+           "gn_transport_run_host", "gn_selftest_arith", "gn_last_error", "gn_version")
 
 
 class GammaNavError(RuntimeError):
@@ -68,6 +68,7 @@ def lib():
         L.gn_transport_run.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_nav_query_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.gn_selftest_arith.argtypes = [C.c_int64, C.c_void_p]
         L.gn_transport_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
@@ -219,3 +220,11 @@ def transport_run_host(geo: Geometry, source, seed, n_photons, precision=32, fir
     _check(lib().gn_transport_run_host(geo._h, precision, C.byref(cs), C.c_uint64(seed), C.c_int64(first_photon_id), C.c_int64(n_photons),
                                        edep.ctypes.data_as(C.c_void_p), C.byref(st)), "gn_transport_run_host")
     return {"edep": edep, "stats": st.as_dict()}
+
+
+def selftest_arith(n_div_pairs=1 << 30):
+    """gn_selftest_arith: in-line fp32 division / square root of the kernels vs. the IEEE intrinsics, bit for bit."""
+    _torch()
+    out = (C.c_uint64 * 4)()
+    _check(lib().gn_selftest_arith(C.c_int64(n_div_pairs), out), "gn_selftest_arith")
+    return {"sqrt_mismatches": out[0], "div_mismatches": out[1], "first_bad_sqrt": out[2], "first_bad_div": out[3]}

@@ -8,8 +8,8 @@
 //   * one wavefront pass = one launch of transport_pass: every thread loads one live photon, advances it by up
 //     to K steps (Algorithm 1 loop body: mu, s_int, ComputeStep, move / interact) keeping the node record of the
 //     current volume in registers, and survivors are compacted into the other queue with a ballot + block-
-//     aggregated atomic cursor, partitioned by a 1-bit key (solid type of the current volume) to the front /
-//     back of the queue; pass 0 generates the photons from the source and takes one step, so photons that miss
+//     aggregated atomic cursor, partitioned by a 1-bit key (photon parked at an interaction point or not) to the
+//     back / front of the queue; pass 0 generates the photons from the source and takes one step, so photons that miss
 //     everything leave the warps at once;
 //   * passes are chained on the device: a pass reads its input count from the counter its predecessor
 //     incremented, so the host enqueues passes back to back and only looks at counts that are two passes old;
@@ -213,7 +213,10 @@ __device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, uint
     io->j = rng.j;
 }
 
-template <class R, bool FROM_SOURCE, bool TRACK>
+// PHYS = false: the lean wavefront pass -- photons that reach an interaction point park there and are written to the
+// back of the output queue; interact_pass handles them before the next pass.  PHYS = true: interactions happen inside
+// the pass (batched per warp); used for the last pass, which runs the few remaining photons to completion.
+template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS>
 __global__ void __launch_bounds__(TR_THREADS)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
@@ -248,6 +251,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     uint64_t h = 0xcbf29ce484222325ull;
     int vol = -1; NodeRec<R> nd = {};
     unsigned c_steps = 0;
+    bool pending = false;       // the photon sits at its interaction point, waiting for an interaction phase
 
     if (FROM_SOURCE) {
         unsigned c_phot = 0; double e_src = 0.0;
@@ -268,17 +272,18 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         if (lane == 0) { atomicAdd(&sh_cnt[ST_PHOTONS], (unsigned long long)c_phot); atomicAdd(&sh_en[EN_SOURCE], e_src); }
     } else if (fate == FATE_ALIVE) {
         PhotonRec<R> r; load_rec(qin, i < n_front ? i : cap - 1u - (i - n_front), r);
+        if (r.vol < 0) fate = FATE_NONE;                 // absorbed by interact_pass
         x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
-        gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = (int)r.tail[0];
+        gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = (int)(r.tail[0] & 1u); pending = (r.tail[0] & 2u) != 0;
         idx = r.idx; misc = r.misc; ctr = r.ctr; vol = r.vol;
-        nd = nav.node(vol);
-        if (TRACK) h = pp.hash[idx];
+        if (fate == FATE_ALIVE) { nd = nav.node(vol); if (TRACK) h = pp.hash[idx]; }
     }
 
     // A lane whose photon reaches its interaction point parks there (pending) instead of running the rare, long
     // physics alone with 31 lanes idle; the warp runs one interaction phase for all parked lanes once
-    // INTERACT_BATCH of them wait, or when nothing else is left to do (group by event type).
-    bool pending = false;
+    // INTERACT_BATCH of them wait, or when nothing else is left to do.  Photons still parked when the pass ends
+    // are written to the BACK of the output queue (key = event type), so the next pass finds
+    // them packed into full warps.
     auto finish_step = [&](int ev, int vol_before) {          // stuck guard (C9) + history hash; after the step's event
         if (fate == FATE_ALIVE && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; fate = FATE_STUCK; }
         if (TRACK) {
@@ -288,10 +293,10 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     };
 #pragma unroll 1
     for (int k = 0;;) {
-        const unsigned pen = __ballot_sync(0xffffffffu, pending);
+        const unsigned pen = PHYS ? __ballot_sync(0xffffffffu, pending) : 0u;
         const unsigned act = __ballot_sync(0xffffffffu, fate == FATE_ALIVE && !pending);
         const bool budget = k < K;
-        if (pen && (act == 0 || !budget || __popc(pen) >= INTERACT_BATCH)) {
+        if (PHYS && budget && pen && (act == 0 || __popc(pen) >= INTERACT_BATCH)) {
             // ---- interaction phase (A6-A9) ----------------------------------------------------------------------
             double dep_d = 0.0;
             if (pending) {
@@ -353,7 +358,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 
     // ---- compaction of survivors into the other queue, partitioned by key -------------------
     const bool alive = fate == FATE_ALIVE;
-    const bool key1 = alive && nav.solid_of(nd).type != SOLID_BOX;
+    const bool key1 = alive && pending;
     const unsigned bal0 = __ballot_sync(0xffffffffu, alive && !key1), bal1 = __ballot_sync(0xffffffffu, key1);
     if (lane == 0) { sh_wcount[0][warp] = __popc(bal0); sh_wcount[1][warp] = __popc(bal1); }
     __syncthreads();
@@ -372,7 +377,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         r.gPE = gPE; r.gKN = gKN; r.L2k = L2k; r.vol = vol; r.idx = idx; r.ctr = ctr; r.misc = misc;
 #pragma unroll
         for (int q = 0; q < (int)(sizeof(r.tail) / 4); ++q) r.tail[q] = 0;
-        r.tail[0] = (uint32_t)above;
+        r.tail[0] = (uint32_t)above | (pending ? 2u : 0u);
         store_rec(qout, o, r);
         if (TRACK) pp.hash[idx] = h;
     }
@@ -390,6 +395,64 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             if (lane == 0) { atomicAdd(&sh_cnt[ST_STUCK], (unsigned long long)ns); atomicAdd(&sh_en[EN_STUCK], es); }
         }
     }
+    __syncthreads();
+    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+}
+
+// The interaction wavefront (A6-A9): every photon parked at an interaction point by the previous pass sits in the
+// back segment of the queue (slots cap-1, cap-2, ...); one thread per photon samples the process, updates the record
+// in place (absorbed photons are marked vol = -1) and the warp tallies the deposits.
+template <class R, bool TRACK>
+__global__ void __launch_bounds__(TR_THREADS)
+interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters* __restrict__ cin, PhotonRec<R>* __restrict__ q, uint32_t cap,
+              double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp) {
+    const unsigned n = cin->back;
+    if (blockIdx.x * TR_THREADS >= n) return;
+    __shared__ unsigned long long sh_cnt[8];
+    __shared__ double sh_en[4];
+    if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
+    if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
+    __syncthreads();
+    const unsigned i = blockIdx.x * TR_THREADS + threadIdx.x;
+    const bool active = i < n;
+    double dep_d = 0.0; int vol = 0;
+    if (active) {
+        PhotonRec<R> r; load_rec(q, cap - 1u - i, r);
+        vol = r.vol;
+        const int above = (int)(r.tail[0] & 1u);
+        const MatRec<R> m = g.mats[__ldg(&g.node[vol].mat)];
+        const R muPE = m.aPE * r.gPE, muC = m.aC * r.gKN;
+        const R P = rmin((R)(28.0 / 9.0) * r.L2k - (R)(218.0 / 27.0), m.capZ);
+        const R muP = (above && P > 0) ? m.aP * P : (R)0;
+        const R mu = (muPE + muC) + muP;
+        InteractIO<R> io;
+        io.E = r.E; io.wx = r.wx; io.wy = r.wy; io.wz = r.wz; io.Y = r.Y; io.gPE = r.gPE; io.gKN = r.gKN; io.L2k = r.L2k; io.j = r.ctr; io.above = above;
+        interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + r.idx);
+        int ev = io.ev;
+        dep_d = (double)io.dep;
+        bool alive = false;
+        if (ev == EV_COMPTON || ev == EV_CUT) {
+            r.E = io.E; r.wx = io.wx; r.wy = io.wy; r.wz = io.wz;
+            atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
+            if (ev == EV_CUT) atomicAdd(&sh_cnt[ST_CUT], 1ull);
+            else { r.Y = io.Y; r.gPE = io.gPE; r.gKN = io.gKN; r.L2k = io.L2k; r.tail[0] = (uint32_t)io.above; alive = true; }
+        } else atomicAdd(&sh_cnt[ev == EV_PE ? ST_PE : ST_PAIR], 1ull);
+        r.ctr = io.j;
+        if (alive && (r.misc & 0xffu) >= (uint32_t)g.stuck_limit) {           // stuck guard (C9), after the step's event
+            ev = EV_STUCK; alive = false;
+            atomicAdd(&sh_cnt[ST_STUCK], 1ull); atomicAdd(&sh_en[EN_STUCK], (double)r.E);
+        }
+        if (TRACK) {
+            uint64_t h = pp.hash[r.idx];
+            fnv_word(h, (uint32_t)vol); fnv_word(h, (uint32_t)ev);
+            pp.hash[r.idx] = h;
+            if (!alive) { if (pp.nsteps) pp.nsteps[r.idx] = r.misc >> 8; if (pp.efinal) pp.efinal[r.idx] = (double)r.E; }
+        }
+        if (alive) r.tail[0] &= 1u; else r.vol = -1;
+        store_rec(q, cap - 1u - i, r);
+    }
+    warp_tally(edep, &sh_en[EN_DEPOSITED], vol, dep_d, active);
     __syncthreads();
     if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
@@ -458,12 +521,18 @@ constexpr int TR_MAX_PASSES = 4096;         // device counters per batch; the la
 constexpr int TR_LAG = 2;                   // the host looks at survivor counts that are this many passes old
 constexpr int K_UNLIMITED = 0x7fffffff;
 
-template <class R, bool SRC>
+template <class R, bool SRC, bool PHYS>
 static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
                         uint32_t n_src, const PassCounters* cin, PassCounters* cout, const PhotonRec<R>* qin, PhotonRec<R>* qout, uint32_t cap,
                         double* edep, DevStats* stats, PerPhotonOut pp, int K) {
-    if (track) transport_pass<R, SRC, true><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
-    else transport_pass<R, SRC, false><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
+    if (track) transport_pass<R, SRC, true, PHYS><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
+    else transport_pass<R, SRC, false, PHYS><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
+}
+template <class R>
+static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, uint64_t seed, uint64_t first_id, const PassCounters* cin,
+                            PhotonRec<R>* q, uint32_t cap, double* edep, DevStats* stats, PerPhotonOut pp) {
+    if (track) interact_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp);
+    else interact_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp);
 }
 
 template <class R>
@@ -529,8 +598,14 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             }
             const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
             const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
-            if (p == 0) launch_pass<R, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0);
-            else launch_pass<R, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, last ? K_UNLIMITED : K);
+            if (p == 0) launch_pass<R, true, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0);
+            else if (last) launch_pass<R, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED);
+            else {
+                // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
+                launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp);
+                launch_pass<R, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K);
+                ++launches;
+            }
             ++passes; ++launches;
             e = cudaGetLastError();
             if (e == cudaSuccess && !last) {
@@ -632,5 +707,61 @@ extern "C" int gn_transport_run_host(const gn_geometry* geo, int precision, cons
     cudaFree(d);
     if (rc != GN_OK) return rc;
     if (e != cudaSuccess) return cuda_fail(e, "gn_transport_run_host");
+    return GN_OK;
+}
+
+// -------------------------------------------------------------------------------------------------------
+// arithmetic self-test: the in-line correctly rounded fp32 division / square root of nav.cuh against the
+// toolchain's __fdiv_rn / __fsqrt_rn (IEEE round-to-nearest), bit for bit
+// -------------------------------------------------------------------------------------------------------
+namespace gn {
+__device__ __forceinline__ uint32_t mix32(uint64_t z) {          // splitmix64 finaliser
+    z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull; z = (z ^ (z >> 27)) * 0x94d049bb133111ebull; z ^= z >> 31;
+    return (uint32_t)(z >> 16);
+}
+__global__ void selftest_sqrt_kernel(unsigned long long* out) {
+    unsigned bad = 0;
+    for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < (1ull << 32); i += (uint64_t)gridDim.x * blockDim.x) {
+        float a = __uint_as_float((uint32_t)i);
+        float mine = rsqrt_(a), ref = __fsqrt_rn(a);
+        bool same = __float_as_uint(mine) == __float_as_uint(ref) || (mine != mine && ref != ref);
+        if (!same) { ++bad; atomicMin(&out[2], (unsigned long long)i); }
+    }
+    if (bad) atomicAdd(&out[0], (unsigned long long)bad);
+}
+__global__ void selftest_div_kernel(unsigned long long n, unsigned long long* out) {
+    unsigned bad = 0;
+    for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        uint32_t ua = mix32(2 * i + 1), ub = mix32(2 * i + 2) ^ 0x9e3779b9u;
+        const unsigned mode = (unsigned)(i & 3);
+        if (mode == 1) {                      // exponents of lengths and direction cosines: 2^-24 .. 2^16
+            ua = (ua & 0x807fffffu) | ((103u + (ua >> 23) % 40u) << 23); ub = (ub & 0x807fffffu) | ((103u + (ub >> 23) % 40u) << 23);
+        } else if (mode == 2) {               // quotient just below / above a power of two and a rounding boundary
+            ub = (ub & 0x807fffffu) | (127u << 23); ua = (ua & 0x80000000u) | ((ub & 0x7fffffffu) + (ua & 3u) - 1u);
+        } else if (mode == 3) {               // few mantissa bits: exact and half-way cases
+            ua &= 0xfff80000u; ub &= 0xffe00000u;
+        }
+        float a = __uint_as_float(ua), b = __uint_as_float(ub);
+        float mine = rdiv(a, b), ref = __fdiv_rn(a, b);
+        bool same = __float_as_uint(mine) == __float_as_uint(ref) || (mine != mine && ref != ref);
+        const float ar = fabsf(ref);
+        if (!same && ar < 1.17549435e-38f) same = fabsf(mine) < 1.17549435e-38f * 1.0001f;      // subnormal quotients: out of contract
+        if (!same) { ++bad; atomicMin(&out[3], (unsigned long long)i); }
+    }
+    if (bad) atomicAdd(&out[1], (unsigned long long)bad);
+}
+}  // namespace gn
+
+extern "C" int gn_selftest_arith(int64_t n_div_pairs, uint64_t h_out[4]) {
+    if (!h_out || n_div_pairs < 0) return fail(GN_INVALID_ARGUMENT, "gn_selftest_arith: bad argument");
+    unsigned long long* d = nullptr;
+    if (cudaMalloc((void**)&d, 32) != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, "gn_selftest_arith: cudaMalloc"); }
+    unsigned long long init[4] = {0, 0, ~0ull, ~0ull};
+    cudaMemcpy(d, init, 32, cudaMemcpyHostToDevice);
+    selftest_sqrt_kernel<<<148 * 16, 256>>>(d);
+    if (n_div_pairs > 0) selftest_div_kernel<<<148 * 16, 256>>>((unsigned long long)n_div_pairs, d);
+    cudaError_t e = cudaMemcpy(h_out, d, 32, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "gn_selftest_arith");
     return GN_OK;
 }

@@ -327,3 +327,12 @@ def test_config2_and_config4_reduced_counts(B):
     wl = W.config(4)
     compare_transport(B, wl.geometry, wl.source, 30000, wl.seed, 32, 0.97)
     compare_transport(B, wl.geometry, wl.source, 30000, wl.seed, 64, 0.999)
+
+
+def test_inline_division_and_sqrt_are_correctly_rounded(B):
+    """navigation may only use correctly rounded operations.  The kernels use their own in-line
+    Newton-Raphson division / square root (no out-of-line slow path); on the device they must equal the IEEE
+    round-to-nearest intrinsics bit for bit: every fp32 square-root argument, 2^31 division pairs."""
+    r = B.selftest_arith(1 << 31)
+    assert r["sqrt_mismatches"] == 0, r
+    assert r["div_mismatches"] == 0, r
