@@ -171,7 +171,14 @@ def run_ours(args):
     if args.precision:
         precision = args.precision
     n = int(wl.n * args.scale)
-    geo = B.Geometry(wl.geometry, **({"steps_per_pass": args.steps_per_pass} if args.steps_per_pass else {}))
+    gopts = {}
+    if args.steps_per_pass:
+        gopts["steps_per_pass"] = args.steps_per_pass
+    if args.tail_photons:
+        gopts["tail_photons"] = args.tail_photons
+    if args.first_pass_steps:
+        gopts["first_pass_steps"] = args.first_pass_steps
+    geo = B.Geometry(wl.geometry, **gopts)
     transport = wl.source is not None
     first_id = rank * n                                       # weak scaling: same work per GPU, disjoint ids
     dev = torch.device("cuda", local)
@@ -307,6 +314,8 @@ def main():
     ap.add_argument("--precision", type=int, default=0, choices=[0, 32, 64])
     ap.add_argument("--scale", type=float, default=1.0, help="fraction of the workload's photons/queries (diagnostics only)")
     ap.add_argument("--steps-per-pass", type=int, default=0)
+    ap.add_argument("--tail-photons", type=int, default=0, help="diagnostics: override gn_opts.tail_photons")
+    ap.add_argument("--first-pass-steps", type=int, default=0, help="diagnostics: override gn_opts.first_pass_steps")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-all-cores", action="store_true")
     ap.add_argument("--allow-short-warmup", action="store_true")
