@@ -295,8 +295,11 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         for (int k = 0; k < 3; ++k) {
             a.gmin[k] = (float)G.gmin[k]; a.w[k] = (float)G.w[k]; a.inv_w[k] = (float)(1.0 / G.w[k]); a.n[k] = G.n[k];
             b.gmin[k] = G.gmin[k]; b.w[k] = G.w[k]; b.inv_w[k] = 1.0 / G.w[k]; b.n[k] = G.n[k];
-            // probe half-width in cell units, 1.5 x for the rounding of the index arithmetic itself
-            a.eps[k] = (float)(1.5 * probe32 / G.w[k]); b.eps[k] = 1.5 * probe64 / G.w[k];
+            // probe half-width in cell units.  A daughter that is not listed in the cell holding the point can only be
+            // occupied / hit if the point (ray) comes within delta = tol / 2 of that cell's boundary: 1.25 delta, plus
+            // a guard for the rounding of the index arithmetic itself (a few ulp of the largest cell coordinate).
+            a.eps[k] = (float)(1.25 * 0.5 * probe32 / G.w[k] + 8.0 * G.n[k] * 0x1p-23);
+            b.eps[k] = 1.25 * 0.5 * probe64 / G.w[k] + 8.0 * G.n[k] * 0x1p-52;
         }
         a.cell_base = b.cell_base = G.cell_base;
         g32.push_back(a); g64.push_back(b);

@@ -107,6 +107,36 @@ def test_voxel_walk_matches_linear_scan_oracle(B):
         assert (rnxt[in_world] > 0).sum() > 1000         # many rays do hit a daughter through the walk
 
 
+def test_points_in_the_tolerance_band_of_voxel_faces(B):
+    """The voxel grid lists a daughter only in the cells its own box overlaps and probes the neighbouring cells
+    when the point is within 1.25 delta of a cell boundary.  Points at k * delta from voxel faces, edges and
+    corners (k on both sides of every threshold in that argument) must locate and step exactly as the oracle."""
+    geom = GEOMS["phantom12"]()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    rng = np.random.default_rng(77)
+    n = 60000
+    for precision in (32, 64):
+        R = np.float64 if precision == 64 else np.float32
+        delta = g.tolerance(precision) / 2
+        base = np.round(rng.uniform(-12, 12, size=(n, 3)) / 2.0) * 2.0              # voxel corners (2 mm pitch)
+        free = rng.uniform(-12, 12, size=(n, 3))
+        on = rng.integers(0, 2, size=(n, 3)).astype(bool); on[:, 0] |= ~on.any(axis=1)   # which coordinates sit on a face
+        k = rng.choice([-3.0, -2.0, -1.3, -1.2, -1.0, -0.9, -0.5, 0.0, 0.5, 0.9, 1.0, 1.2, 1.3, 2.0, 3.0], size=(n, 3))
+        p = np.where(on, base + k * delta, free).astype(R)
+        v = unit(rng, n).astype(R)
+        v[: n // 4] = np.where(on[: n // 4], 0.0, v[: n // 4]).astype(R)            # some rays run along the faces
+        nz = np.linalg.norm(v, axis=1) == 0
+        v[nz] = np.array([0, 0, 1], R)
+        v = (v / np.linalg.norm(v, axis=1, keepdims=True)).astype(R)
+        tp, tv = cuda(p), cuda(v)
+        ref = og.locate(p, v, precision)
+        assert np.array_equal(B.nav_locate(g, tp, tv).cpu().numpy(), ref)
+        assert np.array_equal(B.nav_locate(g, tp, None).cpu().numpy(), og.locate(p, None, precision))
+        step, nxt = B.nav_compute_step(g, tp, tv, cuda(ref))
+        rstep, rnxt = og.compute_step(p, v, ref, None, precision)
+        assert np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(step.cpu().numpy(), rstep)
+
+
 def test_nav_edge_cases(B):
     import torch
     geom = GEOMS["slab"]()
