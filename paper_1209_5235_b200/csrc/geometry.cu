@@ -298,8 +298,10 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             // probe half-width in cell units.  A daughter that is not listed in the cell holding the point can only be
             // occupied / hit if the point (ray) comes within delta = tol / 2 of that cell's boundary: 1.25 delta, plus
             // a guard for the rounding of the index arithmetic itself (a few ulp of the largest cell coordinate).
-            a.eps[k] = (float)(1.25 * 0.5 * probe32 / G.w[k] + 8.0 * G.n[k] * 0x1p-23);
-            b.eps[k] = 1.25 * 0.5 * probe64 / G.w[k] + 8.0 * G.n[k] * 0x1p-52;
+            const float e32 = (float)(1.25 * 0.5 * probe32 / G.w[k] + 8.0 * G.n[k] * 0x1p-23);
+            const double e64 = 1.25 * 0.5 * probe64 / G.w[k] + 8.0 * G.n[k] * 0x1p-52;
+            (k == 0 ? a.eps0 : (k == 1 ? a.eps1 : a.eps2)) = e32;
+            (k == 0 ? b.eps0 : (k == 1 ? b.eps1 : b.eps2)) = e64;
         }
         a.cell_base = b.cell_base = G.cell_base;
         g32.push_back(a); g64.push_back(b);

@@ -205,13 +205,14 @@ __device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R
 // photon birth (C8, Algorithm 1 steps 1-2), out of line: source sampling, energy factors, first optical depth
 template <class R> struct BirthIO { R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k; uint32_t j; int above; };
 template <class R>
-__device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, uint64_t seed, uint64_t id) {
+__device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, const EnergyFactors<R>* mono, uint64_t seed, uint64_t id) {
     PhiloxStream rng; rng.init(seed, id, 0);
     V3<R> x, w; R E;
     sample_source(*src, rng, x, w, E);
     io->x = x.x; io->y = x.y; io->z = x.z; io->wx = w.x; io->wy = w.y; io->wz = w.z; io->E = E;
     io->Y = -rlog(draw<R>(rng));                       // Algorithm 1 steps 1-2
-    EnergyFactors<R> ef = energy_factors(E);
+    // mono-energetic source: the factors of E0 were evaluated once per block (same function, same value)
+    EnergyFactors<R> ef = mono ? *mono : energy_factors(E);
     io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
     io->j = rng.j;
 }
@@ -233,6 +234,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     __shared__ BlockTables<R> tab;
     __shared__ MatRec<R> sh_mats[MAX_SMEM_MATS];
     __shared__ SourceDev<R> sh_src;
+    __shared__ EnergyFactors<R> sh_mono;
     __shared__ unsigned sh_wcount[2][TR_WARPS];
     __shared__ unsigned sh_base[2];
     __shared__ unsigned long long sh_cnt[8];
@@ -240,7 +242,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     stage_tables(g, tab);
     const MatRec<R>* mats = g.mats;
     if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
-    if (FROM_SOURCE && threadIdx.x == 0) sh_src = src;
+    if (FROM_SOURCE && threadIdx.x == 0) { sh_src = src; if (src.energy_kind == 0) sh_mono = energy_factors(src.e0); }
     if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
@@ -261,7 +263,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         if (fate == FATE_ALIVE) {
             idx = i;
             BirthIO<R> b;
-            birth(&b, &sh_src, seed, first_id + i);
+            birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, seed, first_id + i);
             x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
             gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
             c_phot = 1; e_src = (double)E;

@@ -38,10 +38,14 @@ template <class R> struct RotStride;
 template <> struct RotStride<float> { static constexpr int value = 12; };
 template <> struct RotStride<double> { static constexpr int value = 10; };
 
-template <class R> struct GridRec {
-    R gmin[3], inv_w[3], w[3], eps[3];   // eps = probe half-width in cell units (padded)
+// header of one voxel grid; laid out so that the fields a cell lookup needs come in 16-byte words
+template <class R> struct alignas(16) GridRec {
+    R gmin[3], eps0;      // eps = probe half-width in cell units (padded), split over the three words
+    R inv_w[3], eps1;
     int n[3];
     int cell_base;        // offset of this grid's cells in `cells`
+    R w[3], eps2;
+    __host__ __device__ R eps(int k) const { return k == 0 ? eps0 : (k == 1 ? eps1 : eps2); }
 };
 
 template <class R> struct GeoView {
