@@ -72,7 +72,11 @@ typedef struct {
     double e_escaped, e_stuck, e_source, e_deposited;
     uint64_t n_passes;         /* wavefront passes (kernel launches of the step kernel) */
     uint64_t n_kernel_launches;/* all kernels launched by the call */
-    double kernel_ms;          /* sum of the step-kernel launch durations, CUDA events on the launching stream */
+    double kernel_ms;          /* duration of the whole kernel sequence of the run (source pass, step passes, interaction
+                                  passes, tail), CUDA events on the launching stream */
+    double step_pass_ms;       /* sum of the launch durations of the lean wavefront step passes (the dominant kernel), one
+                                  CUDA-event pair per launch (first 24 passes of each batch) */
+    uint64_t n_steps_step_pass;/* steps taken inside those passes */
 } gn_run_stats;
 
 /*

@@ -38,7 +38,8 @@ class CSource(C.Structure):
 class RunStats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons")] + \
                [(n, C.c_double) for n in ("e_escaped", "e_stuck", "e_source", "e_deposited")] + \
-               [("n_passes", C.c_uint64), ("n_kernel_launches", C.c_uint64), ("kernel_ms", C.c_double)]
+               [("n_passes", C.c_uint64), ("n_kernel_launches", C.c_uint64), ("kernel_ms", C.c_double), ("step_pass_ms", C.c_double),
+                ("n_steps_step_pass", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

@@ -21,7 +21,7 @@ struct gn_geometry {
     mutable char* ws_scratch = nullptr;
     mutable size_t ws_bytes = 0;
     mutable void* ws_pinned = nullptr;
-    mutable cudaEvent_t ws_events[8] = {};
+    mutable cudaEvent_t ws_events[8 + 48] = {};
     mutable bool ws_events_ok = false;
 };
 

@@ -109,6 +109,7 @@ enum : int { EN_ESCAPED = 0, EN_STUCK, EN_SOURCE, EN_DEPOSITED };
 
 struct DevStats {
     unsigned long long cnt[8];       // ST_*
+    unsigned long long lean_steps;   // steps taken inside the lean wavefront passes (the dominant kernel)
     double en[4];                    // EN_*
 };
 // survivors of a pass: key-0 photons fill the output queue from the front, key-1 photons from the back
@@ -403,6 +404,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     __syncthreads();
     if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+    if (!FROM_SOURCE && !PHYS && threadIdx.x == 12 && sh_cnt[ST_STEPS]) atomicAdd(&stats->lean_steps, sh_cnt[ST_STEPS]);
 }
 
 // The interaction wavefront (A6-A9): every photon parked at an interaction point by the previous pass sits in the
@@ -525,6 +527,7 @@ constexpr int64_t TR_BATCH = 1ll << 24;     // photons per batch (bounds scratch
 constexpr int TR_MAX_PASSES = 4096;         // device counters per batch; the last one always runs to completion
 constexpr int TR_LAG = 2;                   // the host looks at survivor counts that are this many passes old
 constexpr int K_UNLIMITED = 0x7fffffff;
+constexpr int TR_TIMED = 24;                // lean step passes per batch timed one by one (CUDA events around the launch)
 
 template <class R, bool SRC, bool PHYS>
 static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
@@ -565,6 +568,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     if (!geo->ws_events_ok) {
         bool ok = cudaEventCreate(&geo->ws_events[0]) == cudaSuccess && cudaEventCreate(&geo->ws_events[1]) == cudaSuccess;
         for (int q = 0; q <= TR_LAG; ++q) ok = ok && cudaEventCreateWithFlags(&geo->ws_events[2 + q], cudaEventDisableTiming) == cudaSuccess;
+        for (int q = 0; q < 2 * TR_TIMED; ++q) ok = ok && cudaEventCreate(&geo->ws_events[8 + q]) == cudaSuccess;
         if (!ok) { cudaGetLastError(); return fail(GN_CUDA_ERROR, "gn_transport_run: event create"); }
         geo->ws_events_ok = true;
     }
@@ -578,7 +582,8 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     uint64_t passes = 0, launches = 0;
     cudaEvent_t ev0 = geo->ws_events[0], ev1 = geo->ws_events[1];
     cudaEvent_t* ring = &geo->ws_events[2];
-    double kernel_ms = 0.0;
+    double kernel_ms = 0.0, step_pass_ms = 0.0;
+    cudaEvent_t* tev = &geo->ws_events[8];
     cudaError_t e = cudaSuccess;
     const unsigned tail = (unsigned)geo->opts.tail_photons;
     cudaMemsetAsync(d_stats, 0, 512, s);
@@ -594,6 +599,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         // survivor counts TR_LAG passes late (upper bound for the grid; blocks past the true count return at once)
         unsigned ub = n0;
         bool finished = false;
+        int n_timed = 0;
         for (int p = 0; !finished; ++p) {
             if (p > TR_LAG) {
                 e = cudaEventSynchronize(ring[(p - TR_LAG) % (TR_LAG + 1)]);
@@ -608,7 +614,9 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
                 launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp);
+                if (n_timed < TR_TIMED) cudaEventRecord(tev[2 * n_timed], s);
                 launch_pass<R, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K);
+                if (n_timed < TR_TIMED) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
                 ++launches;
             }
             ++passes; ++launches;
@@ -625,6 +633,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         e = cudaStreamSynchronize(s);
         if (e != cudaSuccess && rc == GN_OK) rc = cuda_fail(e, "gn_transport_run batch");
         { float ms = 0.f; if (rc == GN_OK && cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
+        for (int q = 0; q < n_timed && rc == GN_OK; ++q) { float ms = 0.f; if (cudaEventElapsedTime(&ms, tev[2 * q], tev[2 * q + 1]) == cudaSuccess) step_pass_ms += ms; }
     }
     if (rc == GN_OK) {
         DevStats hs;
@@ -636,6 +645,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             h_stats->n_cut = hs.cnt[ST_CUT]; h_stats->n_escaped = hs.cnt[ST_ESCAPED]; h_stats->n_stuck = hs.cnt[ST_STUCK]; h_stats->n_photons = hs.cnt[ST_PHOTONS];
             h_stats->e_escaped = hs.en[EN_ESCAPED]; h_stats->e_stuck = hs.en[EN_STUCK]; h_stats->e_source = hs.en[EN_SOURCE]; h_stats->e_deposited = hs.en[EN_DEPOSITED];
             h_stats->n_passes = passes; h_stats->n_kernel_launches = launches; h_stats->kernel_ms = kernel_ms;
+            h_stats->step_pass_ms = step_pass_ms; h_stats->n_steps_step_pass = hs.lean_steps;
         }
     }
     return rc;

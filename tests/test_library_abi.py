@@ -35,7 +35,7 @@ def test_struct_layouts_match_header():
     from paper_1209_5235_b200 import binding as B
     assert C.sizeof(B.Opts) == 4 * 8 + 6 * 4
     assert C.sizeof(B.CSource) == 8 + 6 * 8 + 4 * 8
-    assert C.sizeof(B.RunStats) == 8 * 8 + 4 * 8 + 2 * 8 + 8
+    assert C.sizeof(B.RunStats) == 8 * 8 + 4 * 8 + 2 * 8 + 8 + 2 * 8
 
 
 def test_no_cpu_fallback(lib):
