@@ -192,6 +192,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     if (o.steps_per_pass <= 0) o.steps_per_pass = 16;
     if (o.first_pass_steps <= 0) o.first_pass_steps = 1;
     if (o.tail_photons <= 0) o.tail_photons = 148 * 512;
+    const bool regroup_default = o.regroup_percent <= 0;
     o.tol64 = geo->tol64; o.tol32 = geo->tol32;
     geo->opts = o;
 
@@ -227,20 +228,51 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             int k = (G.n[0] >= G.n[1] && G.n[0] >= G.n[2]) ? 0 : (G.n[1] >= G.n[2] ? 1 : 2);
             G.n[k] = (G.n[k] + 1) / 2;
         }
+        // cell range of daughter j along axis k for a grid of n cells
+        auto cell_range = [&](int j, int k, int n, int& a, int& b) {
+            const double w = (mhi[k] - mlo[k]) / n, top = n - 1.0;
+            double fa = std::floor((blo[3 * (size_t)j + k] + shrink - mlo[k]) / w), fb = std::floor((bhi[3 * (size_t)j + k] - shrink - mlo[k]) / w);
+            fa = std::min(std::max(fa, 0.0), top); fb = std::min(std::max(fb, 0.0), top);
+            if (fb < fa) fb = fa;
+            a = (int)fa; b = (int)fb;
+        };
+        // refinement (the smart-voxel idea of choosing the cut that minimises candidate references): while cells hold
+        // more than ~1 candidate on average, double the axis whose doubling shortens the lists most, within a budget of
+        // 64 cells per daughter.  Short, equally long lists keep the lanes of a warp in step during relocation.
+        auto list_stats = [&](const int n[3], double& refs, double& nonempty) {
+            std::vector<int> cnt((size_t)n[0] * n[1] * n[2], 0);
+            for (int j = 0; j < nd; ++j) {
+                int a[3], b[3];
+                for (int k = 0; k < 3; ++k) cell_range(j, k, n[k], a[k], b[k]);
+                for (int iz = a[2]; iz <= b[2]; ++iz) for (int iy = a[1]; iy <= b[1]; ++iy) for (int ix = a[0]; ix <= b[0]; ++ix)
+                    cnt[ix + (size_t)n[0] * (iy + (size_t)n[1] * iz)]++;
+            }
+            refs = 0; nonempty = 0;
+            for (int c : cnt) if (c) { refs += c; nonempty += 1; }
+        };
+        {
+            const double refine_budget = std::max(64.0 * nd, 4096.0);
+            double refs, nonempty; list_stats(G.n, refs, nonempty);
+            while (nonempty > 0 && refs > 1.25 * nonempty) {
+                int best_k = -1; double best_avg = 0.97 * refs / nonempty;
+                for (int k = 0; k < 3; ++k) {
+                    if (G.n[k] * 2 > 1024 || 2.0 * G.n[0] * G.n[1] * G.n[2] > refine_budget) continue;
+                    int t[3] = {G.n[0], G.n[1], G.n[2]}; t[k] *= 2;
+                    double r, ne; list_stats(t, r, ne);
+                    if (ne > 0 && r / ne < best_avg) { best_avg = r / ne; best_k = k; }
+                }
+                if (best_k < 0) break;
+                G.n[best_k] *= 2;
+                list_stats(G.n, refs, nonempty);
+            }
+        }
         for (int k = 0; k < 3; ++k) { G.gmin[k] = mlo[k]; G.w[k] = (mhi[k] - mlo[k]) / G.n[k]; }
         size_t ncell = (size_t)G.n[0] * G.n[1] * G.n[2];
         G.cell_base = (int)cell_start.size() - 1;
         std::vector<int> count(ncell, 0);
         std::vector<int> c0(3 * (size_t)nd), c1(3 * (size_t)nd);
         for (int j = 0; j < nd; ++j) {
-            for (int k = 0; k < 3; ++k) {
-                double top = G.n[k] - 1.0;
-                double a = std::floor((blo[3 * (size_t)j + k] + shrink - G.gmin[k]) / G.w[k]);
-                double b = std::floor((bhi[3 * (size_t)j + k] - shrink - G.gmin[k]) / G.w[k]);
-                a = std::min(std::max(a, 0.0), top); b = std::min(std::max(b, 0.0), top);
-                if (b < a) b = a;
-                c0[3 * (size_t)j + k] = (int)a; c1[3 * (size_t)j + k] = (int)b;
-            }
+            for (int k = 0; k < 3; ++k) cell_range(j, k, G.n[k], c0[3 * (size_t)j + k], c1[3 * (size_t)j + k]);
             for (int iz = c0[3 * (size_t)j + 2]; iz <= c1[3 * (size_t)j + 2]; ++iz)
                 for (int iy = c0[3 * (size_t)j + 1]; iy <= c1[3 * (size_t)j + 1]; ++iy)
                     for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
@@ -310,6 +342,13 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     for (size_t c = 0; c + 1 < cell_start.size(); ++c) {
         int cnt = cell_start[c + 1] - cell_start[c];
         cells[c] = make_int2(cnt == 1 ? cand[cell_start[c]] : cell_start[c], cnt);
+    }
+    {
+        bool coherent = true;
+        for (size_t i = 0; i < V; ++i) coherent = coherent && solids[node[i].y].type == GN_BOX && (n32[i].info & NODE_IDENTITY);
+        for (const int2& c : cells) coherent = coherent && c.y <= 1;
+        geo->coherent = coherent;
+        if (regroup_default) geo->opts.regroup_percent = coherent ? 50 : 75;
     }
     Uploader up{geo};
     const int* d_dlist = up.put(dlist);

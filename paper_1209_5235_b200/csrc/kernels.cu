@@ -54,13 +54,13 @@ template <class R> __device__ __forceinline__ void stage_tables(const GeoView<R>
 // -------------------------------------------------------------------------------------------------------
 // navigation kernels: pure maps over queries
 // -------------------------------------------------------------------------------------------------------
-template <class R, bool HAS_DIR>
+template <class R, bool HAS_DIR, bool FLAT>
 __global__ void __launch_bounds__(NAV_THREADS) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                              int64_t n, int32_t* __restrict__ vol_out) {
     __shared__ BlockTables<R> tab;
     stage_tables(g, tab);
     __syncthreads();
-    Navigator<R, HAS_DIR> nav(g, &tab.ctx);
+    Navigator<R, HAS_DIR, FLAT> nav(g, &tab.ctx);
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{0, 0, 0};
@@ -70,14 +70,14 @@ __global__ void __launch_bounds__(NAV_THREADS) locate_kernel(GeoView<R> g, const
     }
 }
 
-template <class R>
+template <class R, bool FLAT>
 __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                            const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
                                                            int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out) {
     __shared__ BlockTables<R> tab;
     stage_tables(g, tab);
     __syncthreads();
-    Navigator<R, true> nav(g, &tab.ctx);
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
@@ -221,11 +221,11 @@ __device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, cons
 // PHYS = false: the lean wavefront pass -- photons that reach an interaction point park there and are written to the
 // back of the output queue; interact_pass handles them before the next pass.  PHYS = true: interactions happen inside
 // the pass (batched per warp); used for the last pass, which runs the few remaining photons to completion.
-template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS>
+template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
 __global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS && !FROM_SOURCE) ? TR_MIN_BLOCKS : 1)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
-               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K) {
+               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct) {
     // input: pass 0 generates n_src photons; later passes read the survivors of the previous pass, whose count is
     // known only on the device (front + back of cin)
     unsigned n_front = n_src, n_in = n_src;
@@ -247,7 +247,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
-    Navigator<R, true> nav(g, &tab.ctx);
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
     const unsigned i = blockIdx.x * TR_THREADS + threadIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
@@ -297,6 +297,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             if (fate != FATE_ALIVE) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = misc >> 8; if (pp.efinal) pp.efinal[idx] = (double)E; }
         }
     };
+    int act0 = 32;
 #pragma unroll 1
     for (int k = 0;;) {
         const unsigned pen = PHYS ? __ballot_sync(0xffffffffu, pending) : 0u;
@@ -332,6 +333,12 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             continue;
         }
         if (act == 0 || !budget) break;
+        // regroup early: once fewer than regroup_pct % of the lanes that entered the pass still travel, the warp stops
+        // and lets the compaction refill it (only the lean passes; the tail pass has nobody to regroup with)
+        if (!PHYS) {
+            if (k == 0) act0 = __popc(act);
+            else if (__popc(act) * 100 < act0 * regroup_pct) break;
+        }
         ++k;
         if (fate == FATE_ALIVE && !pending) {
             const MatRec<R> m = mats[nd.mat];
@@ -485,15 +492,23 @@ template <> const GeoView<double>& view<double>(const gn_geometry* g) { return g
 
 template <class R> int locate_impl(const gn_geometry* geo, const void* pos, const void* dir, int64_t n, int32_t* out, cudaStream_t s) {
     if (n == 0) return GN_OK;
-    if (dir) locate_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
-    else locate_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
+    // geometries whose lanes do different things per node visit (tubes, rotations, long candidate lists) use the flat
+    // one-visit-per-iteration search, coherent ones (voxel phantoms) the nested climb / descend loops
+    if (geo->coherent) {
+        if (dir) locate_kernel<R, true, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
+        else locate_kernel<R, false, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
+    } else {
+        if (dir) locate_kernel<R, true, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
+        else locate_kernel<R, false, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
+    }
     GN_CUDA(cudaGetLastError(), "gn_nav_locate launch");
     return GN_OK;
 }
 template <class R> int step_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
                                  int64_t n, void* step, int32_t* next, cudaStream_t s) {
     if (n == 0) return GN_OK;
-    step_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next);
+    if (geo->coherent) step_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next);
+    else step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next);
     GN_CUDA(cudaGetLastError(), "gn_nav_compute_step launch");
     return GN_OK;
 }
@@ -529,12 +544,12 @@ constexpr int TR_LAG = 2;                   // the host looks at survivor counts
 constexpr int K_UNLIMITED = 0x7fffffff;
 constexpr int TR_TIMED = 24;                // lean step passes per batch timed one by one (CUDA events around the launch)
 
-template <class R, bool SRC, bool PHYS>
+template <class R, bool SRC, bool PHYS, bool FLAT>
 static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
                         uint32_t n_src, const PassCounters* cin, PassCounters* cout, const PhotonRec<R>* qin, PhotonRec<R>* qout, uint32_t cap,
-                        double* edep, DevStats* stats, PerPhotonOut pp, int K) {
-    if (track) transport_pass<R, SRC, true, PHYS><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
-    else transport_pass<R, SRC, false, PHYS><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K);
+                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct) {
+    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct);
+    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct);
 }
 template <class R>
 static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, uint64_t seed, uint64_t first_id, const PassCounters* cin,
@@ -586,6 +601,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     cudaEvent_t* tev = &geo->ws_events[8];
     cudaError_t e = cudaSuccess;
     const unsigned tail = (unsigned)geo->opts.tail_photons;
+    const int regroup = geo->opts.regroup_percent;
     cudaMemsetAsync(d_stats, 0, 512, s);
     const GeoView<R>& g = view<R>(geo);
     for (int64_t done = 0; done < n_photons && rc == GN_OK; done += (int64_t)cap) {
@@ -609,13 +625,14 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             }
             const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
             const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
-            if (p == 0) launch_pass<R, true, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0);
-            else if (last) launch_pass<R, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED);
+            if (p == 0) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
+            else if (last) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
             else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
                 launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp);
                 if (n_timed < TR_TIMED) cudaEventRecord(tev[2 * n_timed], s);
-                launch_pass<R, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K);
+                if (geo->coherent) launch_pass<R, false, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup);
+                else launch_pass<R, false, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup);
                 if (n_timed < TR_TIMED) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
                 ++launches;
             }
