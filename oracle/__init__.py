@@ -127,6 +127,16 @@ class OracleGeometry:
             out.update(hash=h, nsteps=ns, efinal=ef)
         return out
 
+    def free_path(self, pos, dirs, Y, mu_mass, precision=64, use_grid=True):
+        """The paper's benchmark (Algorithm 2 phase 5): T_i from (x0, w, Y)_i, attenuation only.  -> (T, nsteps)."""
+        R = _real(precision)
+        pos = np.ascontiguousarray(pos, R); dirs = np.ascontiguousarray(dirs, R); Y = np.ascontiguousarray(Y, R)
+        n = pos.shape[0]
+        T = np.empty(n, R); ns = np.empty(n, np.uint32)
+        _check(lib().oracle_free_path_run(self._h, C.c_int(precision), _p(pos), _p(dirs), _p(Y), C.c_int64(n), C.c_double(mu_mass), _p(T), _p(ns),
+                                          C.c_int(int(use_grid))), "free_path_run")
+        return T, ns
+
     def mu(self, material, E, precision=64):
         m = np.empty(3, np.float64)
         _check(lib().oracle_mu(self._h, C.c_int(precision), C.c_int32(material), C.c_double(E), _p(m)), "mu")

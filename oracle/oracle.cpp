@@ -277,15 +277,46 @@ template <class R> R tube_dist_in(const SolidR<R>& s, const R p[3], const R v[3]
     return best;
 }
 
+/* ORB (radius a): s = |p| - r.  D:"orb solid" -- the sphere analogue of the S:C2 cylinder rules; the paper only
+ * names the solid ("aluminium balls").  Sums are (x.x + y.y) + z.z, left to right. */
+template <class R> int orb_inside(const SolidR<R>& s, const R p[3], R delta) {
+    R rp = r_sqrt((p[0] * p[0] + p[1] * p[1]) + p[2] * p[2]);
+    return classify(rp - s.a, delta);
+}
+template <class R> R orb_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R a = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
+    R b = (p[0] * v[0] + p[1] * v[1]) + p[2] * v[2];
+    R r2 = (p[0] * p[0] + p[1] * p[1]) + p[2] * p[2];
+    R rp = r_sqrt(r2);
+    if (b > 0 && rp - s.a >= -delta) return 0;                     /* on the surface band, moving outward */
+    R c = r2 - s.a * s.a;
+    R Dq = r_max(b * b - a * c, (R)0);
+    R t = (b > 0) ? -c / (b + r_sqrt(Dq)) : (-b + r_sqrt(Dq)) / a;   /* larger root, cancellation-free form */
+    return r_max(t, (R)0);
+}
+template <class R> R orb_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R a = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
+    R b = (p[0] * v[0] + p[1] * v[1]) + p[2] * v[2];
+    R r2 = (p[0] * p[0] + p[1] * p[1]) + p[2] * p[2];
+    R rp = r_sqrt(r2);
+    if (!(rp >= s.a - delta) || !(b < 0)) return r_inf<R>();       /* inside, or not approaching */
+    R rs = s.a - delta;                                            /* the ray must cross the radius shrunk by delta */
+    R cs = r2 - rs * rs;
+    if (!(b * b - a * cs > 0)) return r_inf<R>();
+    R c = r2 - s.a * s.a;
+    R Dq = b * b - a * c;
+    return r_max(c / (-b + r_sqrt(Dq)), (R)0);                     /* smaller root */
+}
+
 /* the "fork" on solid type */
 template <class R> int solid_inside(const SolidR<R>& s, const R p[3], R delta) {
-    return s.type == ORACLE_BOX ? box_inside(s, p, delta) : tube_inside(s, p, delta);
+    return s.type == ORACLE_BOX ? box_inside(s, p, delta) : (s.type == ORACLE_TUBE ? tube_inside(s, p, delta) : orb_inside(s, p, delta));
 }
 template <class R> R solid_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
-    return s.type == ORACLE_BOX ? box_dist_in(s, p, v, delta) : tube_dist_in(s, p, v, delta);
+    return s.type == ORACLE_BOX ? box_dist_in(s, p, v, delta) : (s.type == ORACLE_TUBE ? tube_dist_in(s, p, v, delta) : orb_dist_in(s, p, v, delta));
 }
 template <class R> R solid_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
-    return s.type == ORACLE_BOX ? box_dist_out(s, p, v, delta) : tube_dist_out(s, p, v, delta);
+    return s.type == ORACLE_BOX ? box_dist_out(s, p, v, delta) : (s.type == ORACLE_TUBE ? tube_dist_out(s, p, v, delta) : orb_dist_out(s, p, v, delta));
 }
 
 /* ---- navigator (S:C3, S:C4) ------------------------------------------------------------ */
@@ -596,6 +627,51 @@ void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& s
     if (efinal_out) *efinal_out = (double)E;
 }
 
+/* ---- the paper's own benchmark: Algorithm 1 with attenuation only (Eq. 9) ----------
+ * Input per particle: x0, w, Y (the paper generates these on the host, Algorithm 2 steps 2-3).
+ * mu_j = rho(volume) * mu_mass [cm^2/g] / 10 in 1/mm, evaluated in fp64 per material and rounded once to Real.
+ * Walk the boundaries ("Compute the next intersection ... using Geant4") carrying the remaining optical
+ * depth Yrem = Y - S_{j-1}: the free path ends inside the current volume when Yrem / mu_j is not beyond the next
+ * boundary, T = t_{j-1} + (Y - S_{j-1}) / mu_j; leaving the world gives T = +inf ("S_j may be infinite").
+ * Tie s_int == boundary -> boundary, Yrem <- max(Yrem - step mu, 0), stuck guard: as S:C9 / D:readings.
+ * t accumulates in Real: t <- t + step. */
+template <class R>
+void free_path(const Geo& g, const Navigator<R>& nav, const std::vector<R>& mu_of_mat, const R x0[3], const R w[3], R Y,
+               R& T_out, uint32_t& nsteps_out) {
+    R x[3] = {x0[0], x0[1], x0[2]};
+    int vol = nav.locate(x, w);
+    R t = 0, Yrem = Y; uint32_t ns = 0; int zero_steps = 0;
+    T_out = r_inf<R>();
+    while (vol >= 0) {
+        R mu = mu_of_mat[g.material[vol]];
+        R s_int = mu > 0 ? Yrem / mu : r_inf<R>();
+        R step; int next;
+        nav.compute_step(vol, x, w, s_int, step, next);
+        ++ns;
+        if (step == r_inf<R>()) { T_out = t + s_int; break; }          /* S_j >= Y inside this volume */
+        for (int i = 0; i < 3; ++i) x[i] = r_fma(step, w[i], x[i]);
+        t = t + step;
+        Yrem = r_max(Yrem - step * mu, (R)0);
+        vol = next;
+        if (step <= nav.delta) ++zero_steps; else zero_steps = 0;
+        if (vol >= 0 && zero_steps >= g.stuck_limit) break;           /* stuck: T stays +inf */
+    }
+    nsteps_out = ns;
+}
+template <class R> int run_free_path(const Geo& g, const void* pos, const void* dir, const void* Y, int64_t n, double mu_mass,
+                                     void* T_out, uint32_t* nsteps_out, bool grid) {
+    Navigator<R> nav(g, grid);
+    std::vector<R> mu(g.mats.size());
+    for (size_t m = 0; m < g.mats.size(); ++m) mu[m] = (R)(g.mats[m].rho * mu_mass / 10.0);
+    const R* P = (const R*)pos; const R* D = (const R*)dir; const R* Yv = (const R*)Y; R* T = (R*)T_out;
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t ns;
+        free_path(g, nav, mu, P + 3 * i, D + 3 * i, Yv[i], T[i], ns);
+        if (nsteps_out) nsteps_out[i] = ns;
+    }
+    return ORACLE_OK;
+}
+
 /* ---- geometry construction -------------------------------------------------------------- */
 void mat3_mul(const double* A, const double* B, double* C) {
     for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j)
@@ -605,6 +681,7 @@ void mat3_mul(const double* A, const double* B, double* C) {
 /* tight AABB of a solid in its own frame */
 void solid_aabb(const SolidD& s, double lo[3], double hi[3]) {
     if (s.type == ORACLE_BOX) { lo[0] = -s.a; hi[0] = s.a; lo[1] = -s.b; hi[1] = s.b; lo[2] = -s.c; hi[2] = s.c; return; }
+    if (s.type == ORACLE_ORB) { for (int k = 0; k < 3; ++k) { lo[k] = -s.a; hi[k] = s.a; } return; }
     lo[2] = -s.c; hi[2] = s.c;
     if (!s.sector) { lo[0] = lo[1] = -s.b; hi[0] = hi[1] = s.b; return; }
     double xs[16], ys[16]; int n = 0;
@@ -624,6 +701,7 @@ void build_grid(Geo& g, int mother) {
     double mlo[3], mhi[3];
     const SolidD& ms = g.solids[g.solid[mother]];
     if (ms.type == ORACLE_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; mlo[2] = -ms.c; mhi[2] = ms.c; }
+    else if (ms.type == ORACLE_ORB) { for (int k = 0; k < 3; ++k) { mlo[k] = -ms.a; mhi[k] = ms.a; } }
     else { mlo[0] = mlo[1] = -ms.b; mhi[0] = mhi[1] = ms.b; mlo[2] = -ms.c; mhi[2] = ms.c; }
     int nper = (int)std::ceil(std::cbrt((double)ds.size()));
     nper = std::max(1, std::min(nper, 64));
@@ -722,6 +800,11 @@ int make_solid(int type, const double* p, SolidD& s) {
         if (!(s.a > 0 && s.b > 0 && s.c > 0)) return ORACLE_INVALID_ARGUMENT;
         return ORACLE_OK;
     }
+    if (type == ORACLE_ORB) {
+        s.a = p[0]; s.b = s.c = 0;
+        if (!(s.a > 0)) return ORACLE_INVALID_ARGUMENT;
+        return ORACLE_OK;
+    }
     if (type != ORACLE_TUBE) return ORACLE_UNSUPPORTED_SOLID;
     s.a = p[0]; s.b = p[1]; s.c = p[2]; s.sphi = p[3]; s.dphi = p[4];
     if (!(s.a >= 0 && s.b > s.a && s.c > 0)) return ORACLE_INVALID_ARGUMENT;
@@ -784,7 +867,7 @@ int oracle_geometry_create(const double* materials, int32_t n_mats, const int32_
         for (int a = 0; a < 3; ++a) { g->x64[i].T[a] = T[a]; g->x32[i].T[a] = (float)T[a]; }
     }
     const SolidD& ws = g->solids[g->solid[0]];
-    double ext = ws.type == ORACLE_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : std::max(ws.b, ws.c);
+    double ext = ws.type == ORACLE_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == ORACLE_ORB ? ws.a : std::max(ws.b, ws.c));
     g->tol64 = (opts && opts->tol64 > 0) ? opts->tol64 : 1e-9;
     g->tol32 = (opts && opts->tol32 > 0) ? opts->tol32 : (double)(float)(ext * 0x1p-18);
     g->sigma_pe0 = (opts && opts->sigma_pe0 > 0) ? opts->sigma_pe0 : 1750.0;
@@ -855,6 +938,15 @@ int oracle_transport_run(const void* geo, int precision, const oracle_source_t* 
     const Geo& g = *(const Geo*)geo;
     if (precision == 64) return run_transport<double>(g, src, seed, first_id, n_photons, edep_out, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
     if (precision == 32) return run_transport<float>(g, src, seed, first_id, n_photons, edep_out, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+int oracle_free_path_run(const void* geo, int precision, const void* pos, const void* dir, const void* Y, int64_t n,
+                         double mu_mass_cm2_g, void* T_out, uint32_t* nsteps_out, int use_grid) {
+    if (!geo || n < 0 || !(mu_mass_cm2_g >= 0) || (n > 0 && (!pos || !dir || !Y || !T_out))) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    if (precision == 64) return run_free_path<double>(g, pos, dir, Y, n, mu_mass_cm2_g, T_out, nsteps_out, use_grid != 0);
+    if (precision == 32) return run_free_path<float>(g, pos, dir, Y, n, mu_mass_cm2_g, T_out, nsteps_out, use_grid != 0);
     return ORACLE_INVALID_ARGUMENT;
 }
 

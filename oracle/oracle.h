@@ -23,7 +23,7 @@ extern "C" {
 #endif
 
 enum { ORACLE_OK = 0, ORACLE_INVALID_ARGUMENT = -1, ORACLE_UNSUPPORTED_SOLID = -2, ORACLE_BAD_TREE = -3 };
-enum { ORACLE_BOX = 0, ORACLE_TUBE = 1 };
+enum { ORACLE_BOX = 0, ORACLE_TUBE = 1, ORACLE_ORB = 2 };
 enum { ORACLE_SRC_PENCIL = 0, ORACLE_SRC_GAUSS_PENCIL = 1, ORACLE_SRC_CONE = 2, ORACLE_SRC_ISOTROPIC = 3 };
 enum { ORACLE_E_MONO = 0, ORACLE_E_LOGUNIFORM = 1 };
 
@@ -53,7 +53,7 @@ typedef struct {
 
 /* geometry ------------------------------------------------------------------------------ */
 /* materials: n_mats x 3 doubles (Z, A, rho).  solid_type: n_solids int32; solid_params: n_solids x 5
- * doubles (BOX: hx,hy,hz,-,-; TUBE: rmin,rmax,hz,sphi,dphi).  placements: n_places x 4 int32
+ * doubles (BOX: hx,hy,hz,-,-; TUBE: rmin,rmax,hz,sphi,dphi; ORB: r,-,-,-,-).  placements: n_places x 4 int32
  * (parent, solid, material, transform); node 0 is the world (parent -1), parent < child.
  * transforms: n_transforms x 12 doubles, R row-major (local->parent) then T.                      */
 int oracle_geometry_create(const double* materials, int32_t n_mats,
@@ -79,6 +79,12 @@ int oracle_nav_compute_step(const void* geo, int precision, const void* pos, con
 int oracle_transport_run(const void* geo, int precision, const oracle_source_t* src, uint64_t seed,
                          int64_t first_id, int64_t n_photons, double* edep_out, oracle_stats_t* stats_out,
                          uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out, int use_grid);
+
+/* The paper's own benchmark (Algorithm 2 phase 5): free path T_i of particle i from (x0, w, Y)_i by
+ * Algorithm 1 with attenuation only, mu = rho * mu_mass (Eq. 9; mu_mass in cm^2/g, 0.06146 for Al at
+ * 1 MeV).  pos/dir: n x 3 Real, Y: n Real, T_out: n Real (+inf: left the world), nsteps_out: n or NULL. */
+int oracle_free_path_run(const void* geo, int precision, const void* pos, const void* dir, const void* Y, int64_t n,
+                         double mu_mass_cm2_g, void* T_out, uint32_t* nsteps_out, int use_grid);
 
 /* unit entry points used by the pins ------------------------------------------------------- */
 /* one solid, many points.  what: 0 = Inside (out: int32 0 in / 1 surface / 2 out written as Real),

@@ -5,8 +5,8 @@ of the method's arithmetic: no navigation, no physics, no RNG of the method -- o
 inputs as plain numpy arrays in the layout both C interfaces take:
 
     materials    (n_mats, 3)  float64   Z, A, rho [g/cm3]
-    solid_type   (n_solids,)  int32     0 = BOX, 1 = TUBE
-    solid_params (n_solids,5) float64   BOX: hx,hy,hz,0,0 [mm]; TUBE: rmin,rmax,hz [mm], sphi,dphi [rad]
+    solid_type   (n_solids,)  int32     0 = BOX, 1 = TUBE, 2 = ORB
+    solid_params (n_solids,5) float64   BOX: hx,hy,hz,0,0 [mm]; TUBE: rmin,rmax,hz [mm], sphi,dphi [rad]; ORB: r,0,0,0,0
     placements   (n_places,4) int32     parent (-1 for node 0 = world; parent < child), solid, material, transform
     transforms   (n_tr, 12)   float64   R row-major (local->parent) then T [mm]
 
@@ -22,7 +22,7 @@ from typing import Optional
 
 import numpy as np
 
-BOX, TUBE = 0, 1
+BOX, TUBE, ORB = 0, 1, 2
 SRC_PENCIL, SRC_GAUSS_PENCIL, SRC_CONE, SRC_ISOTROPIC = 0, 1, 2, 3
 E_MONO, E_LOGUNIFORM = 0, 1
 
@@ -96,6 +96,9 @@ class _Builder:
 
     def tube(self, rmin, rmax, hz, sphi=0.0, dphi=2 * math.pi):
         self.stype.append(TUBE); self.sparams.append((rmin, rmax, hz, sphi, dphi)); return len(self.stype) - 1
+
+    def orb(self, r):
+        self.stype.append(ORB); self.sparams.append((r, 0.0, 0.0, 0.0, 0.0)); return len(self.stype) - 1
 
     def place(self, parent, solid, material, R=None, T=(0.0, 0.0, 0.0)):
         R = np.eye(3) if R is None else np.asarray(R, dtype=np.float64)
@@ -276,6 +279,50 @@ def lattice_geometry(n=4, seed=7, pitch=100.0, fill="aluminium") -> Geometry:
 
 
 # ----------------------------------------------------------------------------------------------
+# ---- the paper's own benchmark inputs (section 3.5) ----------------------------
+MU_MASS_AL_1MEV = 0.06146       # cm^2/g
+
+
+def spheres_geometry(n_side=20, cube=5000.0, radius=100.0) -> Geometry:
+    """"Spheres": n_side^3 aluminium balls on a regular grid in a vacuum cube (8000 balls, 5 m cube).
+    The paper does not print the radius; 100 mm (pitch 250 mm) is this repo's choice."""
+    b = _Builder(f"spheres{n_side}")
+    world = b.place(-1, b.box(cube / 2, cube / 2, cube / 2), "vacuum")
+    ball = b.orb(radius)
+    pitch = cube / n_side
+    for iz in range(n_side):
+        for iy in range(n_side):
+            for ix in range(n_side):
+                b.place(world, ball, "aluminium", T=(-cube / 2 + pitch * (ix + 0.5), -cube / 2 + pitch * (iy + 0.5), -cube / 2 + pitch * (iz + 0.5)))
+    return b.finish()
+
+
+def random_particles(n=100000, seed=11, dtype=np.float64, origin=(0.0, 0.0, 0.0)):
+    """"Random" set: directions uniform on the unit sphere, lifetimes Y ~ Exp(1); all particles start
+    from the centre of the geometry (L160).  Generated on the host as in Algorithm 2 steps 2-3 (numpy PCG64 here, the
+    paper used Boost's Mersenne Twister)."""
+    rng = np.random.default_rng(seed)
+    d = rng.normal(size=(n, 3)); d /= np.linalg.norm(d, axis=1, keepdims=True)
+    Y = rng.exponential(1.0, size=n)
+    pos = np.tile(np.asarray(origin, dtype=np.float64), (n, 1))
+    d = d.astype(dtype); d64 = d.astype(np.float64)
+    d = (d64 / np.linalg.norm(d64, axis=1, keepdims=True)).astype(dtype)
+    return pos.astype(dtype), d, Y.astype(dtype)
+
+
+def regular_particles(nx=400, ny=250, dtype=np.float64, origin=(0.0, 0.0, 0.0), screen_z=1000.0, pixel=4.0):
+    """"Regular" set: the particles travel towards a regular nx x ny grid, input in column-major order,
+    all with lifetime Y = 1 -- the output is a volume-raytraced bitmap.  The screen is this repo's choice: pixel centres
+    of an nx x ny raster with `pixel` mm pitch on the plane z = screen_z, centred on the axis."""
+    ix, iy = np.meshgrid(np.arange(nx), np.arange(ny), indexing="ij")        # column-major: iy fastest
+    px = (ix.reshape(-1) - (nx - 1) / 2.0) * pixel; py = (iy.reshape(-1) - (ny - 1) / 2.0) * pixel
+    d = np.stack([px, py, np.full(px.shape, screen_z)], axis=1)
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    n = nx * ny
+    pos = np.tile(np.asarray(origin, dtype=np.float64), (n, 1))
+    return pos.astype(dtype), d.astype(dtype), np.ones(n, dtype=dtype)
+
+
 def world_half_extent(geom: Geometry) -> np.ndarray:
     s = int(geom.placements[0, 1])
     p = geom.solid_params[s]
