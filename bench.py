@@ -151,6 +151,123 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ the paper's own benchmark
+PAPER_TABLE1 = {  # PAPER.md Table 1 (L176-181): execution time [ms] of phase 5 for N = 1e5 particles
+    "random": {"cpu_1_thread_ms": 458.0, "cpu_12_threads_ms": 56.0, "gpu_gtx470_ms": 114.0},
+    "regular": {"cpu_1_thread_ms": 442.0, "cpu_12_threads_ms": 54.0, "gpu_gtx470_ms": 33.0},
+}
+
+
+def freepath_inputs(which, precision, scale):
+    from paper_1209_5235_b200 import workloads as W
+    R = np.float32 if precision == 32 else np.float64
+    if which == "random":
+        pos, d, Y = W.random_particles(int(100000 * scale), seed=11, dtype=R)
+    else:
+        pos, d, Y = W.regular_particles(400, max(1, int(250 * scale)), dtype=R)
+    return W.spheres_geometry(), pos, d, Y, W.MU_MASS_AL_1MEV
+
+
+def run_freepath(args):
+    """Configs 6 / 7: Algorithm 2 phase 5 on the Spheres geometry, N = 1e5 (x --scale).  A step = one
+    gn_free_path_run over the whole particle set.  Context beside PAPER.md Table 1, not a BASELINE.json config."""
+    which = "random" if args.config == 6 else "regular"
+    precision = args.precision or 64                          # the paper's port is double-based (PAPER.md L193)
+    geom, pos, d, Y, mu_mass = freepath_inputs(which, precision, args.scale)
+    n = pos.shape[0]
+    unit = "free paths/s"
+    name = f"spheres_{which}"
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return 0
+        import oracle
+        og = oracle.OracleGeometry(geom)
+        m = min(n, 20000)
+        og.free_path(pos[:200], d[:200], Y[:200], mu_mass, precision)
+        t = []
+        for s_ in range(args.steps):
+            lo = (s_ * m) % max(1, n - m + 1)
+            t0 = time.perf_counter(); og.free_path(pos[lo:lo + m], d[lo:lo + m], Y[lo:lo + m], mu_mass, precision); t.append(time.perf_counter() - t0)
+        v = m * args.steps / sum(t)
+        print(json.dumps({"impl": "reference", "metric": "free paths/s (Algorithm 2 phase 5)", "value": v, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": 1e3 * sum(t) / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                          "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": {"workload": name, "precision": precision, "sample_per_step": m},
+                          "cpu_baseline": {"value": v, "unit": unit, "cores": 1, "kind": "oracle", "sample": f"{m} of {n} particles per step, single thread"},
+                          "e2e": {"value": v, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return 0
+    import torch
+    from paper_1209_5235_b200 import binding as B, build as lib_build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        lib_build.build()
+    if world > 1:
+        dist.barrier()
+    dev = torch.device("cuda", local)
+    geo = B.Geometry(geom)
+    tp, td, tY = (torch.from_numpy(a).to(dev) for a in (pos, d, Y))
+    T = torch.empty(n, dtype=tp.dtype, device=dev)
+    for _ in range(max(args.warmup, 3)):
+        B.free_path_run(geo, tp, td, tY, mu_mass, out=T, nsteps=False)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2: written between timed runs
+    for s_ in range(args.steps):
+        flush.fill_(s_ & 255)
+        ev[2 * s_].record()
+        B.free_path_run(geo, tp, td, tY, mu_mass, out=T, nsteps=False)
+        ev[2 * s_ + 1].record()
+    torch.cuda.synchronize()
+    ms = sum(ev[2 * s_].elapsed_time(ev[2 * s_ + 1]) for s_ in range(args.steps))
+    tt = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX); ms = tt.item()
+    clocks = sampler.stop() if rank == 0 else None
+    # end to end = Algorithm 2 phases 4-6: host buffers in, T back on the host
+    hp, hd, hY = (torch.from_numpy(a).pin_memory().numpy() for a in (pos, d, Y))
+    B.free_path_run_host(geo, hp, hd, hY, mu_mass, precision)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        B.free_path_run_host(geo, hp, hd, hY, mu_mass, precision)
+    e2e_dt = time.perf_counter() - t0
+    if rank == 0:
+        rs = 4 if precision == 32 else 8
+        abytes = 8 * rs                                       # 3 + 3 + 1 Real in, 1 Real out per particle
+        peak, peak_src = measured_peaks()
+        achieved = n * abytes / (ms / args.steps * 1e-3) / 1e9
+        cpu = None
+        if not args.no_cpu_baseline:
+            import oracle
+            og = oracle.OracleGeometry(geom); m = min(n, 60000)
+            t0 = time.perf_counter(); og.free_path(pos[:m], d[:m], Y[:m], mu_mass, precision); dt = time.perf_counter() - t0
+            cpu = {"value": m / dt, "unit": unit, "cores": 1, "kind": "oracle", "sample": f"first {m} of {n} particles of {name}, fp{precision}, {dt:.1f} s"}
+        line = {"metric": "free paths/s (Algorithm 2 phase 5)", "value": world * n * args.steps / (ms * 1e-3), "unit": unit, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32" if precision == 32 else "f64", "data": "synthetic",
+                "config": {"workload": name, "precision": precision, "particles_per_gpu": n, "volumes": geo.n_places, "l2": "256 MB buffer written between timed runs (L2 flush)",
+                           "parallelism": f"dp{world} (replicas)"},
+                "clocks": clocks, "gpu_launches": args.steps,
+                "e2e": {"value": world * n * args.steps / e2e_dt, "unit": unit, "h2d_bytes_per_step": 7 * rs * n, "d2h_bytes_per_step": (rs + 4) * n,
+                        "note": "Algorithm 2 phases 4-6: particle states and lifetimes from pinned host memory, T (and step counts) back to the host"},
+                "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                             "kernel": "free_path_kernel", "algorithmic_bytes_per_unit": abytes,
+                             "note": "one thread walks one particle to completion (latency-bound at N = 1e5: 0.4 resident warps per scheduler)"},
+                "cpu_baseline": cpu,
+                "paper_table1": dict(PAPER_TABLE1[which], note="PAPER.md Table 1, N = 1e5, GTX 470 / 2 x Opteron 2427; context, other hardware, ball radius not printed in the paper")}
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier(); dist.destroy_process_group()
+    return 0
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
@@ -324,7 +441,8 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6, 7],
+                    help="1-5: BASELINE.json configs; 6 / 7: the paper's own benchmark, Spheres geometry with the Random / Regular set")
     ap.add_argument("--precision", type=int, default=0, choices=[0, 32, 64])
     ap.add_argument("--scale", type=float, default=1.0, help="fraction of the workload's photons/queries (diagnostics only)")
     ap.add_argument("--steps-per-pass", type=int, default=0)
@@ -334,6 +452,8 @@ def main():
     ap.add_argument("--cpu-all-cores", action="store_true")
     ap.add_argument("--allow-short-warmup", action="store_true")
     args = ap.parse_args()
+    if args.config in (6, 7):
+        return run_freepath(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -35,7 +35,7 @@ typedef enum {
     GN_CUDA_ERROR = -5
 } gn_status;
 
-enum { GN_BOX = 0, GN_TUBE = 1 };
+enum { GN_BOX = 0, GN_TUBE = 1, GN_ORB = 2 };
 enum { GN_SRC_PENCIL = 0, GN_SRC_GAUSS_PENCIL = 1, GN_SRC_CONE = 2, GN_SRC_ISOTROPIC = 3 };
 enum { GN_E_MONO = 0, GN_E_LOGUNIFORM = 1 };
 
@@ -83,7 +83,7 @@ typedef struct {
 /*
  * gn_geometry_create -- PAPER.md L139 / L127 (volumes hierarchy, solids, per-material density).
  *   h_materials    n_mats x 3 doubles: Z, A [g/mol], rho [g/cm3]
- *   h_solid_type   n_solids int32: GN_BOX | GN_TUBE
+ *   h_solid_type   n_solids int32: GN_BOX | GN_TUBE | GN_ORB (ORB: r,-,-,-,- )
  *   h_solid_params n_solids x 5 doubles: BOX hx,hy,hz,-,- ; TUBE rmin,rmax,hz,sphi,dphi  (C2; dphi >= 2 pi
  *                  = full tube, 0 < dphi <= pi = convex sector)
  *   h_placements   n_places x 4 int32: parent (-1 for node 0 = world, parent < child), solid, material,
@@ -147,9 +147,24 @@ int gn_transport_run(const gn_geometry* geo, int precision, const gn_source* h_s
                      double* d_edep_out, gn_run_stats* h_stats_out,
                      uint64_t* d_hash_out, uint32_t* d_nsteps_out, double* d_efinal_out, void* cuda_stream);
 
+/*
+ * gn_free_path_run -- the paper's own benchmark, Algorithm 2 phase 5: the free path T_i of particle i
+ * from (x0, w, Y)_i by Algorithm 1 (L55-76) with attenuation only, mu = rho(volume) * mu_mass (Eq. 9;
+ * mu_mass in cm^2/g: 0.06146 for aluminium at 1 MeV, L150).  One thread walks one particle from boundary to boundary
+ * carrying the remaining optical depth, as the paper's kernel did.
+ *   d_pos, d_dir  n x 3 Real; d_Y n Real (the "lifetimes", generated by the caller as in Algorithm 2 steps 2-3)
+ *   d_T_out       n Real: free path [mm]; +inf when the particle leaves the world first ("S_j may be infinite", L73)
+ *   d_nsteps_out  n uint32 ComputeStep calls per particle, or NULL
+ * Asynchronous on cuda_stream.
+ */
+int gn_free_path_run(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, const void* d_Y,
+                     int64_t n, double mu_mass_cm2_g, void* d_T_out, uint32_t* d_nsteps_out, void* cuda_stream);
+
 /* Host-buffer convenience wrappers (the "end to end" path: copies host<->device inside the call). */
 int gn_nav_query_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, int64_t n,
                       int32_t* h_vol_out, void* h_step_out, int32_t* h_next_vol_out);
+int gn_free_path_run_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, const void* h_Y, int64_t n,
+                          double mu_mass_cm2_g, void* h_T_out, uint32_t* h_nsteps_out /* or NULL */);   /* Algorithm 2 phases 4-6 */
 int gn_transport_run_host(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
                           int64_t first_photon_id, int64_t n_photons, double* h_edep_out, gn_run_stats* h_stats_out);
 

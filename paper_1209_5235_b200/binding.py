@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",
            "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_transport_run", "gn_nav_query_host",
-           "gn_transport_run_host", "gn_selftest_arith", "gn_last_error", "gn_version")
+           "gn_transport_run_host", "gn_free_path_run", "gn_free_path_run_host", "gn_selftest_arith", "gn_last_error", "gn_version")
 
 
 class GammaNavError(RuntimeError):
@@ -70,6 +70,8 @@ def lib():
                                        C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_nav_query_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_selftest_arith.argtypes = [C.c_int64, C.c_void_p]
+        L.gn_free_path_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p]
+        L.gn_free_path_run.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_transport_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
@@ -203,6 +205,32 @@ def transport_run(geo: Geometry, source, seed, n_photons, precision=32, first_ph
     if per_photon:
         out.update(hash=h, nsteps=ns, efinal=ef)
     return out
+
+
+def free_path_run(geo: Geometry, pos, dirs, Y, mu_mass, precision=None, out=None, nsteps=True):
+    """gn_free_path_run on device tensors -> (T (n,) Real, nsteps (n,) int32 bit pattern of uint32 or None)."""
+    torch = _torch()
+    precision = precision or (32 if pos.dtype == torch.float32 else 64)
+    dt = _real_dtype(torch, precision)
+    if pos.dtype != dt or dirs.dtype != dt or Y.dtype != dt or not (pos.is_cuda and dirs.is_cuda and Y.is_cuda):
+        raise GammaNavError("free_path_run: tensors must be CUDA and Real")
+    pos = pos.contiguous(); dirs = dirs.contiguous(); Y = Y.contiguous(); n = pos.shape[0]
+    T = out if out is not None else torch.empty(n, dtype=dt, device=pos.device)
+    ns = torch.empty(n, dtype=torch.int32, device=pos.device) if nsteps else None
+    _check(lib().gn_free_path_run(geo._h, precision, C.c_void_p(pos.data_ptr()), C.c_void_p(dirs.data_ptr()), C.c_void_p(Y.data_ptr()), C.c_int64(n),
+                                  C.c_double(float(mu_mass)), C.c_void_p(T.data_ptr()), C.c_void_p(ns.data_ptr()) if nsteps else None,
+                                  _stream_ptr(torch)), "gn_free_path_run")
+    return T, ns
+
+
+def free_path_run_host(geo: Geometry, pos: np.ndarray, dirs: np.ndarray, Y: np.ndarray, mu_mass, precision=64):
+    """gn_free_path_run_host: host numpy buffers in, T (and steps) out; the copies happen inside (Algorithm 2 phases 4-6)."""
+    R = np.float32 if precision == 32 else np.float64
+    pos = _np(pos, R); dirs = _np(dirs, R); Y = _np(Y, R); n = pos.shape[0]
+    T = np.empty(n, R); ns = np.empty(n, np.uint32)
+    _check(lib().gn_free_path_run_host(geo._h, precision, pos.ctypes.data_as(C.c_void_p), dirs.ctypes.data_as(C.c_void_p), Y.ctypes.data_as(C.c_void_p),
+                                       C.c_int64(n), C.c_double(float(mu_mass)), T.ctypes.data_as(C.c_void_p), ns.ctypes.data_as(C.c_void_p)), "gn_free_path_run_host")
+    return T, ns
 
 
 def nav_query_host(geo: Geometry, pos: np.ndarray, dirs: np.ndarray, precision=64):

@@ -66,7 +66,10 @@ void daughter_bounds(const HostSolid& s, const double* R, const double* T, doubl
     }
     double l[3], h[3];
     if (s.type == GN_BOX) { l[0] = -s.a; h[0] = s.a; l[1] = -s.b; h[1] = s.b; l[2] = -s.c; h[2] = s.c; }
-    else {
+    else if (s.type == GN_ORB) {          // rotation invariant
+        for (int k = 0; k < 3; ++k) { lo[k] = T[k] - s.a; hi[k] = T[k] + s.a; }
+        return;
+    } else {
         l[2] = -s.c; h[2] = s.c;
         if (s.sector) sector_bounds(s.a, s.b, s.sphi, s.sphi + s.dphi, l, h);
         else { l[0] = l[1] = -s.b; h[0] = h[1] = s.b; }
@@ -84,7 +87,7 @@ void daughter_bounds(const HostSolid& s, const double* R, const double* T, doubl
 template <class R> SolidRec<R> make_solid_rec(const HostSolid& s) {
     SolidRec<R> o;
     o.a = (R)s.a; o.b = (R)s.b; o.c = (R)s.c; o.cS = (R)s.cS; o.sS = (R)s.sS; o.cE = (R)s.cE; o.sE = (R)s.sE;
-    o.type = s.type == GN_BOX ? SOLID_BOX : SOLID_TUBE;
+    o.type = s.type == GN_BOX ? SOLID_BOX : (s.type == GN_ORB ? SOLID_ORB : SOLID_TUBE);
     o.flags = 0;
     if (s.type == GN_TUBE) { if (s.sector) o.flags |= TUBE_SECTOR; if (o.a > 0) o.flags |= TUBE_HOLE; }
     return o;
@@ -132,6 +135,9 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         s.a = p[0]; s.b = p[1]; s.c = p[2];
         if (s.type == GN_BOX) {
             if (!(s.a > 0 && s.b > 0 && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: box half-lengths must be positive");
+        } else if (s.type == GN_ORB) {
+            s.b = s.c = 0;
+            if (!(s.a > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: orb radius must be positive");
         } else if (s.type == GN_TUBE) {
             s.sphi = p[3]; s.dphi = p[4];
             if (!(s.a >= 0 && s.b > s.a && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: tube needs 0 <= rmin < rmax, hz > 0");
@@ -182,7 +188,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     cudaGetDevice(&geo->device);
     gn_opts o{}; if (h_opts) o = *h_opts;
     const HostSolid& ws = solids[node[0].y];
-    double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : std::max(ws.b, ws.c);
+    double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == GN_ORB ? ws.a : std::max(ws.b, ws.c));
     geo->tol64 = o.tol64 > 0 ? o.tol64 : 1e-9;
     geo->tol32 = o.tol32 > 0 ? o.tol32 : (double)(float)(ext * 0x1p-18);
     if (!(o.sigma_pe0 > 0)) o.sigma_pe0 = 1750.0;
@@ -205,9 +211,11 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         if (nd < o.voxel_min_daughters) continue;
         const HostSolid& ms = solids[node[mth].y];
         double mlo[3], mhi[3];
-        if (ms.type == GN_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; }
+        if (ms.type == GN_ORB) { mlo[0] = mlo[1] = -ms.a; mhi[0] = mhi[1] = ms.a; }
+        else if (ms.type == GN_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; }
         else { mlo[0] = mlo[1] = -ms.b; mhi[0] = mhi[1] = ms.b; }
         mlo[2] = -ms.c; mhi[2] = ms.c;
+        if (ms.type == GN_ORB) { mlo[2] = -ms.a; mhi[2] = ms.a; }
         std::vector<double> blo(3 * (size_t)nd), bhi(3 * (size_t)nd);
         double minext[3] = {1e300, 1e300, 1e300};
         for (int j = 0; j < nd; ++j) {
@@ -361,6 +369,11 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     a.mats = up.put(m32); b.mats = up.put(m64);
     a.grids = up.put(g32); b.grids = up.put(g64);
     a.n_grids = b.n_grids = (int)grids.size();
+    {
+        std::vector<double> rho(n_mats);
+        for (int i = 0; i < n_mats; ++i) rho[i] = h_materials[3 * i + 2];
+        a.rho = b.rho = up.put(rho);
+    }
     a.tol = (float)geo->tol32; a.delta = a.tol / 2; a.probe = std::max(a.tol, (float)(ext * 0x1p-18)); a.e_cut = (float)o.e_cut;
     b.tol = geo->tol64; b.delta = b.tol / 2; b.probe = b.tol; b.e_cut = o.e_cut;
     a.n_nodes = b.n_nodes = n_places; a.n_solids = b.n_solids = n_solids; a.n_mats = b.n_mats = n_mats;

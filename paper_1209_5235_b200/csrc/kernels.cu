@@ -94,6 +94,45 @@ __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R
 }
 
 // -------------------------------------------------------------------------------------------------------
+// the paper's own benchmark: Algorithm 1 with attenuation only, one thread per particle
+// -------------------------------------------------------------------------------------------------------
+template <class R, bool FLAT>
+__global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+                                                                const R* __restrict__ Yin, int64_t n, double mu_mass,
+                                                                R* __restrict__ T_out, uint32_t* __restrict__ nsteps_out) {
+    __shared__ BlockTables<R> tab;
+    __shared__ R sh_mu[MAX_SMEM_MATS];
+    stage_tables(g, tab);
+    // Eq. 9: mu = rho mu_mass, here in 1/mm; fp64, rounded once to Real
+    for (int i = threadIdx.x; i < g.n_mats && i < MAX_SMEM_MATS; i += blockDim.x) sh_mu[i] = (R)(g.rho[i] * mu_mass / 10.0);
+    __syncthreads();
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        const V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        NodeRec<R> nd;
+        int vol = nav.locate(x, w, nd);
+        R t = 0, Yrem = Yin[i], T = rinf<R>();
+        uint32_t ns = 0; int zero_steps = 0;
+        while (vol >= 0) {
+            const R mu = nd.mat < MAX_SMEM_MATS ? sh_mu[nd.mat] : (R)(g.rho[nd.mat] * mu_mass / 10.0);
+            const R s_int = mu > 0 ? rdiv(Yrem, mu) : rinf<R>();        // remaining part of Eq. 7
+            R step; V3<R> xn;
+            nav.compute_step(vol, nd, x, w, s_int, step, xn);             // "next intersection"
+            ++ns;
+            if (step == rinf<R>()) { T = t + s_int; break; }               // S_j >= Y inside this volume (L76)
+            x = xn;
+            t = t + step;
+            Yrem = rmax(Yrem - step * mu, (R)0);                           // S_j update (L71)
+            zero_steps = (step <= g.delta) ? zero_steps + 1 : 0;
+            if (vol >= 0 && zero_steps >= g.stuck_limit) break;
+        }
+        T_out[i] = T;
+        if (nsteps_out) nsteps_out[i] = ns;
+    }
+}
+
+// -------------------------------------------------------------------------------------------------------
 // transport
 // -------------------------------------------------------------------------------------------------------
 constexpr int TR_THREADS = 128;
@@ -698,6 +737,50 @@ extern "C" int gn_transport_run(const gn_geometry* geo, int precision, const gn_
     if (precision == 32) return transport_impl<float>(geo, h_src, seed, first_photon_id, n_photons, d_edep_out, h_stats_out, d_hash_out, d_nsteps_out, d_efinal_out, (cudaStream_t)cuda_stream);
     if (precision == 64) return transport_impl<double>(geo, h_src, seed, first_photon_id, n_photons, d_edep_out, h_stats_out, d_hash_out, d_nsteps_out, d_efinal_out, (cudaStream_t)cuda_stream);
     return fail(GN_INVALID_ARGUMENT, "gn_transport_run: precision must be 32 or 64");
+}
+
+template <class R> int free_path_impl(const gn_geometry* geo, const void* pos, const void* dir, const void* Y, int64_t n, double mu_mass,
+                                      void* T, uint32_t* ns, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    const int64_t blocks = (n + NAV_THREADS - 1) / NAV_THREADS;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(blocks, 148 * 64));
+    if (geo->coherent) free_path_kernel<R, false><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
+    else free_path_kernel<R, true><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
+    GN_CUDA(cudaGetLastError(), "gn_free_path_run launch");
+    return GN_OK;
+}
+
+extern "C" int gn_free_path_run(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, const void* d_Y, int64_t n,
+                                double mu_mass_cm2_g, void* d_T_out, uint32_t* d_nsteps_out, void* cuda_stream) {
+    if (!geo || n < 0 || !(mu_mass_cm2_g >= 0) || (n > 0 && (!d_pos || !d_dir || !d_Y || !d_T_out)))
+        return fail(GN_INVALID_ARGUMENT, "gn_free_path_run: bad argument");
+    if (precision == 32) return free_path_impl<float>(geo, d_pos, d_dir, d_Y, n, mu_mass_cm2_g, d_T_out, d_nsteps_out, (cudaStream_t)cuda_stream);
+    if (precision == 64) return free_path_impl<double>(geo, d_pos, d_dir, d_Y, n, mu_mass_cm2_g, d_T_out, d_nsteps_out, (cudaStream_t)cuda_stream);
+    return fail(GN_INVALID_ARGUMENT, "gn_free_path_run: precision must be 32 or 64");
+}
+
+extern "C" int gn_free_path_run_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, const void* h_Y, int64_t n,
+                                     double mu_mass_cm2_g, void* h_T_out, uint32_t* h_nsteps_out) {
+    if (!geo || n < 0 || (precision != 32 && precision != 64) || (n > 0 && (!h_pos || !h_dir || !h_Y || !h_T_out)))
+        return fail(GN_INVALID_ARGUMENT, "gn_free_path_run_host: bad argument");
+    if (n == 0) return GN_OK;
+    const size_t rs = precision == 32 ? 4 : 8;
+    const size_t b3 = 3 * rs * (size_t)n, b1 = rs * (size_t)n, bi = 4 * (size_t)n;
+    char* d = nullptr;
+    if (cudaMalloc((void**)&d, 2 * b3 + 2 * b1 + bi) != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, "gn_free_path_run_host: cudaMalloc"); }
+    char *dp = d, *dd = d + b3, *dY = d + 2 * b3, *dT = dY + b1, *dn = dT + b1;
+    // Algorithm 2 phases 4-6: transfer the particle states and lifetimes, compute, transfer T back
+    cudaError_t e = cudaMemcpy(dp, h_pos, b3, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dd, h_dir, b3, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dY, h_Y, b1, cudaMemcpyHostToDevice);
+    int rc = GN_OK;
+    if (e == cudaSuccess) rc = gn_free_path_run(geo, precision, dp, dd, dY, n, mu_mass_cm2_g, dT, h_nsteps_out ? (uint32_t*)dn : nullptr, nullptr);
+    if (rc == GN_OK && e == cudaSuccess) e = cudaMemcpy(h_T_out, dT, b1, cudaMemcpyDeviceToHost);
+    if (rc == GN_OK && e == cudaSuccess && h_nsteps_out) e = cudaMemcpy(h_nsteps_out, dn, bi, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (rc != GN_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "gn_free_path_run_host");
+    return GN_OK;
 }
 
 extern "C" int gn_nav_query_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, int64_t n,

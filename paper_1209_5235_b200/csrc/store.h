@@ -18,12 +18,12 @@
 
 namespace gn {
 
-enum : int { SOLID_BOX = 0, SOLID_TUBE = 1 };
+enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2 };
 enum : int { TUBE_SECTOR = 1, TUBE_HOLE = 2 };
 enum : int { NODE_IDENTITY = 1 << 30, NODE_SOLID_MASK = (1 << 30) - 1 };
 
 template <class R> struct SolidRec {
-    R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz
+    R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -
     R cS, sS, cE, sE;     // trig of sphi and sphi + dphi (host libm, fp64, rounded once)
     int type, flags;
 };
@@ -54,6 +54,7 @@ template <class R> struct GeoView {
     const int* dlist;
     const SolidRec<R>* solids;
     const MatRec<R>* mats;
+    const double* rho;    // density per material [g/cm3] (attenuation-only mode: mu = rho * mu_mass)
     const GridRec<R>* grids;
     const int2* cells;
     const int* cand;

@@ -366,3 +366,61 @@ def test_inline_division_and_sqrt_are_correctly_rounded(B):
     r = B.selftest_arith(1 << 31)
     assert r["sqrt_mismatches"] == 0, r
     assert r["div_mismatches"] == 0, r
+
+
+# ---- the paper's own benchmark (attenuation-only Algorithm 1, Spheres geometry) ------------
+def spheres_small():
+    return W.spheres_geometry(n_side=6, cube=1500.0, radius=100.0)
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_orb_navigation_bit_exact(B, precision):
+    """Orb solid: locate and ComputeStep (voxel walk of the vacuum world through 216 balls) equal the oracle's plain
+    linear scans bit for bit."""
+    geom = spheres_small()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    assert g.voxel_info()["grids"] == 1
+    rng = np.random.default_rng(31)
+    n = 60001
+    R = np.float64 if precision == 64 else np.float32
+    p = (rng.uniform(-1, 1, size=(n, 3)) * 760.0).astype(R); v = unit(rng, n).astype(R)
+    # a share of the points on / near ball surfaces
+    c = (rng.integers(0, 6, size=(n // 4, 3)) + 0.5) * 250.0 - 750.0
+    k = rng.choice([-2.0, -1.0, -0.5, 0.0, 0.5, 1.0, 2.0], size=n // 4)
+    p[: n // 4] = (c + unit(rng, n // 4) * (100.0 + k[:, None] * g.tolerance(precision) / 2)).astype(R)
+    tp, tv = cuda(p), cuda(v)
+    ref = og.locate(p, v, precision, use_grid=False)
+    assert np.array_equal(B.nav_locate(g, tp, tv).cpu().numpy(), ref)
+    assert np.array_equal(B.nav_locate(g, tp, None).cpu().numpy(), og.locate(p, None, precision, use_grid=False))
+    step, nxt = B.nav_compute_step(g, tp, tv, cuda(ref))
+    rstep, rnxt = og.compute_step(p, v, ref, None, precision, use_grid=False)
+    assert np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(step.cpu().numpy(), rstep)
+    assert (ref > 0).sum() > 1000 and (rnxt > 0).sum() > 1000 and (ref == -1).any()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("which", ["random", "regular"])
+def test_free_path_matches_oracle(B, which, precision):
+    """gn_free_path_run (Algorithm 2 phase 5) on the paper's Spheres geometry, N = 1e5 as in the paper for the Random set
+    (Regular: 400 x 250): T_i and the number of steps equal the oracle's bit for bit (same canonical arithmetic)."""
+    import torch
+    geom = W.spheres_geometry()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    R = np.float64 if precision == 64 else np.float32
+    pos, d, Y = (W.random_particles(100000, seed=11, dtype=R) if which == "random" else W.regular_particles(400, 250, dtype=R))
+    T, ns = B.free_path_run(g, cuda(pos), cuda(d), cuda(Y), W.MU_MASS_AL_1MEV)
+    T = T.cpu().numpy(); ns = ns.cpu().numpy().astype(np.uint32)
+    # the oracle's ComputeStep scans all 8000 balls per step: compare a seeded sample of 4000 particles
+    idx = np.random.default_rng(1).choice(len(Y), 4000, replace=False)
+    rT, rns = og.free_path(pos[idx], d[idx], Y[idx], W.MU_MASS_AL_1MEV, precision)
+    assert np.array_equal(T[idx], rT) and np.array_equal(ns[idx], rns)
+    assert np.isinf(T).any() and np.isfinite(T).sum() > len(Y) // 2
+    # whole-set property: every finite free path ends inside a ball (mu = 0 in the vacuum), checked in fp64
+    fin = np.isfinite(T)
+    end = pos[fin].astype(np.float64) + d[fin].astype(np.float64) * T[fin].astype(np.float64)[:, None]
+    rel = np.mod(end + 2500.0, 250.0) - 125.0
+    assert np.all(np.linalg.norm(rel, axis=1) <= 100.0 + (1e-6 if precision == 64 else 2e-2))
+    # empty input
+    e3 = torch.empty((0, 3), dtype=torch.float64 if precision == 64 else torch.float32, device="cuda")
+    Te, _ = B.free_path_run(g, e3, e3, e3[:, 0].contiguous(), W.MU_MASS_AL_1MEV)
+    assert Te.numel() == 0
