@@ -17,7 +17,9 @@
  * signed-distance field, brute-force locate with per-level transforms, chained steps vs. sorted
  * analytic crossings, Klein-Nishina quadrature and k->0 limit, Compton energy-momentum
  * conservation, chi^2 of sampled epsilon, slab transmission exp(-mu x), energy book-keeping,
- * Philox vs. cuRAND's host generator, uniform end points.
+ * Philox vs. cuRAND's host generator, uniform end points; orb closed forms / ray marching and the
+ * attenuation-only free paths (the paper's own benchmark) vs. a sorted-chord closed form in numpy
+ * (tests/test_oracle_freepath.py).
  * PARITY UNPINNED (defined only by SURVEY 8(c)/DESIGN.md, no independent truth exists):
  *   sigma_PE0 normalisation, the capped Bethe-Heitler form, A values, source frame convention,
  *   tolerances, tie-breaks, stuck guard, history hash.
