@@ -114,6 +114,16 @@ class OracleGeometry:
                                              C.c_int(int(use_grid))), "nav_compute_step")
         return step, nxt
 
+    def compute_step_normal(self, pos, dirs, vol, max_step=None, precision=64, use_grid=True):
+        R = _real(precision)
+        pos = np.ascontiguousarray(pos, R); dirs = np.ascontiguousarray(dirs, R); vol = np.ascontiguousarray(vol, np.int32)
+        ms = None if max_step is None else np.ascontiguousarray(max_step, R)
+        n = pos.shape[0]
+        step = np.empty(n, R); nxt = np.empty(n, np.int32); nrm = np.empty((n, 3), R)
+        _check(lib().oracle_nav_compute_step_normal(self._h, C.c_int(precision), _p(pos), _p(dirs), _p(vol), _p(ms), C.c_int64(n), _p(step), _p(nxt),
+                                                    _p(nrm), C.c_int(int(use_grid))), "nav_compute_step_normal")
+        return step, nxt, nrm
+
     def transport(self, src, seed, n, precision=64, first_id=0, per_photon=False, use_grid=True):
         edep = np.zeros(self.n_places, np.float64); st = Stats()
         h = np.empty(n, np.uint64) if per_photon else None
@@ -146,11 +156,11 @@ class OracleGeometry:
 def solid_eval(stype, params, tol, what, pos, dirs=None, precision=64):
     """what: 'inside' | 'dist_in' | 'dist_out' for one solid on many points."""
     R = _real(precision)
-    code = {"inside": 0, "dist_in": 1, "dist_out": 2}[what]
+    code = {"inside": 0, "dist_in": 1, "dist_out": 2, "normal": 3}[what]
     pos = np.ascontiguousarray(pos, R)
     dirs = np.ascontiguousarray(dirs if dirs is not None else np.zeros_like(pos), R)
     p5 = np.zeros(5, np.float64); p5[:len(params)] = params
-    out = np.empty(pos.shape[0], R)
+    out = np.empty((pos.shape[0], 3) if what == "normal" else pos.shape[0], R)
     _check(lib().oracle_solid_eval(C.c_int32(stype), _p(p5), C.c_double(tol), C.c_int(precision), C.c_int(code), _p(pos), _p(dirs),
                                    C.c_int64(pos.shape[0]), _p(out)), "solid_eval")
     return out.astype(np.int32) if what == "inside" else out

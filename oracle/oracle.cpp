@@ -310,6 +310,46 @@ template <class R> R orb_dist_in(const SolidR<R>& s, const R p[3], const R v[3],
     return r_max(c / (-b + r_sqrt(Dq)), (R)0);                     /* smaller root */
 }
 
+/* Outward unit normal of the bounding surface a point q (local frame) lies on -- "what is the normal of the boundary
+ * surface at that point?".  D:"surface normal": the surface is the one whose signed outsideness s_k(q) is the
+ * largest (the one q is on, or nearest to; ties -> first in the order listed), the normal is the gradient of that s_k:
+ *   BOX   s_i = |q_i| - h_i, i = x, y, z                       n = sign(q_i) e_i          (q_i = 0 counts as +)
+ *   TUBE  s_z = |z| - hz; s_out = r - rmax; s_in = rmin - r; s_S; s_E     n = sign(z) e_z; (x, y, 0)/r; -(x, y, 0)/r;
+ *                                                              (sS, -cS, 0); (-sE, cE, 0)
+ *   ORB   n = q / |q|
+ * (r = 0 on a cylinder or |q| = 0 on an orb cannot be on the surface; the x axis is returned.) */
+template <class R> void solid_normal(const SolidR<R>& s, const R q[3], R n[3]) {
+    n[0] = n[1] = n[2] = 0;
+    if (s.type == ORACLE_BOX) {
+        const R h[3] = {s.a, s.b, s.c};
+        int k = 0; R best = r_abs(q[0]) - h[0];
+        for (int i = 1; i < 3; ++i) { R si = r_abs(q[i]) - h[i]; if (si > best) { best = si; k = i; } }
+        n[k] = q[k] < 0 ? (R)-1 : (R)1;
+        return;
+    }
+    if (s.type == ORACLE_ORB) {
+        R rp = r_sqrt((q[0] * q[0] + q[1] * q[1]) + q[2] * q[2]);
+        if (!(rp > 0)) { n[0] = 1; return; }
+        n[0] = q[0] / rp; n[1] = q[1] / rp; n[2] = q[2] / rp;
+        return;
+    }
+    R r = r_sqrt(q[0] * q[0] + q[1] * q[1]);
+    int k = 0; R best = r_abs(q[2]) - s.c;
+    { R so = r - s.b; if (so > best) { best = so; k = 1; } }
+    if (s.a > 0) { R si = s.a - r; if (si > best) { best = si; k = 2; } }
+    if (s.sector) {
+        R sS = s.sS * q[0] - s.cS * q[1]; if (sS > best) { best = sS; k = 3; }
+        R sE = s.cE * q[1] - s.sE * q[0]; if (sE > best) { best = sE; k = 4; }
+    }
+    if (k == 0) n[2] = q[2] < 0 ? (R)-1 : (R)1;
+    else if (k == 1 || k == 2) {
+        if (!(r > 0)) { n[0] = 1; return; }
+        R sg = k == 1 ? (R)1 : (R)-1;
+        n[0] = sg * (q[0] / r); n[1] = sg * (q[1] / r);
+    } else if (k == 3) { n[0] = s.sS; n[1] = -s.cS; }
+    else { n[0] = -s.sE; n[1] = s.cE; }
+}
+
 /* the "fork" on solid type */
 template <class R> int solid_inside(const SolidR<R>& s, const R p[3], R delta) {
     return s.type == ORACLE_BOX ? box_inside(s, p, delta) : (s.type == ORACLE_TUBE ? tube_inside(s, p, delta) : orb_inside(s, p, delta));
@@ -399,6 +439,32 @@ template <class R> struct Navigator {
         if (best > max_step) { step = r_inf<R>(); next = vol; return; }
         step = best;
         R xn[3] = {r_fma(best, w[0], x[0]), r_fma(best, w[1], x[1]), r_fma(best, w[2], x[2])};
+        next = relocate(vol, xn, w);
+    }
+    /* ComputeStep that also answers "what is the normal of the boundary surface at that point?": the outward
+     * normal, in the global frame, of the solid whose surface ends the step -- the current volume's own solid (exit), or
+     * the daughter entered (strict <: ties favour the mother, then the lowest daughter index, S:C4).  No boundary within
+     * max_step -> normal (0,0,0).  Local -> global: n_g[k] = fma(M[2][k], n.z, fma(M[1][k], n.y, M[0][k] n.x)) (M = X.M). */
+    void compute_step_normal(int vol, const R x[3], const R w[3], R max_step, R& step, int& next, R ng[3]) const {
+        ng[0] = ng[1] = ng[2] = 0;
+        if (vol < 0) { step = r_inf<R>(); next = -1; return; }
+        R p[3], v[3];
+        local_point(vol, x, p); local_dir(vol, w, v);
+        R best = solid_dist_out(S[g.solid[vol]], p, v, delta);
+        int hit = vol;
+        for (int d : g.daughters[vol]) {
+            local_point(d, x, p); local_dir(d, w, v);
+            R t = solid_dist_in(S[g.solid[d]], p, v, delta);
+            if (t < best) { best = t; hit = d; }
+        }
+        if (best > max_step) { step = r_inf<R>(); next = vol; return; }
+        step = best;
+        R xn[3] = {r_fma(best, w[0], x[0]), r_fma(best, w[1], x[1]), r_fma(best, w[2], x[2])};
+        R q[3], nl[3];
+        local_point(hit, xn, q);
+        solid_normal(S[g.solid[hit]], q, nl);
+        const XformR<R>& t = X[hit];
+        for (int k = 0; k < 3; ++k) ng[k] = r_fma(t.M[6 + k], nl[2], r_fma(t.M[3 + k], nl[1], t.M[k] * nl[0]));
         next = relocate(vol, xn, w);
     }
 };
@@ -770,6 +836,18 @@ template <class R> int run_step(const Geo& g, const void* pos, const void* dir, 
     }
     return ORACLE_OK;
 }
+template <class R> int run_step_normal(const Geo& g, const void* pos, const void* dir, const int32_t* vol, const void* maxs,
+                                       int64_t n, void* step_out, int32_t* next_out, void* normal_out, bool grid) {
+    Navigator<R> nav(g, grid);
+    const R* P = (const R*)pos; const R* D = (const R*)dir; const R* Mx = (const R*)maxs; R* S = (R*)step_out; R* N = (R*)normal_out;
+    for (int64_t i = 0; i < n; ++i) {
+        R st; int nx;
+        if (vol[i] >= (int32_t)g.parent.size()) return ORACLE_INVALID_ARGUMENT;
+        nav.compute_step_normal(vol[i], P + 3 * i, D + 3 * i, Mx ? Mx[i] : r_inf<R>(), st, nx, N + 3 * i);
+        S[i] = st; next_out[i] = nx;
+    }
+    return ORACLE_OK;
+}
 template <class R> int run_transport(const Geo& g, const oracle_source_t* src, uint64_t seed, int64_t first, int64_t n,
                                      double* edep, oracle_stats_t* st, uint64_t* hash, uint32_t* ns, double* ef, bool grid) {
     SourceR<R> s;
@@ -790,6 +868,7 @@ template <class R> int run_solid_eval(const SolidD& sd, double tol, int what, co
     for (int64_t i = 0; i < n; ++i) {
         if (what == 0) O[i] = (R)solid_inside(s, P + 3 * i, delta);
         else if (what == 1) O[i] = solid_dist_in(s, P + 3 * i, D + 3 * i, delta);
+        else if (what == 3) solid_normal(s, P + 3 * i, O + 3 * i);            /* out: n x 3 */
         else O[i] = solid_dist_out(s, P + 3 * i, D + 3 * i, delta);
     }
     return ORACLE_OK;
@@ -930,6 +1009,15 @@ int oracle_nav_compute_step(const void* geo, int precision, const void* pos, con
     const Geo& g = *(const Geo*)geo;
     if (precision == 64) return run_step<double>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, use_grid != 0);
     if (precision == 32) return run_step<float>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, use_grid != 0);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+int oracle_nav_compute_step_normal(const void* geo, int precision, const void* pos, const void* dir, const int32_t* vol_in,
+                                   const void* max_step, int64_t n, void* step_out, int32_t* next_vol_out, void* normal_out, int use_grid) {
+    if (!geo || n < 0 || (n > 0 && (!pos || !dir || !vol_in || !step_out || !next_vol_out || !normal_out))) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    if (precision == 64) return run_step_normal<double>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, normal_out, use_grid != 0);
+    if (precision == 32) return run_step_normal<float>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, normal_out, use_grid != 0);
     return ORACLE_INVALID_ARGUMENT;
 }
 

@@ -74,6 +74,12 @@ int oracle_nav_compute_step(const void* geo, int precision, const void* pos, con
                             const int32_t* vol_in, const void* max_step /*or NULL*/, int64_t n,
                             void* step_out, int32_t* next_vol_out, int use_grid);
 
+/* ComputeStep with the surface normal ("what is the normal of the boundary surface at that point?"): as
+ * oracle_nav_compute_step, plus normal_out n x 3 Real: outward unit normal, global frame, of the solid whose surface ends
+ * the step (own solid on exit, the entered daughter otherwise); (0,0,0) when no boundary lies within max_step. */
+int oracle_nav_compute_step_normal(const void* geo, int precision, const void* pos, const void* dir, const int32_t* vol_in,
+                                   const void* max_step, int64_t n, void* step_out, int32_t* next_vol_out, void* normal_out, int use_grid);
+
 /* transport (C6-C9).  Photons first_id .. first_id+n-1; edep_out has n_places doubles and is
  * ACCUMULATED INTO (caller zeroes); per-photon outputs may be NULL.                                */
 int oracle_transport_run(const void* geo, int precision, const oracle_source_t* src, uint64_t seed,
@@ -88,7 +94,7 @@ int oracle_free_path_run(const void* geo, int precision, const void* pos, const 
 
 /* unit entry points used by the pins ------------------------------------------------------- */
 /* one solid, many points.  what: 0 = Inside (out: int32 0 in / 1 surface / 2 out written as Real),
- * 1 = DistanceToIn, 2 = DistanceToOut.  pos/dir: n x 3 Real, out: n Real.                          */
+ * 1 = DistanceToIn, 2 = DistanceToOut, 3 = surface normal at pos (out: n x 3 Real).  pos/dir: n x 3 Real, out: n Real.                          */
 int oracle_solid_eval(int32_t type, const double* params5, double tol, int precision, int what,
                       const void* pos, const void* dir, int64_t n, void* out);
 double oracle_sigma_kn(double k);                       /* Klein-Nishina total, cm^2 per electron */
