@@ -131,6 +131,17 @@ int gn_nav_compute_step(const gn_geometry* geo, int precision, const void* d_pos
                         void* d_step_out, int32_t* d_next_vol_out, void* cuda_stream);
 
 /*
+ * gn_nav_compute_step_normal -- PAPER.md L125 in full: "... If so, where, and what is the normal of the boundary surface at
+ * that point?"  As gn_nav_compute_step, plus d_normal_out n x 3 Real: the outward unit normal, in the global frame, of the
+ * solid whose surface ends the step -- the current volume's own solid (the step leaves it), or the daughter entered (ties:
+ * mother first, then the lowest daughter index).  The surface of that solid is the one with the largest signed outsideness
+ * at the crossing point.  (0,0,0) when no boundary lies within max_step.
+ */
+int gn_nav_compute_step_normal(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir,
+                               const int32_t* d_vol_in, const void* d_max_step, int64_t n,
+                               void* d_step_out, int32_t* d_next_vol_out, void* d_normal_out, void* cuda_stream);
+
+/*
  * gn_transport_run -- PAPER.md Algorithm 1 (L55-76) for photons first_photon_id .. first_photon_id + n - 1,
  * each with its own Philox4x32-10 stream keyed by (seed, photon id).
  *   d_edep_out    gn_geometry_num_places doubles [MeV]; ZEROED by the callee, then accumulated (fp64 atomics)

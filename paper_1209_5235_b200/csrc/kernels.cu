@@ -93,6 +93,30 @@ __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R
     }
 }
 
+// ComputeStep + surface normal of the boundary crossed
+template <class R, bool FLAT>
+__global__ void __launch_bounds__(NAV_THREADS) step_normal_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+                                                                  const int32_t* __restrict__ vol_in, const R* __restrict__ max_step, int64_t n,
+                                                                  R* __restrict__ step_out, int32_t* __restrict__ next_out, R* __restrict__ normal_out) {
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
+    __syncthreads();
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        int vol = vol_in[i];
+        R step = rinf<R>(); int next = -1; V3<R> ng{0, 0, 0};
+        if (vol >= 0 && vol < g.n_nodes) {
+            NodeRec<R> nd = nav.node(vol);
+            nav.compute_step_normal(vol, nd, x, w, max_step ? max_step[i] : rinf<R>(), step, ng);
+            next = vol;
+        }
+        step_out[i] = step; next_out[i] = next;
+        normal_out[3 * i] = ng.x; normal_out[3 * i + 1] = ng.y; normal_out[3 * i + 2] = ng.z;
+    }
+}
+
 // -------------------------------------------------------------------------------------------------------
 // the paper's own benchmark: Algorithm 1 with attenuation only, one thread per particle
 // -------------------------------------------------------------------------------------------------------
@@ -737,6 +761,25 @@ extern "C" int gn_transport_run(const gn_geometry* geo, int precision, const gn_
     if (precision == 32) return transport_impl<float>(geo, h_src, seed, first_photon_id, n_photons, d_edep_out, h_stats_out, d_hash_out, d_nsteps_out, d_efinal_out, (cudaStream_t)cuda_stream);
     if (precision == 64) return transport_impl<double>(geo, h_src, seed, first_photon_id, n_photons, d_edep_out, h_stats_out, d_hash_out, d_nsteps_out, d_efinal_out, (cudaStream_t)cuda_stream);
     return fail(GN_INVALID_ARGUMENT, "gn_transport_run: precision must be 32 or 64");
+}
+
+template <class R> int step_normal_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
+                                        int64_t n, void* step, int32_t* next, void* normal, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    if (geo->coherent) step_normal_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, (R*)normal);
+    else step_normal_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, (R*)normal);
+    GN_CUDA(cudaGetLastError(), "gn_nav_compute_step_normal launch");
+    return GN_OK;
+}
+
+extern "C" int gn_nav_compute_step_normal(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, const int32_t* d_vol_in,
+                                          const void* d_max_step, int64_t n, void* d_step_out, int32_t* d_next_vol_out, void* d_normal_out,
+                                          void* cuda_stream) {
+    if (!geo || n < 0 || (n > 0 && (!d_pos || !d_dir || !d_vol_in || !d_step_out || !d_next_vol_out || !d_normal_out)))
+        return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step_normal: bad argument");
+    if (precision == 32) return step_normal_impl<float>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, d_normal_out, (cudaStream_t)cuda_stream);
+    if (precision == 64) return step_normal_impl<double>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, d_normal_out, (cudaStream_t)cuda_stream);
+    return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step_normal: precision must be 32 or 64");
 }
 
 template <class R> int free_path_impl(const gn_geometry* geo, const void* pos, const void* dir, const void* Y, int64_t n, double mu_mass,

@@ -424,3 +424,28 @@ def test_free_path_matches_oracle(B, which, precision):
     e3 = torch.empty((0, 3), dtype=torch.float64 if precision == 64 else torch.float32, device="cuda")
     Te, _ = B.free_path_run(g, e3, e3, e3[:, 0].contiguous(), W.MU_MASS_AL_1MEV)
     assert Te.numel() == 0
+
+
+# ---- surface normal of the boundary crossed ---------------------------------
+@pytest.mark.parametrize("name", list(GEOMS) + ["spheres"])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_step_normals_bit_exact(B, name, precision):
+    """gn_nav_compute_step_normal: step, next volume and the outward normal of the surface that ends the step equal the
+    oracle's (plain linear scan, so the voxel walk's tie rule for the daughter hit is checked too)."""
+    geom = spheres_small() if name == "spheres" else GEOMS[name]()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    rng = np.random.default_rng(202)
+    n = 40003
+    R = np.float64 if precision == 64 else np.float32
+    p = query_points(geom, rng, n).astype(R); v = unit(rng, n).astype(R)
+    ref = og.locate(p, v, precision, use_grid=False)
+    step, nxt, nrm = B.nav_compute_step_normal(g, cuda(p), cuda(v), cuda(ref))
+    rstep, rnxt, rnrm = og.compute_step_normal(p, v, ref, None, precision, use_grid=False)
+    assert np.array_equal(step.cpu().numpy(), rstep) and np.array_equal(nxt.cpu().numpy(), rnxt)
+    assert np.array_equal(nrm.cpu().numpy(), rnrm)
+    fin = np.isfinite(rstep)
+    assert np.allclose(np.linalg.norm(rnrm[fin].astype(np.float64), axis=1), 1.0, atol=1e-5) and np.all(rnrm[~fin] == 0)
+    ms = rng.uniform(0, 300, n).astype(R)
+    step, nxt, nrm = B.nav_compute_step_normal(g, cuda(p), cuda(v), cuda(ref), cuda(ms))
+    rstep, rnxt, rnrm = og.compute_step_normal(p, v, ref, ms, precision, use_grid=False)
+    assert np.array_equal(step.cpu().numpy(), rstep) and np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(nrm.cpu().numpy(), rnrm)
