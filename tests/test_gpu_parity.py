@@ -449,3 +449,48 @@ def test_step_normals_bit_exact(B, name, precision):
     step, nxt, nrm = B.nav_compute_step_normal(g, cuda(p), cuda(v), cuda(ref), cuda(ms))
     rstep, rnxt, rnrm = og.compute_step_normal(p, v, ref, ms, precision, use_grid=False)
     assert np.array_equal(step.cpu().numpy(), rstep) and np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(nrm.cpu().numpy(), rnrm)
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled outputs ------------------
+@pytest.mark.parametrize("k,precision,min_same", [(2, 64, 0.999), (2, 32, 0.97), (4, 32, 0.97)])
+def test_config2_config4_full_size_sampled(B, k, precision, min_same):
+    wl = W.config(k)
+    g = B.Geometry(wl.geometry)
+    got = B.transport_run(g, wl.source, wl.seed, wl.n, precision, per_photon=True)
+    s = got["stats"]
+    assert s["n_photons"] == wl.n and s["n_stuck"] <= max(1, wl.n // 10 ** 6)
+    book = float(got["edep"].sum().item()) + s["e_escaped"] + s["e_stuck"]
+    assert abs(book / s["e_source"] - 1) < (1e-11 if precision == 64 else 2e-6)
+    assert int(got["nsteps"].sum(dtype=__import__("torch").int64).item()) == s["n_steps"]
+    og = oracle.OracleGeometry(wl.geometry)
+    first, m = wl.n // 2, 20000
+    ref = og.transport(wl.source, wl.seed, m, precision, first_id=first, per_photon=True)
+    hg = got["hash"][first:first + m].cpu().numpy().view(np.uint64)
+    ng = got["nsteps"][first:first + m].cpu().numpy().astype(np.uint32)
+    ef = got["efinal"][first:first + m].cpu().numpy()
+    same = (hg == ref["hash"]) & (ng == ref["nsteps"]) & (np.abs(ef - ref["efinal"]) <= (1e-9 if precision == 64 else 1e-4) * np.abs(ref["efinal"]))
+    print(f"config {k} fp{precision} full size: identical histories on the sample {same.mean():.5f}")
+    assert same.mean() >= min_same
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_config5_full_size_sampled(B, precision):
+    """1e8 queries (fp32; 5e7 in fp64 to stay within a few seconds), generated on the device as bench.py does; the oracle
+    checks a seeded sample of 40000 of them bit for bit."""
+    import torch
+    wl = W.config(5)
+    g = B.Geometry(wl.geometry)
+    og = oracle.OracleGeometry(wl.geometry)
+    n = wl.n if precision == 32 else wl.n // 2
+    dt = torch.float32 if precision == 32 else torch.float64
+    pos, dirs = W.nav_queries_torch(wl.geometry, n, wl.seed, dt, torch.device("cuda"))
+    vol = B.nav_locate(g, pos, dirs)
+    step, nxt = B.nav_compute_step(g, pos, dirs, vol)
+    sel = torch.from_numpy(np.sort(np.random.default_rng(3).choice(n, 40000, replace=False))).cuda()
+    p = pos[sel].cpu().numpy(); v = dirs[sel].cpu().numpy()
+    rv = og.locate(p, v, precision)
+    rs, rn = og.compute_step(p, v, rv, None, precision)
+    assert np.array_equal(vol[sel].cpu().numpy(), rv)
+    assert np.array_equal(step[sel].cpu().numpy(), rs) and np.array_equal(nxt[sel].cpu().numpy(), rn)
+    # every point of the world box is located, except those within the tolerance of its surface that head outwards (C3)
+    assert n - int((vol >= 0).sum().item()) < n // 10 ** 5
