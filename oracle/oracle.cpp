@@ -310,6 +310,72 @@ template <class R> R orb_dist_in(const SolidR<R>& s, const R p[3], const R v[3],
     return r_max(c / (-b + r_sqrt(Dq)), (R)0);                     /* smaller root */
 }
 
+/* CONE (solid frustum about z: radius r1 at z = -hz, r2 at z = +hz; the paper names the solid, nothing more).
+ * D:"cone solid".  Stored: a = r0 = (r1 + r2)/2, b = m = (r2 - r1)/(2 hz), c = hz, cS = cs = 1/sqrt(1 + m^2) (fp64 on the
+ * host, rounded once).  Surface radius u(z) = r0 + m z; s_z = |z| - hz; s_c = (r - u) cs (true distance to the cone).
+ * Along a ray, f(t) = r(t)^2 - u(t)^2 = A t^2 + 2 B t + C with du = m v_z, A = (vx^2 + vy^2) - du^2,
+ * B = (x vx + y vy) - u du, C = (x^2 + y^2) - u^2; B > 0 <=> moving outward at the surface. */
+template <class R> int cone_inside(const SolidR<R>& s, const R p[3], R delta) {
+    R r = r_sqrt(p[0] * p[0] + p[1] * p[1]);
+    R u = s.a + s.b * p[2];
+    R D = r_max(r_abs(p[2]) - s.c, (r - u) * s.cS);
+    return classify(D, delta);
+}
+template <class R> R cone_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R best = r_inf<R>();
+    if (!slab_out(p[2], v[2], s.c, delta, best)) return 0;            /* z planes */
+    R u = s.a + s.b * p[2], du = s.b * v[2];
+    R A = (v[0] * v[0] + v[1] * v[1]) - du * du;
+    R B = (p[0] * v[0] + p[1] * v[1]) - u * du;
+    R r2 = p[0] * p[0] + p[1] * p[1];
+    R C = r2 - u * u;
+    if (B > 0 && (r_sqrt(r2) - u) * s.cS >= -delta) return 0;          /* on the cone's band, moving outward */
+    R q = r_sqrt(r_max(B * B - A * C, (R)0));
+    /* first t > 0 at which f turns positive: -C/(B + q) when B > 0 (any A), else the larger root if A > 0, else never */
+    if (B > 0) best = r_min(best, -C / (B + q));
+    else if (A > 0) best = r_min(best, (-B + q) / A);
+    return r_max(best, (R)0);
+}
+template <class R> R cone_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
+    R best = r_inf<R>();
+    R u = s.a + s.b * p[2], du = s.b * v[2];
+    R r2 = p[0] * p[0] + p[1] * p[1];
+    R r = r_sqrt(r2);
+    /* (i) end planes: validate against the cone at the hit point */
+    R sz = r_abs(p[2]) - s.c;
+    if (sz >= -delta) {
+        if (p[2] * v[2] >= 0) return r_inf<R>();
+        R t = r_max(sz / r_abs(v[2]), (R)0);
+        R q[3] = {r_fma(t, v[0], p[0]), r_fma(t, v[1], p[1]), r_fma(t, v[2], p[2])};
+        R rq = r_sqrt(q[0] * q[0] + q[1] * q[1]);
+        if ((rq - (s.a + s.b * q[2])) * s.cS <= delta) best = r_min(best, t);
+    }
+    /* (ii) conical surface from outside: the root where f turns from + to - (slope A t + B = -q < 0), i.e.
+     * t = (-B - q)/A, evaluated without cancellation: C / (-B + q) when B < 0, (B + q) / (-A) when B >= 0 and A < 0 (a ray
+     * steeper than the cone, possibly starting beyond the apex), none otherwise.  The ray must cross the surface moved
+     * inwards by delta (no graze loops); z is validated at the hit point (this also rejects the other nappe). */
+    if ((r - u) * s.cS >= -delta) {
+        R A = (v[0] * v[0] + v[1] * v[1]) - du * du;
+        R us = u - delta / s.cS;
+        R Bs = (p[0] * v[0] + p[1] * v[1]) - us * du, Cs = r2 - us * us;
+        if (Bs * Bs - A * Cs > 0) {
+            R B = (p[0] * v[0] + p[1] * v[1]) - u * du, C = r2 - u * u;
+            R Dq = B * B - A * C;
+            if (Dq > 0) {
+                R q = r_sqrt(Dq), t = 0; bool have = false;
+                if (B < 0) { t = C / (-B + q); have = true; }
+                else if (A < 0) { t = (B + q) / (-A); have = true; }
+                if (have) {
+                    t = r_max(t, (R)0);
+                    R zq = r_fma(t, v[2], p[2]);
+                    if (r_abs(zq) <= s.c + delta && (B + A * t) < 0) best = r_min(best, t);      /* moving inward there */
+                }
+            }
+        }
+    }
+    return best;
+}
+
 /* Outward unit normal of the bounding surface a point q (local frame) lies on -- "what is the normal of the boundary
  * surface at that point?".  D:"surface normal": the surface is the one whose signed outsideness s_k(q) is the
  * largest (the one q is on, or nearest to; ties -> first in the order listed), the normal is the gradient of that s_k:
@@ -317,6 +383,7 @@ template <class R> R orb_dist_in(const SolidR<R>& s, const R p[3], const R v[3],
  *   TUBE  s_z = |z| - hz; s_out = r - rmax; s_in = rmin - r; s_S; s_E     n = sign(z) e_z; (x, y, 0)/r; -(x, y, 0)/r;
  *                                                              (sS, -cS, 0); (-sE, cE, 0)
  *   ORB   n = q / |q|
+ *   CONE  s_z, s_c = (r - u(z)) cs                             n = sign(z) e_z; cs (x/r, y/r, -m)
  * (r = 0 on a cylinder or |q| = 0 on an orb cannot be on the surface; the x axis is returned.) */
 template <class R> void solid_normal(const SolidR<R>& s, const R q[3], R n[3]) {
     n[0] = n[1] = n[2] = 0;
@@ -331,6 +398,14 @@ template <class R> void solid_normal(const SolidR<R>& s, const R q[3], R n[3]) {
         R rp = r_sqrt((q[0] * q[0] + q[1] * q[1]) + q[2] * q[2]);
         if (!(rp > 0)) { n[0] = 1; return; }
         n[0] = q[0] / rp; n[1] = q[1] / rp; n[2] = q[2] / rp;
+        return;
+    }
+    if (s.type == ORACLE_CONE) {                  /* surfaces: z planes, cone; grad s_c = cs (x/r, y/r, -m) */
+        R rc = r_sqrt(q[0] * q[0] + q[1] * q[1]);
+        R sz = r_abs(q[2]) - s.c, sc = (rc - (s.a + s.b * q[2])) * s.cS;
+        if (!(sc > sz)) { n[2] = q[2] < 0 ? (R)-1 : (R)1; return; }
+        if (!(rc > 0)) { n[0] = 1; return; }
+        n[0] = (q[0] / rc) * s.cS; n[1] = (q[1] / rc) * s.cS; n[2] = -s.b * s.cS;
         return;
     }
     R r = r_sqrt(q[0] * q[0] + q[1] * q[1]);
@@ -352,13 +427,13 @@ template <class R> void solid_normal(const SolidR<R>& s, const R q[3], R n[3]) {
 
 /* the "fork" on solid type */
 template <class R> int solid_inside(const SolidR<R>& s, const R p[3], R delta) {
-    return s.type == ORACLE_BOX ? box_inside(s, p, delta) : (s.type == ORACLE_TUBE ? tube_inside(s, p, delta) : orb_inside(s, p, delta));
+    return s.type == ORACLE_BOX ? box_inside(s, p, delta) : (s.type == ORACLE_TUBE ? tube_inside(s, p, delta) : (s.type == ORACLE_ORB ? orb_inside(s, p, delta) : cone_inside(s, p, delta)));
 }
 template <class R> R solid_dist_in(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
-    return s.type == ORACLE_BOX ? box_dist_in(s, p, v, delta) : (s.type == ORACLE_TUBE ? tube_dist_in(s, p, v, delta) : orb_dist_in(s, p, v, delta));
+    return s.type == ORACLE_BOX ? box_dist_in(s, p, v, delta) : (s.type == ORACLE_TUBE ? tube_dist_in(s, p, v, delta) : (s.type == ORACLE_ORB ? orb_dist_in(s, p, v, delta) : cone_dist_in(s, p, v, delta)));
 }
 template <class R> R solid_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
-    return s.type == ORACLE_BOX ? box_dist_out(s, p, v, delta) : (s.type == ORACLE_TUBE ? tube_dist_out(s, p, v, delta) : orb_dist_out(s, p, v, delta));
+    return s.type == ORACLE_BOX ? box_dist_out(s, p, v, delta) : (s.type == ORACLE_TUBE ? tube_dist_out(s, p, v, delta) : (s.type == ORACLE_ORB ? orb_dist_out(s, p, v, delta) : cone_dist_out(s, p, v, delta)));
 }
 
 /* ---- navigator (S:C3, S:C4) ------------------------------------------------------------ */
@@ -750,6 +825,7 @@ void mat3_mul(const double* A, const double* B, double* C) {
 void solid_aabb(const SolidD& s, double lo[3], double hi[3]) {
     if (s.type == ORACLE_BOX) { lo[0] = -s.a; hi[0] = s.a; lo[1] = -s.b; hi[1] = s.b; lo[2] = -s.c; hi[2] = s.c; return; }
     if (s.type == ORACLE_ORB) { for (int k = 0; k < 3; ++k) { lo[k] = -s.a; hi[k] = s.a; } return; }
+    if (s.type == ORACLE_CONE) { lo[0] = lo[1] = -s.sphi; hi[0] = hi[1] = s.sphi; lo[2] = -s.c; hi[2] = s.c; return; }
     lo[2] = -s.c; hi[2] = s.c;
     if (!s.sector) { lo[0] = lo[1] = -s.b; hi[0] = hi[1] = s.b; return; }
     double xs[16], ys[16]; int n = 0;
@@ -770,6 +846,7 @@ void build_grid(Geo& g, int mother) {
     const SolidD& ms = g.solids[g.solid[mother]];
     if (ms.type == ORACLE_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; mlo[2] = -ms.c; mhi[2] = ms.c; }
     else if (ms.type == ORACLE_ORB) { for (int k = 0; k < 3; ++k) { mlo[k] = -ms.a; mhi[k] = ms.a; } }
+    else if (ms.type == ORACLE_CONE) { mlo[0] = mlo[1] = -ms.sphi; mhi[0] = mhi[1] = ms.sphi; mlo[2] = -ms.c; mhi[2] = ms.c; }
     else { mlo[0] = mlo[1] = -ms.b; mhi[0] = mhi[1] = ms.b; mlo[2] = -ms.c; mhi[2] = ms.c; }
     int nper = (int)std::ceil(std::cbrt((double)ds.size()));
     nper = std::max(1, std::min(nper, 64));
@@ -886,6 +963,14 @@ int make_solid(int type, const double* p, SolidD& s) {
         if (!(s.a > 0)) return ORACLE_INVALID_ARGUMENT;
         return ORACLE_OK;
     }
+    if (type == ORACLE_CONE) {                    /* params r1, r2, hz -> a = r0, b = slope, c = hz, cS = 1/sqrt(1 + slope^2) */
+        double r1 = p[0], r2 = p[1], hz = p[2];
+        if (!(r1 >= 0 && r2 >= 0 && r1 + r2 > 0 && hz > 0)) return ORACLE_INVALID_ARGUMENT;
+        s.a = (r1 + r2) / 2; s.b = (r2 - r1) / (2 * hz); s.c = hz;
+        s.cS = 1 / std::sqrt(1 + s.b * s.b);
+        s.sphi = r1 > r2 ? r1 : r2;               /* largest radius, for bounding boxes only */
+        return ORACLE_OK;
+    }
     if (type != ORACLE_TUBE) return ORACLE_UNSUPPORTED_SOLID;
     s.a = p[0]; s.b = p[1]; s.c = p[2]; s.sphi = p[3]; s.dphi = p[4];
     if (!(s.a >= 0 && s.b > s.a && s.c > 0)) return ORACLE_INVALID_ARGUMENT;
@@ -948,7 +1033,7 @@ int oracle_geometry_create(const double* materials, int32_t n_mats, const int32_
         for (int a = 0; a < 3; ++a) { g->x64[i].T[a] = T[a]; g->x32[i].T[a] = (float)T[a]; }
     }
     const SolidD& ws = g->solids[g->solid[0]];
-    double ext = ws.type == ORACLE_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == ORACLE_ORB ? ws.a : std::max(ws.b, ws.c));
+    double ext = ws.type == ORACLE_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == ORACLE_ORB ? ws.a : (ws.type == ORACLE_CONE ? std::max(ws.sphi, ws.c) : std::max(ws.b, ws.c)));
     g->tol64 = (opts && opts->tol64 > 0) ? opts->tol64 : 1e-9;
     g->tol32 = (opts && opts->tol32 > 0) ? opts->tol32 : (double)(float)(ext * 0x1p-18);
     g->sigma_pe0 = (opts && opts->sigma_pe0 > 0) ? opts->sigma_pe0 : 1750.0;

@@ -23,7 +23,7 @@ extern "C" {
 #endif
 
 enum { ORACLE_OK = 0, ORACLE_INVALID_ARGUMENT = -1, ORACLE_UNSUPPORTED_SOLID = -2, ORACLE_BAD_TREE = -3 };
-enum { ORACLE_BOX = 0, ORACLE_TUBE = 1, ORACLE_ORB = 2 };
+enum { ORACLE_BOX = 0, ORACLE_TUBE = 1, ORACLE_ORB = 2, ORACLE_CONE = 3 };
 enum { ORACLE_SRC_PENCIL = 0, ORACLE_SRC_GAUSS_PENCIL = 1, ORACLE_SRC_CONE = 2, ORACLE_SRC_ISOTROPIC = 3 };
 enum { ORACLE_E_MONO = 0, ORACLE_E_LOGUNIFORM = 1 };
 
@@ -53,7 +53,7 @@ typedef struct {
 
 /* geometry ------------------------------------------------------------------------------ */
 /* materials: n_mats x 3 doubles (Z, A, rho).  solid_type: n_solids int32; solid_params: n_solids x 5
- * doubles (BOX: hx,hy,hz,-,-; TUBE: rmin,rmax,hz,sphi,dphi; ORB: r,-,-,-,-).  placements: n_places x 4 int32
+ * doubles (BOX: hx,hy,hz,-,-; TUBE: rmin,rmax,hz,sphi,dphi; ORB: r,-,-,-,-; CONE: r1 (at -hz),r2 (at +hz),hz,-,-).  placements: n_places x 4 int32
  * (parent, solid, material, transform); node 0 is the world (parent -1), parent < child.
  * transforms: n_transforms x 12 doubles, R row-major (local->parent) then T.                      */
 int oracle_geometry_create(const double* materials, int32_t n_mats,

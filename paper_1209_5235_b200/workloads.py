@@ -5,8 +5,8 @@ of the method's arithmetic: no navigation, no physics, no RNG of the method -- o
 inputs as plain numpy arrays in the layout both C interfaces take:
 
     materials    (n_mats, 3)  float64   Z, A, rho [g/cm3]
-    solid_type   (n_solids,)  int32     0 = BOX, 1 = TUBE, 2 = ORB
-    solid_params (n_solids,5) float64   BOX: hx,hy,hz,0,0 [mm]; TUBE: rmin,rmax,hz [mm], sphi,dphi [rad]; ORB: r,0,0,0,0
+    solid_type   (n_solids,)  int32     0 = BOX, 1 = TUBE, 2 = ORB, 3 = CONE
+    solid_params (n_solids,5) float64   BOX: hx,hy,hz,0,0 [mm]; TUBE: rmin,rmax,hz [mm], sphi,dphi [rad]; ORB: r,0,0,0,0; CONE: r1 (at -hz),r2 (at +hz),hz,0,0
     placements   (n_places,4) int32     parent (-1 for node 0 = world; parent < child), solid, material, transform
     transforms   (n_tr, 12)   float64   R row-major (local->parent) then T [mm]
 
@@ -22,7 +22,7 @@ from typing import Optional
 
 import numpy as np
 
-BOX, TUBE, ORB = 0, 1, 2
+BOX, TUBE, ORB, CONE = 0, 1, 2, 3
 SRC_PENCIL, SRC_GAUSS_PENCIL, SRC_CONE, SRC_ISOTROPIC = 0, 1, 2, 3
 E_MONO, E_LOGUNIFORM = 0, 1
 
@@ -99,6 +99,9 @@ class _Builder:
 
     def orb(self, r):
         self.stype.append(ORB); self.sparams.append((r, 0.0, 0.0, 0.0, 0.0)); return len(self.stype) - 1
+
+    def cone(self, r1, r2, hz):
+        self.stype.append(CONE); self.sparams.append((r1, r2, hz, 0.0, 0.0)); return len(self.stype) - 1
 
     def place(self, parent, solid, material, R=None, T=(0.0, 0.0, 0.0)):
         R = np.eye(3) if R is None else np.asarray(R, dtype=np.float64)
@@ -275,6 +278,38 @@ def lattice_geometry(n=4, seed=7, pitch=100.0, fill="aluminium") -> Geometry:
         r = rmax * 0.5
         pos = (r * math.cos(1.0), r * math.sin(1.0), 0.0) if s != 0 else (0.0, 0.0, 0.0)
         b.place(node, inner, "lead", R=rot_z(rng.uniform(0, 6.28)), T=pos)
+    return b.finish()
+
+
+def mixed_solids_geometry(n=4, seed=9, pitch=100.0) -> Geometry:
+    """All four solid types the paper names (boxes, tubes, cones, spheres) on a regular grid in a vacuum
+    cube, randomly rotated; every fourth solid holds a small ball.  Test geometry for the orb and cone solids."""
+    rng = np.random.default_rng(seed)
+    b = _Builder(f"mixed_{n}")
+    half = n * pitch / 2
+    world = b.place(-1, b.box(half + 40, half + 40, half + 40), "vacuum")
+    rmax = 0.5 * pitch / math.sqrt(3) * 0.95
+    solids = [
+        b.box(rmax * 0.55, rmax * 0.5, rmax * 0.6),
+        b.tube(rmax * 0.3, rmax * 0.7, rmax * 0.7, 0.3, 2.1),
+        b.orb(rmax * 0.8),
+        b.cone(rmax * 0.2, rmax * 0.7, rmax * 0.65),
+        b.cone(rmax * 0.7, 0.0, rmax * 0.5),
+        b.cone(rmax * 0.6, rmax * 0.6, rmax * 0.6),
+    ]
+    inner = b.orb(rmax * 0.1)
+    k = 0
+    for iz in range(n):
+        for iy in range(n):
+            for ix in range(n):
+                s = int(rng.integers(len(solids)))
+                c = (-half + pitch * (ix + 0.5), -half + pitch * (iy + 0.5), -half + pitch * (iz + 0.5))
+                node = b.place(world, solids[s], "aluminium", R=random_rotation(rng), T=c)
+                if k % 4 == 0:
+                    # on the axis at z = -0.3 hz for cones (inside every frustum above), at a radius with material for the tube
+                    pos = (rmax * 0.5 * math.cos(1.3), rmax * 0.5 * math.sin(1.3), 0.0) if s == 1 else (0.0, 0.0, -0.1 * rmax)
+                    b.place(node, inner, "lead", T=pos)
+                k += 1
     return b.finish()
 
 
