@@ -35,7 +35,7 @@ typedef enum {
     GN_CUDA_ERROR = -5
 } gn_status;
 
-enum { GN_BOX = 0, GN_TUBE = 1, GN_ORB = 2 };
+enum { GN_BOX = 0, GN_TUBE = 1, GN_ORB = 2, GN_CONE = 3 };
 enum { GN_SRC_PENCIL = 0, GN_SRC_GAUSS_PENCIL = 1, GN_SRC_CONE = 2, GN_SRC_ISOTROPIC = 3 };
 enum { GN_E_MONO = 0, GN_E_LOGUNIFORM = 1 };
 
@@ -83,7 +83,8 @@ typedef struct {
 /*
  * gn_geometry_create -- PAPER.md L139 / L127 (volumes hierarchy, solids, per-material density).
  *   h_materials    n_mats x 3 doubles: Z, A [g/mol], rho [g/cm3]
- *   h_solid_type   n_solids int32: GN_BOX | GN_TUBE | GN_ORB (ORB: r,-,-,-,- )
+ *   h_solid_type   n_solids int32: GN_BOX | GN_TUBE | GN_ORB | GN_CONE (ORB: r,-,-,-,- ; CONE: solid frustum, r1 at -hz, r2 at +hz, hz,-,- ;
+ *                  DESIGN.md "orb solid" / "cone solid"; the four solid types PAPER.md L160 names)
  *   h_solid_params n_solids x 5 doubles: BOX hx,hy,hz,-,- ; TUBE rmin,rmax,hz,sphi,dphi  (C2; dphi >= 2 pi
  *                  = full tube, 0 < dphi <= pi = convex sector)
  *   h_placements   n_places x 4 int32: parent (-1 for node 0 = world, parent < child), solid, material,

@@ -21,7 +21,7 @@ namespace {
 const double kRe = 2.8179403262e-13, kAlpha = 7.2973525693e-3, kNA = 6.02214076e23, kBarn = 1e-24;
 const double kPi = 3.14159265358979323846;
 
-struct HostSolid { int type; double a, b, c, sphi, dphi; bool sector; double cS, sS, cE, sE; };
+struct HostSolid { int type; double a, b, c, sphi, dphi; bool sector; double cS, sS, cE, sE; double rbound; };
 
 struct Uploader {
     gn_geometry* geo; bool ok = true; std::string err;
@@ -66,6 +66,7 @@ void daughter_bounds(const HostSolid& s, const double* R, const double* T, doubl
     }
     double l[3], h[3];
     if (s.type == GN_BOX) { l[0] = -s.a; h[0] = s.a; l[1] = -s.b; h[1] = s.b; l[2] = -s.c; h[2] = s.c; }
+    else if (s.type == GN_CONE) { l[0] = l[1] = -s.rbound; h[0] = h[1] = s.rbound; l[2] = -s.c; h[2] = s.c; }
     else if (s.type == GN_ORB) {          // rotation invariant
         for (int k = 0; k < 3; ++k) { lo[k] = T[k] - s.a; hi[k] = T[k] + s.a; }
         return;
@@ -87,7 +88,7 @@ void daughter_bounds(const HostSolid& s, const double* R, const double* T, doubl
 template <class R> SolidRec<R> make_solid_rec(const HostSolid& s) {
     SolidRec<R> o;
     o.a = (R)s.a; o.b = (R)s.b; o.c = (R)s.c; o.cS = (R)s.cS; o.sS = (R)s.sS; o.cE = (R)s.cE; o.sE = (R)s.sE;
-    o.type = s.type == GN_BOX ? SOLID_BOX : (s.type == GN_ORB ? SOLID_ORB : SOLID_TUBE);
+    o.type = s.type == GN_BOX ? SOLID_BOX : (s.type == GN_ORB ? SOLID_ORB : (s.type == GN_CONE ? SOLID_CONE : SOLID_TUBE));
     o.flags = 0;
     if (s.type == GN_TUBE) { if (s.sector) o.flags |= TUBE_SECTOR; if (o.a > 0) o.flags |= TUBE_HOLE; }
     return o;
@@ -135,6 +136,12 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         s.a = p[0]; s.b = p[1]; s.c = p[2];
         if (s.type == GN_BOX) {
             if (!(s.a > 0 && s.b > 0 && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: box half-lengths must be positive");
+        } else if (s.type == GN_CONE) {       // r1 (at -hz), r2 (at +hz), hz -> a = r0, b = slope, c = hz, cS = 1/sqrt(1 + slope^2)
+            const double r1 = p[0], r2 = p[1], hz = p[2];
+            if (!(r1 >= 0 && r2 >= 0 && r1 + r2 > 0 && hz > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: cone needs r1, r2 >= 0, r1 + r2 > 0, hz > 0");
+            s.a = (r1 + r2) / 2; s.b = (r2 - r1) / (2 * hz); s.c = hz;
+            s.cS = 1 / std::sqrt(1 + s.b * s.b);
+            s.rbound = r1 > r2 ? r1 : r2;
         } else if (s.type == GN_ORB) {
             s.b = s.c = 0;
             if (!(s.a > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: orb radius must be positive");
@@ -188,7 +195,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     cudaGetDevice(&geo->device);
     gn_opts o{}; if (h_opts) o = *h_opts;
     const HostSolid& ws = solids[node[0].y];
-    double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == GN_ORB ? ws.a : std::max(ws.b, ws.c));
+    double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == GN_ORB ? ws.a : (ws.type == GN_CONE ? std::max(ws.rbound, ws.c) : std::max(ws.b, ws.c)));
     geo->tol64 = o.tol64 > 0 ? o.tol64 : 1e-9;
     geo->tol32 = o.tol32 > 0 ? o.tol32 : (double)(float)(ext * 0x1p-18);
     if (!(o.sigma_pe0 > 0)) o.sigma_pe0 = 1750.0;
@@ -212,6 +219,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         const HostSolid& ms = solids[node[mth].y];
         double mlo[3], mhi[3];
         if (ms.type == GN_ORB) { mlo[0] = mlo[1] = -ms.a; mhi[0] = mhi[1] = ms.a; }
+        else if (ms.type == GN_CONE) { mlo[0] = mlo[1] = -ms.rbound; mhi[0] = mhi[1] = ms.rbound; }
         else if (ms.type == GN_BOX) { mlo[0] = -ms.a; mhi[0] = ms.a; mlo[1] = -ms.b; mhi[1] = ms.b; }
         else { mlo[0] = mlo[1] = -ms.b; mhi[0] = mhi[1] = ms.b; }
         mlo[2] = -ms.c; mhi[2] = ms.c;

@@ -18,13 +18,13 @@
 
 namespace gn {
 
-enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2 };
+enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2, SOLID_CONE = 3 };
 enum : int { TUBE_SECTOR = 1, TUBE_HOLE = 2 };
 enum : int { NODE_IDENTITY = 1 << 30, NODE_SOLID_MASK = (1 << 30) - 1 };
 
 template <class R> struct SolidRec {
-    R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -
-    R cS, sS, cE, sE;     // trig of sphi and sphi + dphi (host libm, fp64, rounded once)
+    R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -      CONE: r0 = (r1 + r2)/2, slope m, hz
+    R cS, sS, cE, sE;     // trig of sphi and sphi + dphi (host libm, fp64, rounded once);  CONE: cS = 1/sqrt(1 + m^2)
     int type, flags;
 };
 

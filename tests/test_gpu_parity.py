@@ -41,6 +41,7 @@ GEOMS = {
     "calorimeter": lambda: W.calorimeter_geometry(8),
     "detector": lambda: W.detector_geometry(seed=4, n_phi=16, n_z=8, barrels=((200, 400), (450, 650))),
     "lattice": lambda: W.lattice_geometry(4, seed=7),
+    "mixed": lambda: W.mixed_solids_geometry(),          # boxes, tubes, cones, balls, rotated, nested balls
 }
 
 
@@ -50,7 +51,7 @@ def query_points(geom, rng, n):
     s = int(geom.placements[1, 1]); q = geom.solid_params[s]
     ext = np.array([q[0], q[1], q[2]]) if geom.solid_type[s] == 0 else np.array([q[1], q[1], q[2]])
     c = geom.transforms[int(geom.placements[1, 3]), 9:]
-    if geom.name.startswith("lattice"):
+    if geom.name.startswith("lattice") or geom.name.startswith("mixed"):
         ext, c = h * 0.9, np.zeros(3)
     p[: n // 2] = c + rng.uniform(-1, 1, size=(n // 2, 3)) * ext * 1.05
     if geom.name.startswith("config3"):                 # points exactly on voxel faces / edges / corners
@@ -494,3 +495,41 @@ def test_config5_full_size_sampled(B, precision):
     assert np.array_equal(step[sel].cpu().numpy(), rs) and np.array_equal(nxt[sel].cpu().numpy(), rn)
     # every point of the world box is located, except those within the tolerance of its surface that head outwards (C3)
     assert n - int((vol >= 0).sum().item()) < n // 10 ** 5
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_cones_and_balls_dense_queries(B, precision):
+    """queries concentrated in and around every solid of the mixed geometry (boxes, tube sectors, balls,
+    three cone shapes incl. one with its apex on an end plane, all randomly rotated, some with a nested ball), a share of
+    them exactly on the solids' bounding spheres' tangent directions: locate, ComputeStep and the surface normal equal the
+    oracle's linear scans bit for bit."""
+    geom = W.mixed_solids_geometry()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    rng = np.random.default_rng(77)
+    R = np.float64 if precision == 64 else np.float32
+    centres = geom.transforms[geom.placements[1:65, 3], 9:]                   # the 64 top-level solids
+    n = 120000
+    c = centres[rng.integers(0, len(centres), n)]
+    p = (c + unit(rng, n) * rng.uniform(0, 40.0, n)[:, None]).astype(R)
+    v = unit(rng, n)
+    aim = rng.random(n) < 0.5                                                  # half of the rays aim at the solid's region
+    tgt = c + unit(rng, n) * rng.uniform(0, 25.0, n)[:, None]
+    dv = tgt - p.astype(np.float64); nv = np.linalg.norm(dv, axis=1, keepdims=True)
+    v = np.where(aim[:, None] & (nv > 1e-6), dv / np.maximum(nv, 1e-300), v).astype(R)
+    v = (v.astype(np.float64) / np.linalg.norm(v.astype(np.float64), axis=1, keepdims=True)).astype(R)
+    tp, tv = cuda(p), cuda(v)
+    ref = og.locate(p, v, precision, use_grid=False)
+    assert np.array_equal(B.nav_locate(g, tp, tv).cpu().numpy(), ref)
+    stype = geom.solid_type[geom.placements[np.maximum(ref, 0), 1]]
+    assert (stype[ref > 0] == 3).sum() > 5000 and (stype[ref > 0] == 2).sum() > 3000
+    step, nxt, nrm = B.nav_compute_step_normal(g, tp, tv, cuda(ref))
+    rstep, rnxt, rnrm = og.compute_step_normal(p, v, ref, None, precision, use_grid=False)
+    assert np.array_equal(step.cpu().numpy(), rstep) and np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(nrm.cpu().numpy(), rnrm)
+    s2, n2 = B.nav_compute_step(g, tp, tv, cuda(ref))
+    assert np.array_equal(s2.cpu().numpy(), rstep) and np.array_equal(n2.cpu().numpy(), rnxt)
+    # second leg from the crossing points (on the surfaces): relocation and the next step
+    fin = np.isfinite(rstep) & (rnxt >= 0)
+    x2 = oracle.move(p[fin], v[fin], rstep[fin], precision)
+    r2s, r2n, r2m = og.compute_step_normal(x2, v[fin], rnxt[fin], None, precision, use_grid=False)
+    g2s, g2n, g2m = B.nav_compute_step_normal(g, cuda(x2), cuda(v[fin]), cuda(rnxt[fin]))
+    assert np.array_equal(g2s.cpu().numpy(), r2s) and np.array_equal(g2n.cpu().numpy(), r2n) and np.array_equal(g2m.cpu().numpy(), r2m)
