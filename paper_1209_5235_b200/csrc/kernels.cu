@@ -688,8 +688,14 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             }
             const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
             const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
-            if (p == 0) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
-            else if (last) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
+            // FLAT = general geometry (any solid, rotations, long candidate lists); !FLAT = unrotated boxes only (geo->coherent)
+            if (p == 0) {
+                if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
+                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
+            } else if (last) {
+                if (geo->coherent) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
+                else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
+            }
             else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
                 launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp);
