@@ -162,7 +162,10 @@ __global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, co
 constexpr int TR_THREADS = 128;
 constexpr int TR_WARPS = TR_THREADS / 32;
 #ifndef TR_MIN_BLOCKS
-#define TR_MIN_BLOCKS 8
+#define TR_MIN_BLOCKS 8          // general fp32 step pass: 64 registers, 32 warps / SM
+#endif
+#ifndef TR_MIN_BLOCKS_BOX
+#define TR_MIN_BLOCKS_BOX 6      // box-only fp32 step pass: 80 registers (no spills), 24 warps / SM
 #endif
 constexpr int INTERACT_BATCH = 8;     // parked lanes that trigger a warp's interaction phase
 enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
@@ -285,7 +288,7 @@ __device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, cons
 // back of the output queue; interact_pass handles them before the next pass.  PHYS = true: interactions happen inside
 // the pass (batched per warp); used for the last pass, which runs the few remaining photons to completion.
 template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
-__global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS && !FROM_SOURCE) ? TR_MIN_BLOCKS : 1)
+__global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS && !FROM_SOURCE) ? (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX) : 1)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
                double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct) {
