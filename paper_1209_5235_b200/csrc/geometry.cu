@@ -211,6 +211,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
 
     // ---- voxel grids (C5): one uniform 3-D grid per mother = three nested levels of uniform slices, flattened
     std::vector<HostGrid> grids;
+    std::vector<int> regular_cell(V, -1);      // leaf box that coincides with one voxel cell of its mother: ix | iy << 10 | iz << 20
     std::vector<int> cell_start(1, 0), cand;
     const double shrink = geo->tol64 / 8;
     for (size_t mth = 0; mth < V; ++mth) {
@@ -304,6 +305,21 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
                     for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
                         cand[pos[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++] = d;
         }
+        // regular voxels: an unrotated leaf box that fills exactly one cell, alone
+        for (int j = 0; j < nd; ++j) {
+            int d = dlist[kids[mth].x + j];
+            if (kids[d].y != 0 || solids[node[d].y].type != GN_BOX) continue;
+            const double* Rl = h_transforms + 12 * (size_t)h_placements[4 * (size_t)d + 3];
+            bool ok = Rl[0] == 1.0 && Rl[4] == 1.0 && Rl[8] == 1.0 && Rl[1] == 0.0 && Rl[2] == 0.0 && Rl[3] == 0.0 && Rl[5] == 0.0 && Rl[6] == 0.0 && Rl[7] == 0.0;
+            for (int k = 0; k < 3 && ok; ++k) {
+                int a = c0[3 * (size_t)j + k], b = c1[3 * (size_t)j + k];
+                ok = a == b && a < 1024 && std::fabs(blo[3 * (size_t)j + k] - (G.gmin[k] + a * G.w[k])) <= geo->tol64 && std::fabs(bhi[3 * (size_t)j + k] - (G.gmin[k] + (a + 1) * G.w[k])) <= geo->tol64;
+            }
+            if (!ok) continue;
+            size_t cell = c0[3 * (size_t)j] + (size_t)G.n[0] * (c0[3 * (size_t)j + 1] + (size_t)G.n[1] * c0[3 * (size_t)j + 2]);
+            if (count[cell] != 1) continue;
+            regular_cell[d] = c0[3 * (size_t)j] | (c0[3 * (size_t)j + 1] << 10) | (c0[3 * (size_t)j + 2] << 20);
+        }
         node[mth].w = (int)grids.size();
         grids.push_back(G);
         geo->n_cells += (int64_t)ncell;
@@ -326,6 +342,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         a.mat = b.mat = node[i].z;
         a.ndau = b.ndau = kids[i].y;
         a.link = b.link = node[i].w >= 0 ? ~node[i].w : kids[i].x;        // voxelised mother: ~grid id
+        if (regular_cell[i] >= 0) { a.info = b.info = a.info | NODE_REGULAR; a.link = b.link = regular_cell[i]; }
         b.pad = 0;
         for (int k = 0; k < 3; ++k) { b.t[k] = Tg[3 * i + k]; a.t[k] = (float)Tg[3 * i + k]; }
     }
@@ -382,8 +399,8 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         for (int i = 0; i < n_mats; ++i) rho[i] = h_materials[3 * i + 2];
         a.rho = b.rho = up.put(rho);
     }
-    a.tol = (float)geo->tol32; a.delta = a.tol / 2; a.probe = std::max(a.tol, (float)(ext * 0x1p-18)); a.e_cut = (float)o.e_cut;
-    b.tol = geo->tol64; b.delta = b.tol / 2; b.probe = b.tol; b.e_cut = o.e_cut;
+    a.tol = (float)geo->tol32; a.delta = a.tol / 2; a.probe = (float)(1.25 * 0.5 * geo->tol32 + 4.0 * ext * 0x1p-23); a.e_cut = (float)o.e_cut;
+    b.tol = geo->tol64; b.delta = b.tol / 2; b.probe = 1.25 * 0.5 * geo->tol64 + 4.0 * ext * 0x1p-52; b.e_cut = o.e_cut;
     a.n_nodes = b.n_nodes = n_places; a.n_solids = b.n_solids = n_solids; a.n_mats = b.n_mats = n_mats;
     a.stuck_limit = b.stuck_limit = o.stuck_limit;
     if (!up.ok) {

@@ -8,6 +8,10 @@
 //             flag NODE_IDENTITY: the composed rotation is exactly the identity, so p_local = x - Tg and
 //             v_local = w (the general fma chain gives the same values; only the sign of zeros can differ,
 //             which no comparison in the navigator can see) and `rot` is never read for this node
+//             flag NODE_REGULAR (leaf boxes only): the box coincides with exactly one cell of its mother's voxel grid,
+//             is that cell's only candidate and is not rotated against the mother; link = ix | iy << 10 | iz << 20
+//             (its cell).  A photon leaving it through a face or an edge finds the candidates in the neighbouring
+//             cells directly, without the general cell lookup (nav.cuh: settle, box-only kernels)
 //   rot[i]    M (row-major, global->local rotation), 9 Real padded to 12 (fp32, three 16-byte loads) /
 //             10 (fp64, five 16-byte loads);  p_local = M (x - Tg)
 //   solids, mats, grids: small tables (staged to shared memory by every kernel)
@@ -20,7 +24,7 @@ namespace gn {
 
 enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2, SOLID_CONE = 3 };
 enum : int { TUBE_SECTOR = 1, TUBE_HOLE = 2 };
-enum : int { NODE_IDENTITY = 1 << 30, NODE_SOLID_MASK = (1 << 30) - 1 };
+enum : int { NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SOLID_MASK = (1 << 29) - 1 };
 
 template <class R> struct SolidRec {
     R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -      CONE: r0 = (r1 + r2)/2, slope m, hz
