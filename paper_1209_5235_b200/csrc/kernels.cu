@@ -164,6 +164,9 @@ constexpr int TR_WARPS = TR_THREADS / 32;
 #ifndef TR_MIN_BLOCKS
 #define TR_MIN_BLOCKS 8          // general fp32 step pass: 64 registers, 32 warps / SM
 #endif
+#ifndef TR_MIN_BLOCKS_SRC
+#define TR_MIN_BLOCKS_SRC 6      // source pass (birth + locate + first step)
+#endif
 #ifndef TR_MIN_BLOCKS_BOX
 #define TR_MIN_BLOCKS_BOX 6      // box-only fp32 step pass: 80 registers (no spills), 24 warps / SM
 #endif
@@ -272,7 +275,7 @@ __device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R
 // photon birth (C8, Algorithm 1 steps 1-2), out of line: source sampling, energy factors, first optical depth
 template <class R> struct BirthIO { R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k; uint32_t j; int above; };
 template <class R>
-__device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, const EnergyFactors<R>* mono, uint64_t seed, uint64_t id) {
+__device__ __forceinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, const EnergyFactors<R>* mono, uint64_t seed, uint64_t id) {
     PhiloxStream rng; rng.init(seed, id, 0);
     V3<R> x, w; R E;
     sample_source(*src, rng, x, w, E);
@@ -288,7 +291,7 @@ __device__ __noinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, cons
 // back of the output queue; interact_pass handles them before the next pass.  PHYS = true: interactions happen inside
 // the pass (batched per warp); used for the last pass, which runs the few remaining photons to completion.
 template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
-__global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS && !FROM_SOURCE) ? (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX) : 1)
+__global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS) ? (FROM_SOURCE ? TR_MIN_BLOCKS_SRC : (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX)) : 1)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
                double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct) {

@@ -8,7 +8,7 @@ namespace gn {
 
 // ---- counter-based RNG (C7): key = seed, counter = (photon id lo, hi, block, 0); draw j = 64-bit lane j&1 of block j>>1
 // One copy of the ten rounds, out of line: draws happen only at interactions (rare next to navigation steps).
-__device__ __noinline__ uint64_t philox_lane(uint32_t k0, uint32_t k1, uint32_t id0, uint32_t id1, uint32_t j) {
+__device__ __forceinline__ uint64_t philox_lane(uint32_t k0, uint32_t k1, uint32_t id0, uint32_t id1, uint32_t j) {
     uint32_t c0 = id0, c1 = id1, c2 = j >> 1, c3 = 0, a = k0, b = k1;
 #pragma unroll 1
     for (int r = 0; r < 10; ++r) {
