@@ -70,15 +70,72 @@ __global__ void __launch_bounds__(NAV_THREADS) locate_kernel(GeoView<R> g, const
     }
 }
 
+// Sort of the navigation queries by volume key (SURVEY 8(a) A10 applied to A11): queries arrive in arbitrary order, so in
+// a geometry with mixed solids the lanes of a warp would do different things (world: box exit + scan of the barrels;
+// sector: tube exit; ...).  Two small kernels build a work order -- a counting sort of the query indices by key = (solid
+// type of the current volume, has daughters) -- and step_kernel runs through it; outputs go back to the original slots.
+// Which query lands where inside its key's segment depends on block scheduling; the results do not.
+constexpr int SORT_KEYS = 9;              // 4 solid types x {leaf, mother} + "no volume"
+constexpr int SORT_TILE = 1024;
+template <class R>
+__global__ void __launch_bounds__(NAV_THREADS) sort_keys_kernel(GeoView<R> g, const int32_t* __restrict__ vol_in, int64_t n,
+                                                                uint8_t* __restrict__ keys, unsigned long long* __restrict__ totals) {
+    __shared__ unsigned sh[SORT_KEYS];
+    if (threadIdx.x < SORT_KEYS) sh[threadIdx.x] = 0;
+    __syncthreads();
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int v = vol_in[i];
+        int key = SORT_KEYS - 1;
+        if (v >= 0 && v < g.n_nodes) {
+            const int4 h = __ldg(reinterpret_cast<const int4*>(g.node + v));          // {parent, info, mat, ndau}
+            key = 2 * __ldg(&g.solids[h.y & NODE_SOLID_MASK].type) + (h.w > 0 ? 1 : 0);
+        }
+        keys[i] = (uint8_t)key;
+        atomicAdd(&sh[key], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x < SORT_KEYS && sh[threadIdx.x]) atomicAdd(&totals[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
+}
+__global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const uint8_t* __restrict__ keys, int64_t n, const unsigned long long* __restrict__ totals,
+                                                                   unsigned long long* __restrict__ cursors, uint32_t* __restrict__ perm) {
+    __shared__ unsigned sh_cnt[SORT_KEYS];
+    __shared__ unsigned long long sh_base[SORT_KEYS];
+    const int64_t n_tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        if (threadIdx.x < SORT_KEYS) sh_cnt[threadIdx.x] = 0;
+        __syncthreads();
+        int key[SORT_TILE / NAV_THREADS]; unsigned rank[SORT_TILE / NAV_THREADS];
+#pragma unroll
+        for (int q = 0; q < SORT_TILE / NAV_THREADS; ++q) {
+            const int64_t i = tile * SORT_TILE + q * NAV_THREADS + threadIdx.x;
+            key[q] = i < n ? keys[i] : -1;
+            rank[q] = key[q] >= 0 ? atomicAdd(&sh_cnt[key[q]], 1u) : 0u;
+        }
+        __syncthreads();
+        if (threadIdx.x < SORT_KEYS) {
+            unsigned long long seg = 0;                                        // start of this key's segment
+            for (int k = 0; k < (int)threadIdx.x; ++k) seg += totals[k];
+            sh_base[threadIdx.x] = seg + (sh_cnt[threadIdx.x] ? atomicAdd(&cursors[threadIdx.x], (unsigned long long)sh_cnt[threadIdx.x]) : 0ull);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < SORT_TILE / NAV_THREADS; ++q)
+            if (key[q] >= 0) perm[sh_base[key[q]] + rank[q]] = (uint32_t)(tile * SORT_TILE + q * NAV_THREADS + threadIdx.x);
+        __syncthreads();
+    }
+}
+
 template <class R, bool FLAT>
 __global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                            const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
-                                                           int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out) {
+                                                           int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out,
+                                                           const uint32_t* __restrict__ perm) {
     __shared__ BlockTables<R> tab;
     stage_tables(g, tab);
     __syncthreads();
     Navigator<R, true, FLAT> nav(g, &tab.ctx);
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = perm ? (int64_t)perm[t] : t;                     // work order: queries grouped by volume key (sort_queries)
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
         int vol = vol_in[i];
@@ -576,9 +633,29 @@ template <class R> int locate_impl(const gn_geometry* geo, const void* pos, cons
 template <class R> int step_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
                                  int64_t n, void* step, int32_t* next, cudaStream_t s) {
     if (n == 0) return GN_OK;
-    if (geo->coherent) step_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next);
-    else step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next);
-    GN_CUDA(cudaGetLastError(), "gn_nav_compute_step launch");
+    if (geo->coherent) {
+        step_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, nullptr);
+        GN_CUDA(cudaGetLastError(), "gn_nav_compute_step launch");
+        return GN_OK;
+    }
+    // general geometry: group the queries by volume key first (large batches only; stream-ordered scratch)
+    uint32_t* perm = nullptr;
+    char* scratch = nullptr;
+    if (n >= (1 << 16) && n < (1ll << 32)) {
+        const size_t bytes = 256 + (size_t)n + 4 * (size_t)n + 64;
+        if (cudaMallocAsync((void**)&scratch, bytes, s) == cudaSuccess) {
+            unsigned long long* totals = (unsigned long long*)scratch; unsigned long long* cursors = totals + 16;
+            uint8_t* keys = (uint8_t*)(scratch + 256);
+            perm = (uint32_t*)(scratch + 256 + (((size_t)n + 63) & ~(size_t)63));
+            cudaMemsetAsync(scratch, 0, 256, s);
+            sort_keys_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), vol, n, keys, totals);
+            sort_scatter_kernel<<<nav_grid((n + 3) / 4), NAV_THREADS, 0, s>>>(keys, n, totals, cursors, perm);
+        } else { cudaGetLastError(); scratch = nullptr; }                     // no scratch: run in arrival order
+    }
+    step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, perm);
+    cudaError_t e = cudaGetLastError();
+    if (scratch) cudaFreeAsync(scratch, s);
+    GN_CUDA(e, "gn_nav_compute_step launch");
     return GN_OK;
 }
 
