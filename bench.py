@@ -322,7 +322,7 @@ def run_ours(args):
             B.nav_locate(geo, pos, dirs, out=vol)
             B.nav_compute_step(geo, pos, dirs, vol, out=out)
             ev[1].record(); ev[1].synchronize()
-            return n, 2, ev[0].elapsed_time(ev[1])
+            return n, 4, ev[0].elapsed_time(ev[1])      # locate_kernel, sort_keys_kernel, sort_scatter_kernel, step_kernel
 
     def barrier():
         if world > 1:
@@ -402,7 +402,7 @@ def run_ours(args):
                 traffic = None
         roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
                     "traffic": traffic, "peak_source": peak_src,
-                    "kernel": "transport_pass<R,0,0,0> (lean wavefront step pass)" if transport else "locate_kernel+step_kernel",
+                    "kernel": "transport_pass<R,0,0,0> (lean wavefront step pass)" if transport else "locate_kernel + query sort + step_kernel",
                     "algorithmic_bytes_per_unit": abytes,
                     "kernel_steps_per_run": dom[0] / args.steps if transport else None, "kernel_ms_per_run": dom[1] / args.steps if transport else kernel_ms / args.steps,
                     "whole_run": {"achieved": whole, "frac": (whole / peak) if whole else None, "ms_per_run": kernel_ms / args.steps,

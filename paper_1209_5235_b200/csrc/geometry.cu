@@ -190,6 +190,16 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     { int acc = 0; for (size_t i = 0; i < V; ++i) { kids[i] = make_int2(acc, 0); acc += kid_count[i]; } }
     for (size_t i = 1; i < V; ++i) { int p = node[i].x; dlist[kids[p].x + kids[p].y] = (int)i; kids[p].y++; }
 
+    {
+        // the library's stream-ordered scratch (query sort) comes from the device's default memory pool: keep freed blocks
+        // in the pool instead of returning them to the driver at every synchronisation
+        cudaMemPool_t pool = nullptr; int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
+    }
     gn_geometry* geo = new gn_geometry();
     geo->n_places = n_places; geo->n_solids = n_solids; geo->n_mats = n_mats;
     cudaGetDevice(&geo->device);
