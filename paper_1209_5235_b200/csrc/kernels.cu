@@ -97,9 +97,11 @@ __global__ void __launch_bounds__(NAV_THREADS) sort_keys_kernel(GeoView<R> g, co
     if (threadIdx.x < SORT_KEYS && sh[threadIdx.x]) atomicAdd(&totals[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
 }
 __global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const uint8_t* __restrict__ keys, int64_t n, const unsigned long long* __restrict__ totals,
-                                                                   unsigned long long* __restrict__ cursors, uint32_t* __restrict__ perm) {
+                                                                   unsigned long long* __restrict__ cursors, uint32_t* __restrict__ perm,
+                                                                   const unsigned* __restrict__ n_ptr) {
     __shared__ unsigned sh_cnt[SORT_KEYS];
     __shared__ unsigned long long sh_base[SORT_KEYS];
+    if (n_ptr) n = (int64_t)*n_ptr;                                          // count known only on the device (transport passes)
     const int64_t n_tiles = (n + SORT_TILE - 1) / SORT_TILE;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         if (threadIdx.x < SORT_KEYS) sh_cnt[threadIdx.x] = 0;
@@ -240,6 +242,10 @@ struct DevStats {
 };
 // survivors of a pass: key-0 photons fill the output queue from the front, key-1 photons from the back
 struct PassCounters { unsigned front, back; };
+// general geometries: the travelling survivors of a pass are also counted by volume key, and a small kernel turns the
+// keys into the work order of the next pass (sort_scatter_kernel), so that its warps are mostly of one kind
+struct KeyCounters { unsigned long long tot[SORT_KEYS], cur[SORT_KEYS]; unsigned long long pad[2]; };
+struct SortIO { KeyCounters* kout; uint8_t* keys_out; const uint32_t* perm_in; };
 
 // one photon in the queue; sizeof = 64 (float) / 112 (double), moved as 16-byte words
 template <class R> struct alignas(16) PhotonRec {
@@ -351,7 +357,7 @@ template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
 __global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS) ? (FROM_SOURCE ? TR_MIN_BLOCKS_SRC : (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX)) : 1)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
-               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct) {
+               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio) {
     // input: pass 0 generates n_src photons; later passes read the survivors of the previous pass, whose count is
     // known only on the device (front + back of cin)
     unsigned n_front = n_src, n_in = n_src;
@@ -366,6 +372,8 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     __shared__ unsigned sh_base[2];
     __shared__ unsigned long long sh_cnt[8];
     __shared__ double sh_en[4];
+    __shared__ unsigned sh_key[SORT_KEYS];
+    if (threadIdx.x < SORT_KEYS) sh_key[threadIdx.x] = 0;
     stage_tables(g, tab);
     const MatRec<R>* mats = g.mats;
     if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
@@ -403,7 +411,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         c_phot = warp_sum(c_phot); e_src = warp_sum(e_src);
         if (lane == 0) { atomicAdd(&sh_cnt[ST_PHOTONS], (unsigned long long)c_phot); atomicAdd(&sh_en[EN_SOURCE], e_src); }
     } else if (fate == FATE_ALIVE) {
-        PhotonRec<R> r; load_rec(qin, i < n_front ? i : cap - 1u - (i - n_front), r);
+        PhotonRec<R> r; load_rec(qin, i < n_front ? ((FLAT && sio.perm_in) ? sio.perm_in[i] : i) : cap - 1u - (i - n_front), r);
         if (r.vol < 0) fate = FATE_NONE;                 // absorbed by interact_pass
         x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
         gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = (int)(r.tail[0] & 1u); pending = (r.tail[0] & 2u) != 0;
@@ -519,6 +527,11 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         r.tail[0] = (uint32_t)above | (pending ? 2u : 0u);
         store_rec(qout, o, r);
         if (TRACK) pp.hash[idx] = h;
+        if (FLAT && sio.keys_out && !key1) {                                 // volume key of a travelling survivor
+            const int key = 2 * nav.solid_of(nd).type + (nd.ndau > 0 ? 1 : 0);
+            sio.keys_out[o] = (uint8_t)key;
+            atomicAdd(&sh_key[key], 1u);
+        }
     }
     // ---- statistics: warp tree, shared atomics, one global atomic per counter per block -----------------------
     {
@@ -538,6 +551,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
     if (!FROM_SOURCE && !PHYS && threadIdx.x == 12 && sh_cnt[ST_STEPS]) atomicAdd(&stats->lean_steps, sh_cnt[ST_STEPS]);
+    if (FLAT && sio.kout && threadIdx.x >= 32 && threadIdx.x < 32 + SORT_KEYS && sh_key[threadIdx.x - 32]) atomicAdd(&sio.kout->tot[threadIdx.x - 32], (unsigned long long)sh_key[threadIdx.x - 32]);
 }
 
 // The interaction wavefront (A6-A9): every photon parked at an interaction point by the previous pass sits in the
@@ -649,7 +663,7 @@ template <class R> int step_impl(const gn_geometry* geo, const void* pos, const 
             perm = (uint32_t*)(scratch + 256 + (((size_t)n + 63) & ~(size_t)63));
             cudaMemsetAsync(scratch, 0, 256, s);
             sort_keys_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), vol, n, keys, totals);
-            sort_scatter_kernel<<<nav_grid((n + 3) / 4), NAV_THREADS, 0, s>>>(keys, n, totals, cursors, perm);
+            sort_scatter_kernel<<<nav_grid((n + 3) / 4), NAV_THREADS, 0, s>>>(keys, n, totals, cursors, perm, nullptr);
         } else { cudaGetLastError(); scratch = nullptr; }                     // no scratch: run in arrival order
     }
     step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, perm);
@@ -693,9 +707,9 @@ constexpr int TR_TIMED = 24;                // lean step passes per batch timed 
 template <class R, bool SRC, bool PHYS, bool FLAT>
 static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
                         uint32_t n_src, const PassCounters* cin, PassCounters* cout, const PhotonRec<R>* qin, PhotonRec<R>* qout, uint32_t cap,
-                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct) {
-    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct);
-    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct);
+                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio = SortIO{nullptr, nullptr, nullptr}) {
+    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio);
+    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio);
 }
 template <class R>
 static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, uint64_t seed, uint64_t first_id, const PassCounters* cin,
@@ -716,7 +730,10 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     const size_t qb = cap * sizeof(PhotonRec<R>);
     const size_t hb = (track && !d_hash) ? cap * 8 : 0;       // the hash array doubles as per-photon state between passes
     const size_t cb = sizeof(PassCounters) * (TR_MAX_PASSES + 2);
-    const size_t need = 2 * qb + hb + 512 + cb;
+    const bool sorted = !geo->coherent;                        // general geometries: work order of every pass sorted by volume key
+    const size_t kb = sorted ? sizeof(KeyCounters) * (TR_MAX_PASSES + 2) : 0;
+    const size_t sb = sorted ? ((cap + 255) & ~(size_t)255) + 4 * cap : 0;      // keys + perm
+    const size_t need = 2 * qb + hb + 512 + cb + kb + sb;
     std::lock_guard<std::mutex> lock(geo->ws_mutex);          // one run at a time per handle: the workspace is shared
     GN_CUDA(cudaMemsetAsync(d_edep, 0, sizeof(double) * (size_t)geo->n_places, s), "gn_transport_run memset edep");
     if (geo->ws_bytes < need) {
@@ -739,6 +756,9 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     DevStats* d_stats = (DevStats*)(scratch + 2 * qb + hb);
     PassCounters* d_ctr = (PassCounters*)(scratch + 2 * qb + hb + 512);
     PassCounters* h_ctr = (PassCounters*)geo->ws_pinned;
+    KeyCounters* d_kctr = sorted ? (KeyCounters*)(scratch + 2 * qb + hb + 512 + cb) : nullptr;
+    uint8_t* d_keys = sorted ? (uint8_t*)(scratch + 2 * qb + hb + 512 + cb + kb) : nullptr;
+    uint32_t* d_perm = sorted ? (uint32_t*)(scratch + 2 * qb + hb + 512 + cb + kb + ((cap + 255) & ~(size_t)255)) : nullptr;
     int rc = GN_OK;
     uint64_t passes = 0, launches = 0;
     cudaEvent_t ev0 = geo->ws_events[0], ev1 = geo->ws_events[1];
@@ -756,6 +776,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         PerPhotonOut pp{d_hash ? d_hash + done : tmp_hash, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
         PhotonRec<R>* in = qb_; PhotonRec<R>* out = qa;
         cudaMemsetAsync(d_ctr, 0, cb, s);
+        if (sorted) cudaMemsetAsync(d_kctr, 0, kb, s);
         cudaEventRecord(ev0, s);
         // pass p reads counter p and adds to counter p + 1; the host enqueues passes back to back and learns the
         // survivor counts TR_LAG passes late (upper bound for the grid; blocks past the true count return at once)
@@ -774,18 +795,22 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             // FLAT = general geometry (any solid, rotations, long candidate lists); !FLAT = unrotated boxes only (geo->coherent)
             if (p == 0) {
                 if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
-                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
+                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup, SortIO{d_kctr + 1, d_keys, nullptr});
             } else if (last) {
                 if (geo->coherent) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
-                else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
+                else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, SortIO{nullptr, nullptr, d_perm});
             }
             else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
                 launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp);
                 if (n_timed < TR_TIMED) cudaEventRecord(tev[2 * n_timed], s);
                 if (geo->coherent) launch_pass<R, false, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup);
-                else launch_pass<R, false, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup);
+                else launch_pass<R, false, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, SortIO{d_kctr + p + 1, d_keys, d_perm});
                 if (n_timed < TR_TIMED) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
+                ++launches;
+            }
+            if (sorted && !last) {                                           // work order of the next pass: travelling survivors by volume key
+                sort_scatter_kernel<<<nav_grid(((int64_t)ub + 3) / 4), NAV_THREADS, 0, s>>>(d_keys, 0, d_kctr[p + 1].tot, d_kctr[p + 1].cur, d_perm, &d_ctr[p + 1].front);
                 ++launches;
             }
             ++passes; ++launches;
