@@ -295,6 +295,8 @@ def run_ours(args):
         gopts["tail_photons"] = args.tail_photons
     if args.first_pass_steps:
         gopts["first_pass_steps"] = args.first_pass_steps
+    if args.regroup_percent:
+        gopts["regroup_percent"] = args.regroup_percent
     geo = B.Geometry(wl.geometry, **gopts)
     transport = wl.source is not None
     dom = [0, 0.0]                                            # dominant kernel: steps taken in / summed duration of the lean step passes
@@ -448,6 +450,7 @@ def main():
     ap.add_argument("--steps-per-pass", type=int, default=0)
     ap.add_argument("--tail-photons", type=int, default=0, help="diagnostics: override gn_opts.tail_photons")
     ap.add_argument("--first-pass-steps", type=int, default=0, help="diagnostics: override gn_opts.first_pass_steps")
+    ap.add_argument("--regroup-percent", type=int, default=0, help="diagnostics: override gn_opts.regroup_percent")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-all-cores", action="store_true")
     ap.add_argument("--allow-short-warmup", action="store_true")
