@@ -283,21 +283,28 @@ template <class T> __device__ __forceinline__ T warp_sum(T v) {
 
 // warp-aggregated tally: one fp64 atomic per distinct volume per warp
 __device__ __noinline__ void warp_tally(double* __restrict__ edep, double* sh_dep_total, int vol, double dep, bool has) {
-    unsigned pending = __ballot_sync(0xffffffffu, has);
     const int lane = threadIdx.x & 31;
+    {   // book-keeping total: one shared atomic per warp
+        double tot = has ? dep : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+        if (lane == 0 && tot != 0.0) atomicAdd(sh_dep_total, tot);
+    }
+    // lanes whose volume no other lane of the warp deposits in add directly; the rest are summed per distinct volume
+    const unsigned grp = __match_any_sync(0xffffffffu, has ? vol : ~lane);
+    const bool alone = grp == (1u << lane);
+    if (has && alone) atomicAdd(&edep[vol], dep);
+    unsigned pending = __ballot_sync(0xffffffffu, has && !alone);
     while (pending) {
         int leader = __ffs(pending) - 1;
         int v = __shfl_sync(0xffffffffu, vol, leader);
         bool same = has && vol == v;
-        unsigned grp = __ballot_sync(0xffffffffu, same);
-        double s = dep;
-        if (grp != (1u << leader)) {
-            s = same ? dep : 0.0;
+        unsigned g2 = __ballot_sync(0xffffffffu, same);
+        double s = same ? dep : 0.0;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        }
-        if (lane == leader) { atomicAdd(&edep[v], s); atomicAdd(sh_dep_total, s); }
-        pending &= ~grp;
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == leader) atomicAdd(&edep[v], s);
+        pending &= ~g2;
     }
 }
 

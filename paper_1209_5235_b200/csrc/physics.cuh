@@ -8,9 +8,10 @@ namespace gn {
 
 // ---- counter-based RNG (C7): key = seed, counter = (photon id lo, hi, block, 0); draw j = 64-bit lane j&1 of block j>>1
 // One copy of the ten rounds, out of line: draws happen only at interactions (rare next to navigation steps).
-__device__ __forceinline__ uint64_t philox_lane(uint32_t k0, uint32_t k1, uint32_t id0, uint32_t id1, uint32_t j) {
-    uint32_t c0 = id0, c1 = id1, c2 = j >> 1, c3 = 0, a = k0, b = k1;
-#pragma unroll 1
+// the ten rounds of one block: counter (id0, id1, blk, 0) under key (k0, k1) -> two 64-bit lanes
+__device__ __forceinline__ void philox_block(uint32_t k0, uint32_t k1, uint32_t id0, uint32_t id1, uint32_t blk, uint64_t& l0, uint64_t& l1) {
+    uint32_t c0 = id0, c1 = id1, c2 = blk, c3 = 0, a = k0, b = k1;
+#pragma unroll
     for (int r = 0; r < 10; ++r) {
         uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
         uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
@@ -18,14 +19,27 @@ __device__ __forceinline__ uint64_t philox_lane(uint32_t k0, uint32_t k1, uint32
         c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
         a += 0x9E3779B9u; b += 0xBB67AE85u;
     }
-    return (j & 1) ? ((uint64_t)c2 | ((uint64_t)c3 << 32)) : ((uint64_t)c0 | ((uint64_t)c1 << 32));
+    l0 = (uint64_t)c0 | ((uint64_t)c1 << 32);
+    l1 = (uint64_t)c2 | ((uint64_t)c3 << 32);
 }
+// draw j = lane (j & 1) of block j >> 1; the second lane of a block is kept for the next draw
 struct PhiloxStream {
     uint32_t k0, k1, id0, id1, j;
+    uint64_t spare; bool have_spare;
     __device__ __forceinline__ void init(uint64_t seed, uint64_t id, uint32_t draws_done) {
         k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32); id0 = (uint32_t)id; id1 = (uint32_t)(id >> 32); j = draws_done;
+        spare = 0; have_spare = false;
     }
-    __device__ __forceinline__ uint64_t next() { uint64_t out = philox_lane(k0, k1, id0, id1, j); ++j; return out; }
+    __device__ __forceinline__ uint64_t next() {
+        uint64_t out;
+        if ((j & 1u) && have_spare) { out = spare; have_spare = false; }
+        else {
+            uint64_t l0, l1; philox_block(k0, k1, id0, id1, j >> 1, l0, l1);
+            if (j & 1u) out = l1; else { out = l0; spare = l1; have_spare = true; }
+        }
+        ++j;
+        return out;
+    }
 };
 // uniforms in (0, 1] as Algorithm 1 step 1 requires
 __device__ __forceinline__ float to_uniform(uint64_t lane, float) { return (float)((uint32_t)(lane >> 40) + 1u) * 5.9604644775390625e-08f; }
