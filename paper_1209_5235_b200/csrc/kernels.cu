@@ -31,6 +31,9 @@
 namespace gn {
 
 constexpr int NAV_THREADS = 256;
+#ifndef NAV_STEP_MIN_BLOCKS
+#define NAV_STEP_MIN_BLOCKS 8      // ComputeStep kernels are latency-bound at ~10 of 32 lanes: full occupancy (32 registers, spills) wins
+#endif
 constexpr int MAX_SMEM_SOLIDS = 32;
 constexpr int MAX_SMEM_GRIDS = 8;
 constexpr int MAX_SMEM_MATS = 32;
@@ -128,7 +131,7 @@ __global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const uint8_t
 }
 
 template <class R, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLOCKS : 3) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                            const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
                                                            int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out,
                                                            const uint32_t* __restrict__ perm) {
