@@ -31,6 +31,9 @@
 namespace gn {
 
 constexpr int NAV_THREADS = 256;
+#ifndef NAV_LOCATE_MIN_BLOCKS
+#define NAV_LOCATE_MIN_BLOCKS 8
+#endif
 #ifndef NAV_STEP_MIN_BLOCKS
 #define NAV_STEP_MIN_BLOCKS 8      // ComputeStep kernels are latency-bound at ~10 of 32 lanes: full occupancy (32 registers, spills) wins
 #endif
@@ -58,7 +61,7 @@ template <class R> __device__ __forceinline__ void stage_tables(const GeoView<R>
 // navigation kernels: pure maps over queries
 // -------------------------------------------------------------------------------------------------------
 template <class R, bool HAS_DIR, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : 3) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                              int64_t n, int32_t* __restrict__ vol_out) {
     __shared__ BlockTables<R> tab;
     stage_tables(g, tab);
