@@ -313,6 +313,68 @@ def mixed_solids_geometry(n=4, seed=9, pitch=100.0) -> Geometry:
     return b.finish()
 
 
+def cms_like_geometry(seed=13, n_rings=8, n_phi=16) -> Geometry:
+    """A synthetic collider-detector hierarchy, six levels deep, of all four solid types (the paper's second test geometry is
+    the CMS detector; that model is not available, SURVEY 8(f) NEXT-2 asks for a "deeper CMS-like synthetic
+    hierarchy").  world box -> { beam pipe, tracker tube with silicon layers, ECAL barrel -> z rings -> phi sectors -> rotated
+    crystal boxes -> rotated cones -> balls; HCAL barrel -> phi sectors -> radial layers; two end-cap cones (one flipped) with
+    a ring and a ball each; twelve rotated muon boxes with layer boxes and a transverse drift tube }.  Daughters lie strictly
+    inside their mothers and siblings do not overlap (checked against the brute-force locate in tests/)."""
+    rng = np.random.default_rng(seed)
+    b = _Builder(f"cmslike_{n_rings}x{n_phi}")
+    world = b.place(-1, b.box(3000, 3000, 3000), "air")
+    b.place(world, b.tube(0.0, 30.0, 2700.0), "vacuum")                                  # beam pipe
+    tracker = b.place(world, b.tube(40.0, 1100.0, 2700.0), "air")
+    for r in (100.0, 250.0, 400.0, 600.0, 800.0, 1000.0):
+        b.place(tracker, b.tube(r, r + 4.0, 2600.0), "silicon")
+    # ECAL: barrel -> rings -> sectors -> crystal -> cone -> ball
+    ecal = b.place(world, b.tube(1200.0, 1500.0, 2700.0), "air")
+    hz_r = 2700.0 / n_rings
+    dphi = 2 * math.pi / n_phi
+    ring_solid = b.tube(1205.0, 1495.0, hz_r - 2.0)
+    sector_solid = b.tube(1210.0, 1490.0, hz_r - 4.0, -dphi / 2 + 0.004, dphi - 0.008)
+    crystal = b.box(110.0, min(150.0, 1220.0 * math.tan(dphi / 2 - 0.01) - 5.0), min(200.0, hz_r - 10.0))
+    cone = b.cone(20.0, 60.0, 80.0)
+    ball = b.orb(25.0)
+    for iz in range(n_rings):
+        ring = b.place(ecal, ring_solid, "air", T=(0, 0, -2700.0 + hz_r * (2 * iz + 1)))
+        for j in range(n_phi):
+            sec = b.place(ring, sector_solid, "scint", R=rot_z(j * dphi))
+            cr = b.place(sec, crystal, "lead", R=rot_z(rng.uniform(-0.05, 0.05)), T=(1350.0, 0, 0))
+            co = b.place(cr, cone, "iron", R=random_rotation(rng))
+            b.place(co, ball, "silicon", T=(0, 0, 10.0))
+    # HCAL: barrel -> sectors -> radial layers (tube sectors of the same opening, inset)
+    hcal = b.place(world, b.tube(1600.0, 2400.0, 2700.0), "air")
+    n_h = 12
+    dph = 2 * math.pi / n_h
+    hsec = b.tube(1605.0, 2395.0, 2690.0, -dph / 2 + 0.003, dph - 0.006)
+    layers = [b.tube(r, r + 150.0, 2680.0, -dph / 2 + 0.006, dph - 0.012) for r in (1620.0, 1820.0, 2020.0, 2220.0)]
+    for j in range(n_h):
+        s = b.place(hcal, hsec, "scint", R=rot_z(j * dph))
+        for k, lay in enumerate(layers):
+            b.place(s, lay, "iron" if k % 2 == 0 else "lead")
+    # end caps: frustums opening away from the centre, the one at -z flipped about x
+    cap = b.cone(400.0, 1500.0, 120.0)
+    flip = np.array([[1.0, 0.0, 0.0], [0.0, -1.0, 0.0], [0.0, 0.0, -1.0]])
+    ring_in_cap = b.tube(150.0, 350.0, 100.0)
+    for sgn, Rm in ((1.0, None), (-1.0, flip)):
+        c = b.place(world, cap, "iron", R=Rm, T=(0, 0, sgn * 2850.0))
+        b.place(c, ring_in_cap, "lead")
+        b.place(c, b.orb(40.0), "silicon", T=(0.0, 0.0, -50.0))
+    # muon chambers: boxes around the barrel, rotated about z; three layer boxes and a drift tube across each
+    chamber = b.box(100.0, 500.0, 2500.0)
+    layer = b.box(15.0, 480.0, 2400.0)
+    drift = b.tube(0.0, 12.0, 450.0)
+    rot_x90 = np.array([[1.0, 0.0, 0.0], [0.0, 0.0, -1.0], [0.0, 1.0, 0.0]])         # tube axis along the chamber's y
+    for j in range(12):
+        a = j * math.pi / 6 + 0.02
+        ch = b.place(world, chamber, "air", R=rot_z(a), T=(2700.0 * math.cos(a), 2700.0 * math.sin(a), 0.0))
+        for x in (-70.0, -20.0, 30.0):
+            b.place(ch, layer, "aluminium", T=(x, 0, 0))
+        b.place(ch, drift, "air", R=rot_x90, T=(80.0, 0.0, 2450.0 * rng.uniform(-1, 1)))
+    return b.finish()
+
+
 # ----------------------------------------------------------------------------------------------
 # ---- the paper's own benchmark inputs (PAPER.md section 3.5, L152-160) ----------------------------
 MU_MASS_AL_1MEV = 0.06146       # cm^2/g, PAPER.md L150

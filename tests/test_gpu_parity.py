@@ -42,7 +42,21 @@ GEOMS = {
     "detector": lambda: W.detector_geometry(seed=4, n_phi=16, n_z=8, barrels=((200, 400), (450, 650))),
     "lattice": lambda: W.lattice_geometry(4, seed=7),
     "mixed": lambda: W.mixed_solids_geometry(),          # boxes, tubes, cones, balls, rotated, nested balls
+    "cmslike": lambda: W.cms_like_geometry(),            # six-level detector hierarchy of all four solids (8(f) NEXT-2)
 }
+
+
+def deep_centres(geom, nodes):
+    """Global positions of the origins of `nodes` (composition of the placement translations / rotations, test-side numpy)."""
+    out = []
+    for i in nodes:
+        x = np.zeros(3)
+        while i > 0:
+            tr = geom.transforms[geom.placements[i, 3]]
+            x = tr[:9].reshape(3, 3) @ x + tr[9:]
+            i = geom.placements[i, 0]
+        out.append(x)
+    return np.array(out)
 
 
 def query_points(geom, rng, n):
@@ -53,6 +67,12 @@ def query_points(geom, rng, n):
     c = geom.transforms[int(geom.placements[1, 3]), 9:]
     if geom.name.startswith("lattice") or geom.name.startswith("mixed"):
         ext, c = h * 0.9, np.zeros(3)
+    if geom.name.startswith("cmslike"):                 # half of the points around the deepest branch (crystal / cone / ball)
+        deep = np.nonzero(geom.solid_type[geom.placements[:, 1]] == 3)[0]
+        deep = deep[geom.placements[deep, 0] > 0]       # the cones inside the crystals (the end caps hang off the world)
+        cg = deep_centres(geom, deep)
+        p[: n // 2] = cg[rng.integers(0, len(cg), n // 2)] + rng.normal(size=(n // 2, 3)) * 60.0
+        return p
     p[: n // 2] = c + rng.uniform(-1, 1, size=(n // 2, 3)) * ext * 1.05
     if geom.name.startswith("config3"):                 # points exactly on voxel faces / edges / corners
         k = n // 8
@@ -203,6 +223,7 @@ TRANSPORT_CASES = {
     "phantom16": lambda: (W.phantom_geometry(16, 2.0, 3), W.phantom_source(16, half_angle_deg=0.8), 20000, 3),
     "detector": lambda: (W.detector_geometry(seed=4, n_phi=16, n_z=8, barrels=((200, 400), (450, 650))), W.detector_source(), 20000, 4),
     "lattice": lambda: (W.lattice_geometry(4, seed=7), W.Source(W.SRC_ISOTROPIC, (3.0, 2.0, 1.0), (0, 0, 1.0), W.E_LOGUNIFORM, 0.05, 20.0), 20000, 5),
+    "cmslike": lambda: (W.cms_like_geometry(), W.Source(W.SRC_ISOTROPIC, (0.0, 0.0, 0.0), (0, 0, 1.0), W.E_LOGUNIFORM, 0.1, 1000.0), 20000, 6),
 }
 
 
