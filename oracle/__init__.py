@@ -18,7 +18,7 @@ _lib = None
 
 class Opts(C.Structure):
     _fields_ = [("tol64", C.c_double), ("tol32", C.c_double), ("sigma_pe0", C.c_double), ("e_cut", C.c_double),
-                ("grid_min_daughters", C.c_int32), ("stuck_limit", C.c_int32)]
+                ("grid_min_daughters", C.c_int32), ("stuck_limit", C.c_int32), ("secondaries", C.c_int32), ("reserved", C.c_int32)]
 
 
 class CSource(C.Structure):
@@ -176,6 +176,13 @@ def sigma_pair(k, Z):
 
 def sigma_pe(E, Z, s0=1750.0):
     return lib().oracle_sigma_pe(float(E), float(Z), float(s0))
+
+
+def pair_directions(seed, first_id, n, precision=64):
+    """Directions of the two annihilation photons of photons first_id .. first_id + n - 1 (test hook)."""
+    w1 = np.empty((n, 3), np.float64); w2 = np.empty((n, 3), np.float64)
+    _check(lib().oracle_pair_directions(C.c_int(precision), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n), _p(w1), _p(w2)), "pair_directions")
+    return w1, w2
 
 
 def philox(counter, key):

@@ -81,7 +81,7 @@ struct Geo {
     std::vector<MaterialR<double>> m64; std::vector<MaterialR<float>> m32;
     std::vector<int> grid_of;                /* node -> index in grids or -1 */
     std::vector<Grid> grids;
-    double tol64, tol32, sigma_pe0, e_cut; int stuck_limit, grid_min;
+    double tol64, tol32, sigma_pe0, e_cut; int stuck_limit, grid_min, secondaries;
 };
 
 template <class R> struct Sel;
@@ -600,10 +600,10 @@ template <class R> R uniform_from_lane(uint64_t lane);
 template <> double uniform_from_lane<double>(uint64_t lane) { return (double)((lane >> 11) + 1) * 0x1p-53; }
 template <> float uniform_from_lane<float>(uint64_t lane) { return (float)((lane >> 40) + 1) * 0x1p-24f; }
 
-struct Stream {      /* draw j of photon id: lane (j mod 2) of block j/2 */
-    uint64_t seed, id; uint32_t j;
+struct Stream {      /* draw j of photon id: lane (j mod 2) of block j/2; tag 0 = the primary, 1 / 2 = its annihilation photons */
+    uint64_t seed, id; uint32_t j; uint32_t tag = 0;
     uint64_t lane() {
-        uint32_t c[4] = {(uint32_t)id, (uint32_t)(id >> 32), j >> 1, 0};
+        uint32_t c[4] = {(uint32_t)id, (uint32_t)(id >> 32), j >> 1, tag};
         philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
         uint64_t l = (j & 1) ? ((uint64_t)c[2] | ((uint64_t)c[3] << 32)) : ((uint64_t)c[0] | ((uint64_t)c[1] << 32));
         ++j;
@@ -709,15 +709,29 @@ inline void fnv_word(uint64_t& h, uint32_t w) {
 }
 enum { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
 
+/* One history from (x, w, E) with stream rng: locate, first optical depth, then the loop of Algorithm 1.
+ * Returns the history hash and the step count; E holds the energy at the end.  With g.secondaries (S:8(f) NEXT-3,
+ * D:reading 16) a pair event deposits E - 2 me c^2 and the two annihilation photons are followed right after the parent. */
+template <class R> struct History { uint64_t h; uint32_t ns; };
+
 template <class R>
-void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& src, uint64_t seed, uint64_t id,
-                      double* edep, oracle_stats_t& st, uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out) {
+void pair_directions(uint64_t seed, uint64_t id, R w1[3], R w2[3], Stream& s1) {
+    /* isotropic u from draws 0, 1 of stream (seed, id, tag 1): cos(theta) = 1 - 2 u0, phi = 2 pi u1; second photon exactly -u */
+    const R twopi = (R)6.283185307179586;
+    s1 = Stream{seed, id, 0, 1};
+    R u0 = s1.u<R>(), u1 = s1.u<R>();
+    R ct = (R)1 - (R)2 * u0;
+    R st = r_sqrt(r_max(((R)1 - ct) * ((R)1 + ct), (R)0));
+    R phi = twopi * u1;
+    w1[0] = st * std::cos(phi); w1[1] = st * std::sin(phi); w1[2] = ct;
+    for (int i = 0; i < 3; ++i) w2[i] = -w1[i];
+}
+
+template <class R>
+History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t id, Stream& rng, R x[3], R w[3], R& E,
+                 double* edep, oracle_stats_t& st) {
     const std::vector<MaterialR<R>>& mats = Sel<R>::m(g);
     const R twopi = (R)6.283185307179586;
-    Stream rng{seed, id, 0};
-    R x[3], w[3], E;
-    sample_source(src, rng, x, w, E);
-    st.n_photons++; st.e_source += (double)E;
     uint64_t h = 0xcbf29ce484222325ull; uint32_t ns = 0;
     int vol = nav.locate(x, w);
     bool alive = true;
@@ -725,6 +739,7 @@ void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& s
     R Y = 0; EnergyFactors<R> ef{};
     if (alive) { Y = -std::log(rng.u<R>()); ef = energy_factors(E); }           /* Alg.1 steps 1-2 */
     int zero_steps = 0;
+    bool annihilate = false;
     while (alive) {
         R mu3[3]; mu_partials(mats[g.material[vol]], ef, mu3);
         R mu = (mu3[0] + mu3[1]) + mu3[2];
@@ -750,8 +765,10 @@ void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& s
                 if (Ep < (R)g.e_cut) { dep = dep + Ep; st.n_cut++; ev = EV_CUT; alive = false; }
                 edep[vol] += (double)dep; st.e_deposited += (double)dep;
                 if (alive) { ef = energy_factors(E); Y = -std::log(rng.u<R>()); }
-            } else {                                                            /* pair: local deposit */
-                edep[vol] += (double)E; st.e_deposited += (double)E; st.n_pair++; ev = EV_PAIR; alive = false;
+            } else {                                                            /* pair */
+                R dep = g.secondaries ? E - (R)(2.0 * kMeC2) : E;               /* local deposit: all of E, or the pair's kinetic energy */
+                edep[vol] += (double)dep; st.e_deposited += (double)dep; st.n_pair++; ev = EV_PAIR; alive = false;
+                annihilate = g.secondaries != 0;
             }
         } else {                                                                /* boundary */
             len = step;
@@ -765,8 +782,31 @@ void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& s
         if (alive && zero_steps >= g.stuck_limit) { st.n_stuck++; st.e_stuck += (double)E; ev = EV_STUCK; alive = false; }
         fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
     }
-    if (hash_out) *hash_out = h;
-    if (nsteps_out) *nsteps_out = ns;
+    if (annihilate) {
+        /* positron at rest at the vertex x: two photons of me c^2, back to back; photon 1 carries on with stream tag 1
+         * (after the two direction draws), photon 2 starts stream tag 2.  Their hashes and step counts are added to the
+         * parent's (sums, so the order in which an implementation follows them does not matter). */
+        R w1[3], w2[3]; Stream s1{seed, id, 0, 1}, s2{seed, id, 0, 2};
+        pair_directions<R>(seed, id, w1, w2, s1);
+        R xa[3] = {x[0], x[1], x[2]}, xb[3] = {x[0], x[1], x[2]};
+        R Ea = (R)kMeC2, Eb = (R)kMeC2;
+        History<R> a = track<R>(g, nav, seed, id, s1, xa, w1, Ea, edep, st);
+        History<R> b = track<R>(g, nav, seed, id, s2, xb, w2, Eb, edep, st);
+        h += a.h + b.h; ns += a.ns + b.ns;
+    }
+    return History<R>{h, ns};
+}
+
+template <class R>
+void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& src, uint64_t seed, uint64_t id,
+                      double* edep, oracle_stats_t& st, uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out) {
+    Stream rng{seed, id, 0, 0};
+    R x[3], w[3], E;
+    sample_source(src, rng, x, w, E);
+    st.n_photons++; st.e_source += (double)E;
+    History<R> hs = track<R>(g, nav, seed, id, rng, x, w, E, edep, st);
+    if (hash_out) *hash_out = hs.h;
+    if (nsteps_out) *nsteps_out = hs.ns;
     if (efinal_out) *efinal_out = (double)E;
 }
 
@@ -1040,6 +1080,7 @@ int oracle_geometry_create(const double* materials, int32_t n_mats, const int32_
     g->e_cut = (opts && opts->e_cut > 0) ? opts->e_cut : 0.010;
     g->grid_min = (opts && opts->grid_min_daughters > 0) ? opts->grid_min_daughters : 8;
     g->stuck_limit = (opts && opts->stuck_limit > 0) ? opts->stuck_limit : 8;
+    g->secondaries = (opts && opts->secondaries > 0) ? 1 : 0;
     for (const SolidD& s : g->solids) { g->s64.push_back(round_solid<double>(s)); g->s32.push_back(round_solid<float>(s)); }
     for (const MaterialD& m : g->mats) { g->m64.push_back(round_material<double>(m, g->sigma_pe0)); g->m32.push_back(round_material<float>(m, g->sigma_pe0)); }
     g->grid_of.assign(n_places, -1);
@@ -1155,6 +1196,20 @@ double oracle_uniform_from_lane(uint64_t lane, int precision) {
 double oracle_draw(uint64_t seed, uint64_t id, uint32_t j, int precision) {
     Stream s{seed, id, j};
     return precision == 32 ? (double)s.u<float>() : s.u<double>();
+}
+
+int oracle_pair_directions(int precision, uint64_t seed, int64_t first_id, int64_t n, double* w1_out, double* w2_out) {
+    for (int64_t i = 0; i < n; ++i) {
+        Stream s1{seed, 0, 0, 0};
+        if (precision == 64) {
+            double a[3], b[3]; pair_directions<double>(seed, (uint64_t)(first_id + i), a, b, s1);
+            for (int k = 0; k < 3; ++k) { w1_out[3 * i + k] = a[k]; w2_out[3 * i + k] = b[k]; }
+        } else {
+            float a[3], b[3]; pair_directions<float>(seed, (uint64_t)(first_id + i), a, b, s1);
+            for (int k = 0; k < 3; ++k) { w1_out[3 * i + k] = a[k]; w2_out[3 * i + k] = b[k]; }
+        }
+    }
+    return ORACLE_OK;
 }
 
 int oracle_kn_sample(int precision, double E, uint64_t seed, int64_t first_id, int64_t n, double* eps_out, double* cost_out, int32_t* ntrials_out) {

@@ -34,6 +34,8 @@ typedef struct {
     double e_cut;        /* photon cut [MeV]; <=0 -> 0.010                                      (C6) */
     int32_t grid_min_daughters; /* mothers with >= this many daughters get a locate grid; <=0 -> 8 */
     int32_t stuck_limit; /* consecutive steps of length <= delta before a photon is killed; <=0 -> 8 (C9) */
+    int32_t secondaries; /* 1: a pair event deposits E - 2 me c^2 and two annihilation photons are followed (S:8(f) NEXT-3); 0: deposits E */
+    int32_t reserved;
 } oracle_opts_t;
 
 typedef struct {
@@ -102,6 +104,8 @@ double oracle_sigma_pair(double k, double Z);           /* cm^2 per atom */
 double oracle_sigma_pe(double E, double Z, double sigma_pe0_barn); /* cm^2 per atom */
 /* mu[3] = (mu_PE, mu_C, mu_pair) in 1/mm for material m at energy E, in the given precision */
 int oracle_mu(const void* geo, int precision, int32_t material, double E, double* mu3);
+/* directions of the two annihilation photons of photon id's pair event (S:8(f) NEXT-3): n x 3 doubles each */
+int oracle_pair_directions(int precision, uint64_t seed, int64_t first_id, int64_t n, double* w1_out, double* w2_out);
 void oracle_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t* out4);
 double oracle_uniform_from_lane(uint64_t lane, int precision);
 /* draw j (0-based) of photon id under seed, as a uniform in (0,1] */
