@@ -276,6 +276,27 @@ template <class R> __device__ __forceinline__ void store_rec(PhotonRec<R>* q, un
 
 struct PerPhotonOut { uint64_t* hash; uint32_t* nsteps; double* efinal; };
 
+// Secondary photons (reading 16).  A pair event of a primary appends its vertex to a list
+// (out / n_out); when the batch of primaries is done, the list is the source of a batch of 2 x n_pairs annihilation
+// photons (in): photon k belongs to pair k >> 1, runs on Philox stream tag 1 + (k & 1) of its parent's id, and adds its
+// history hash and step count to the parent's (sums: the order in which they finish does not matter).
+template <class R> struct alignas(16) PairVtx { R x, y, z; uint32_t idx; };
+template <class R> struct SecIO {
+    PairVtx<R>* out; unsigned* n_out;                          // primaries: where pair vertices go (nullptr = secondaries off)
+    const PairVtx<R>* in;                                      // secondaries: their parents' vertices (nullptr = a batch of primaries)
+    unsigned long long* parent_hash; uint32_t* parent_nsteps;  // secondaries, per-photon outputs wanted: the parents' slots
+};
+// per-photon outputs at the end of a history
+template <class R> __device__ __forceinline__ void history_out(const PerPhotonOut& pp, const SecIO<R>& sec, uint32_t idx, uint64_t h, uint32_t ns, R E) {
+    if (sec.in) {
+        const uint32_t parent = sec.in[idx >> 1].idx;
+        if (sec.parent_hash) atomicAdd(&sec.parent_hash[parent], (unsigned long long)h);
+        if (sec.parent_nsteps) atomicAdd(&sec.parent_nsteps[parent], ns);
+    } else {
+        pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = ns; if (pp.efinal) pp.efinal[idx] = (double)E;
+    }
+}
+
 __device__ __forceinline__ void fnv_word(uint64_t& h, uint32_t w) {
 #pragma unroll
     for (int i = 0; i < 4; ++i) { h ^= (w >> (8 * i)) & 0xffu; h *= 0x100000001b3ull; }
@@ -322,8 +343,8 @@ template <class R> struct InteractIO {
     uint32_t j; int above, ev;
 };
 template <class R>
-__device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R mu, R e_cut, uint64_t seed, uint64_t id) {
-    PhiloxStream rng; rng.init(seed, id, io->j);
+__device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R mu, R e_cut, uint64_t seed, uint64_t id, uint32_t tag, bool annihilate) {
+    PhiloxStream rng; rng.init(seed, id, io->j, tag);
     R E = io->E;
     R t = draw<R>(rng) * mu;
     if (t < muPE) { io->dep = E; io->ev = EV_PE; }
@@ -344,7 +365,7 @@ __device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R
             io->Y = -rlog(draw<R>(rng));
         }
         io->dep = dep;
-    } else { io->dep = E; io->ev = EV_PAIR; }
+    } else { io->dep = annihilate ? E - (R)(2.0 * GN_ME_C2) : E; io->ev = EV_PAIR; }   // pair: all of E, or the pair's kinetic energy
     io->j = rng.j;
 }
 
@@ -363,6 +384,25 @@ __device__ __forceinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, c
     io->j = rng.j;
 }
 
+// birth of annihilation photon k (NEXT-3): isotropic direction from draws 0, 1 of stream tag 1 of the parent (cos theta =
+// 1 - 2 u0, phi = 2 pi u1); photon 2 flies exactly the other way on stream tag 2; both have E = me c^2
+template <class R>
+__device__ __noinline__ void birth_secondary(BirthIO<R>* io, const PairVtx<R>* vtx, uint32_t k, uint64_t seed, uint64_t first_id) {
+    const PairVtx<R> pv = vtx[k >> 1];
+    PhiloxStream rng; rng.init(seed, first_id + pv.idx, 0, 1);
+    R u0 = draw<R>(rng), u1 = draw<R>(rng);
+    R ct = (R)1 - (R)2 * u0;
+    R st = rsqrt_(rmax(((R)1 - ct) * ((R)1 + ct), (R)0));
+    R sp, cp; rsincos((R)6.283185307179586 * u1, &sp, &cp);
+    R wx = st * cp, wy = st * sp, wz = ct;
+    if (k & 1u) { wx = -wx; wy = -wy; wz = -wz; rng.init(seed, first_id + pv.idx, 0, 2); }
+    io->x = pv.x; io->y = pv.y; io->z = pv.z; io->wx = wx; io->wy = wy; io->wz = wz; io->E = (R)GN_ME_C2;
+    io->Y = -rlog(draw<R>(rng));
+    EnergyFactors<R> ef = energy_factors(io->E);
+    io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
+    io->j = rng.j;
+}
+
 // PHYS = false: the lean wavefront pass -- photons that reach an interaction point park there and are written to the
 // back of the output queue; interact_pass handles them before the next pass.  PHYS = true: interactions happen inside
 // the pass (batched per warp); used for the last pass, which runs the few remaining photons to completion.
@@ -370,7 +410,7 @@ template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
 __global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS) ? (FROM_SOURCE ? TR_MIN_BLOCKS_SRC : (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX)) : 1)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
-               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio) {
+               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio, SecIO<R> sec) {
     // input: pass 0 generates n_src photons; later passes read the survivors of the previous pass, whose count is
     // known only on the device (front + back of cin)
     unsigned n_front = n_src, n_in = n_src;
@@ -411,14 +451,15 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         if (fate == FATE_ALIVE) {
             idx = i;
             BirthIO<R> b;
-            birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, seed, first_id + i);
+            if (sec.in) birth_secondary(&b, sec.in, i, seed, first_id);
+            else birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, seed, first_id + i);
             x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
             gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
-            c_phot = 1; e_src = (double)E;
+            if (!sec.in) { c_phot = 1; e_src = (double)E; }               // annihilation photons are not source photons
             vol = nav.locate(x, w, nd);
             if (vol < 0) {
                 fate = FATE_ESCAPED;
-                if (TRACK) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = 0; if (pp.efinal) pp.efinal[idx] = (double)E; }
+                if (TRACK) history_out(pp, sec, idx, h, 0u, E);
             }
         }
         c_phot = warp_sum(c_phot); e_src = warp_sum(e_src);
@@ -441,7 +482,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         if (fate == FATE_ALIVE && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; fate = FATE_STUCK; }
         if (TRACK) {
             fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
-            if (fate != FATE_ALIVE) { pp.hash[idx] = h; if (pp.nsteps) pp.nsteps[idx] = misc >> 8; if (pp.efinal) pp.efinal[idx] = (double)E; }
+            if (fate != FATE_ALIVE) history_out(pp, sec, idx, h, misc >> 8, E);
         }
     };
     int act0 = 32;
@@ -461,8 +502,9 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
                 const R mu = (muPE + muC) + muP;
                 InteractIO<R> io;
                 io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
-                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + idx);
+                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + (sec.in ? sec.in[idx >> 1].idx : idx), sec.in ? 1u + (idx & 1u) : 0u, sec.out != nullptr);
                 const int ev = io.ev; ctr = io.j;
+                if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = x.x; pv.y = x.y; pv.z = x.z; pv.idx = idx; sec.out[atomicAdd(sec.n_out, 1u)] = pv; }
                 dep_d = (double)io.dep;
                 if (ev == EV_COMPTON || ev == EV_CUT) {
                     E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
@@ -573,7 +615,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 template <class R, bool TRACK>
 __global__ void __launch_bounds__(TR_THREADS)
 interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters* __restrict__ cin, PhotonRec<R>* __restrict__ q, uint32_t cap,
-              double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp) {
+              double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = cin->back;
     if (blockIdx.x * TR_THREADS >= n) return;
     __shared__ unsigned long long sh_cnt[8];
@@ -595,8 +637,9 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         const R mu = (muPE + muC) + muP;
         InteractIO<R> io;
         io.E = r.E; io.wx = r.wx; io.wy = r.wy; io.wz = r.wz; io.Y = r.Y; io.gPE = r.gPE; io.gKN = r.gKN; io.L2k = r.L2k; io.j = r.ctr; io.above = above;
-        interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + r.idx);
+        interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + (sec.in ? sec.in[r.idx >> 1].idx : r.idx), sec.in ? 1u + (r.idx & 1u) : 0u, sec.out != nullptr);
         int ev = io.ev;
+        if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = r.x; pv.y = r.y; pv.z = r.z; pv.idx = r.idx; sec.out[atomicAdd(sec.n_out, 1u)] = pv; }
         dep_d = (double)io.dep;
         bool alive = false;
         if (ev == EV_COMPTON || ev == EV_CUT) {
@@ -613,8 +656,8 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         if (TRACK) {
             uint64_t h = pp.hash[r.idx];
             fnv_word(h, (uint32_t)vol); fnv_word(h, (uint32_t)ev);
-            pp.hash[r.idx] = h;
-            if (!alive) { if (pp.nsteps) pp.nsteps[r.idx] = r.misc >> 8; if (pp.efinal) pp.efinal[r.idx] = (double)r.E; }
+            if (alive) pp.hash[r.idx] = h;
+            else history_out(pp, sec, r.idx, h, r.misc >> 8, r.E);
         }
         if (alive) r.tail[0] &= 1u; else r.vol = -1;
         store_rec(q, cap - 1u - i, r);
@@ -720,15 +763,15 @@ constexpr int TR_TIMED = 24;                // lean step passes per batch timed 
 template <class R, bool SRC, bool PHYS, bool FLAT>
 static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
                         uint32_t n_src, const PassCounters* cin, PassCounters* cout, const PhotonRec<R>* qin, PhotonRec<R>* qout, uint32_t cap,
-                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio = SortIO{nullptr, nullptr, nullptr}) {
-    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio);
-    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio);
+                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct, SecIO<R> sec, SortIO sio = SortIO{nullptr, nullptr, nullptr}) {
+    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio, sec);
+    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio, sec);
 }
 template <class R>
 static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, uint64_t seed, uint64_t first_id, const PassCounters* cin,
-                            PhotonRec<R>* q, uint32_t cap, double* edep, DevStats* stats, PerPhotonOut pp) {
-    if (track) interact_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp);
-    else interact_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp);
+                            PhotonRec<R>* q, uint32_t cap, double* edep, DevStats* stats, PerPhotonOut pp, SecIO<R> sec) {
+    if (track) interact_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
+    else interact_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
 }
 
 template <class R>
@@ -739,14 +782,18 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     const bool track = d_hash || d_nsteps || d_efinal;
     const int K = geo->opts.steps_per_pass;
     const int K0 = std::min(K, geo->opts.first_pass_steps);      // first pass: short, sheds photons that miss
-    const size_t cap = (size_t)std::min<int64_t>(std::max<int64_t>(n_photons, 1), TR_BATCH);
+    const bool secondaries = geo->opts.secondaries > 0;        // NEXT-3: pair events leave two annihilation photons
+    const size_t cap = (size_t)std::min<int64_t>(std::max<int64_t>(n_photons, 2), TR_BATCH);
     const size_t qb = cap * sizeof(PhotonRec<R>);
     const size_t hb = (track && !d_hash) ? cap * 8 : 0;       // the hash array doubles as per-photon state between passes
     const size_t cb = sizeof(PassCounters) * (TR_MAX_PASSES + 2);
     const bool sorted = !geo->coherent;                        // general geometries: work order of every pass sorted by volume key
     const size_t kb = sorted ? sizeof(KeyCounters) * (TR_MAX_PASSES + 2) : 0;
     const size_t sb = sorted ? ((cap + 255) & ~(size_t)255) + 4 * cap : 0;      // keys + perm
-    const size_t need = 2 * qb + hb + 512 + cb + kb + sb;
+    const size_t pb = secondaries ? cap * sizeof(PairVtx<R>) + 16 : 0;          // pair vertices of a batch + their count
+    const size_t hb2 = (secondaries && track) ? cap * 8 : 0;                    // hash state of a batch of annihilation photons
+    const size_t base = (2 * qb + hb + 512 + cb + kb + sb + 15) & ~(size_t)15;
+    const size_t need = base + pb + hb2;
     std::lock_guard<std::mutex> lock(geo->ws_mutex);          // one run at a time per handle: the workspace is shared
     GN_CUDA(cudaMemsetAsync(d_edep, 0, sizeof(double) * (size_t)geo->n_places, s), "gn_transport_run memset edep");
     if (geo->ws_bytes < need) {
@@ -772,6 +819,9 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     KeyCounters* d_kctr = sorted ? (KeyCounters*)(scratch + 2 * qb + hb + 512 + cb) : nullptr;
     uint8_t* d_keys = sorted ? (uint8_t*)(scratch + 2 * qb + hb + 512 + cb + kb) : nullptr;
     uint32_t* d_perm = sorted ? (uint32_t*)(scratch + 2 * qb + hb + 512 + cb + kb + ((cap + 255) & ~(size_t)255)) : nullptr;
+    unsigned* d_npairs = secondaries ? (unsigned*)(scratch + base) : nullptr;
+    PairVtx<R>* d_pairs = secondaries ? (PairVtx<R>*)(scratch + base + 16) : nullptr;
+    uint64_t* sec_hash = hb2 ? (uint64_t*)(scratch + base + pb) : nullptr;
     int rc = GN_OK;
     uint64_t passes = 0, launches = 0;
     cudaEvent_t ev0 = geo->ws_events[0], ev1 = geo->ws_events[1];
@@ -783,10 +833,9 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     const int regroup = geo->opts.regroup_percent;
     cudaMemsetAsync(d_stats, 0, 512, s);
     const GeoView<R>& g = view<R>(geo);
-    for (int64_t done = 0; done < n_photons && rc == GN_OK; done += (int64_t)cap) {
-        const uint32_t n0 = (uint32_t)std::min<int64_t>((int64_t)cap, n_photons - done);
-        const uint64_t fid = (uint64_t)(first_id + done);
-        PerPhotonOut pp{d_hash ? d_hash + done : tmp_hash, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
+    // one batch of photons through the wavefront: n0 photons born in pass 0 (from the source, or -- sec.in -- at their
+    // parents' pair vertices), passes until none is left; ends with a stream synchronise
+    auto run_batch = [&](uint32_t n0, uint64_t fid, PerPhotonOut pp, SecIO<R> sec) {
         PhotonRec<R>* in = qb_; PhotonRec<R>* out = qa;
         cudaMemsetAsync(d_ctr, 0, cb, s);
         if (sorted) cudaMemsetAsync(d_kctr, 0, kb, s);
@@ -807,18 +856,18 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
             // FLAT = general geometry (any solid, rotations, long candidate lists); !FLAT = unrotated boxes only (geo->coherent)
             if (p == 0) {
-                if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup);
-                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup, SortIO{d_kctr + 1, d_keys, nullptr});
+                if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup, sec);
+                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup, sec, SortIO{d_kctr + 1, d_keys, nullptr});
             } else if (last) {
-                if (geo->coherent) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup);
-                else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, SortIO{nullptr, nullptr, d_perm});
+                if (geo->coherent) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec);
+                else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec, SortIO{nullptr, nullptr, d_perm});
             }
             else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
-                launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp);
+                launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
                 if (n_timed < TR_TIMED) cudaEventRecord(tev[2 * n_timed], s);
-                if (geo->coherent) launch_pass<R, false, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup);
-                else launch_pass<R, false, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, SortIO{d_kctr + p + 1, d_keys, d_perm});
+                if (geo->coherent) launch_pass<R, false, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec);
+                else launch_pass<R, false, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec, SortIO{d_kctr + p + 1, d_keys, d_perm});
                 if (n_timed < TR_TIMED) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
                 ++launches;
             }
@@ -841,6 +890,25 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         if (e != cudaSuccess && rc == GN_OK) rc = cuda_fail(e, "gn_transport_run batch");
         { float ms = 0.f; if (rc == GN_OK && cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
         for (int q = 0; q < n_timed && rc == GN_OK; ++q) { float ms = 0.f; if (cudaEventElapsedTime(&ms, tev[2 * q], tev[2 * q + 1]) == cudaSuccess) step_pass_ms += ms; }
+    };
+    for (int64_t done = 0; done < n_photons && rc == GN_OK; done += (int64_t)cap) {
+        const uint32_t n0 = (uint32_t)std::min<int64_t>((int64_t)cap, n_photons - done);
+        const uint64_t fid = (uint64_t)(first_id + done);
+        PerPhotonOut pp{d_hash ? d_hash + done : tmp_hash, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
+        if (secondaries) cudaMemsetAsync(d_npairs, 0, sizeof(unsigned), s);
+        run_batch(n0, fid, pp, SecIO<R>{d_pairs, d_npairs, nullptr, nullptr, nullptr});
+        if (!secondaries || rc != GN_OK) continue;
+        // the annihilation photons of this batch's pair events, at most cap at a time (511 keV: they cannot pair again)
+        unsigned n_pairs = 0;
+        e = cudaMemcpyAsync(&n_pairs, d_npairs, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pair count"); break; }
+        const unsigned chunk = (unsigned)(cap / 2);
+        for (unsigned off = 0; off < n_pairs && rc == GN_OK; off += chunk) {
+            const unsigned np = std::min(chunk, n_pairs - off);
+            run_batch(2u * np, fid, PerPhotonOut{sec_hash, nullptr, nullptr},
+                      SecIO<R>{nullptr, nullptr, d_pairs + off, d_hash ? (unsigned long long*)(d_hash + done) : nullptr, d_nsteps ? d_nsteps + done : nullptr});
+        }
     }
     if (rc == GN_OK) {
         DevStats hs;

@@ -6,11 +6,12 @@
 
 namespace gn {
 
-// ---- counter-based RNG (C7): key = seed, counter = (photon id lo, hi, block, 0); draw j = 64-bit lane j&1 of block j>>1
+// ---- counter-based RNG (C7): key = seed, counter = (photon id lo, hi, block, tag); draw j = 64-bit lane j&1 of block j>>1;
+// tag 0 = the primary photon, 1 / 2 = the annihilation photons of its pair event
 // One copy of the ten rounds, out of line: draws happen only at interactions (rare next to navigation steps).
-// the ten rounds of one block: counter (id0, id1, blk, 0) under key (k0, k1) -> two 64-bit lanes
-__device__ __forceinline__ void philox_block(uint32_t k0, uint32_t k1, uint32_t id0, uint32_t id1, uint32_t blk, uint64_t& l0, uint64_t& l1) {
-    uint32_t c0 = id0, c1 = id1, c2 = blk, c3 = 0, a = k0, b = k1;
+// the ten rounds of one block: counter (id0, id1, blk, tag) under key (k0, k1) -> two 64-bit lanes
+__device__ __forceinline__ void philox_block(uint32_t k0, uint32_t k1, uint32_t id0, uint32_t id1, uint32_t blk, uint32_t tag, uint64_t& l0, uint64_t& l1) {
+    uint32_t c0 = id0, c1 = id1, c2 = blk, c3 = tag, a = k0, b = k1;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
@@ -24,17 +25,17 @@ __device__ __forceinline__ void philox_block(uint32_t k0, uint32_t k1, uint32_t 
 }
 // draw j = lane (j & 1) of block j >> 1; the second lane of a block is kept for the next draw
 struct PhiloxStream {
-    uint32_t k0, k1, id0, id1, j;
+    uint32_t k0, k1, id0, id1, j, tag;
     uint64_t spare; bool have_spare;
-    __device__ __forceinline__ void init(uint64_t seed, uint64_t id, uint32_t draws_done) {
-        k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32); id0 = (uint32_t)id; id1 = (uint32_t)(id >> 32); j = draws_done;
+    __device__ __forceinline__ void init(uint64_t seed, uint64_t id, uint32_t draws_done, uint32_t stream_tag = 0) {
+        k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32); id0 = (uint32_t)id; id1 = (uint32_t)(id >> 32); j = draws_done; tag = stream_tag;
         spare = 0; have_spare = false;
     }
     __device__ __forceinline__ uint64_t next() {
         uint64_t out;
         if ((j & 1u) && have_spare) { out = spare; have_spare = false; }
         else {
-            uint64_t l0, l1; philox_block(k0, k1, id0, id1, j >> 1, l0, l1);
+            uint64_t l0, l1; philox_block(k0, k1, id0, id1, j >> 1, tag, l0, l1);
             if (j & 1u) out = l1; else { out = l0; spare = l1; have_spare = true; }
         }
         ++j;

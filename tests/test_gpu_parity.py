@@ -227,8 +227,8 @@ TRANSPORT_CASES = {
 }
 
 
-def compare_transport(B, geom, src, n, seed, precision, min_identical, opts=None):
-    og = oracle.OracleGeometry(geom); g = B.Geometry(geom, **(opts or {}))
+def compare_transport(B, geom, src, n, seed, precision, min_identical, opts=None, oracle_opts=None):
+    og = oracle.OracleGeometry(geom, **(oracle_opts or {})); g = B.Geometry(geom, **(opts or {}))
     got = B.transport_run(g, src, seed, n, precision, per_photon=True)
     ref = og.transport(src, seed, n, precision, per_photon=True)
     hg = got["hash"].cpu().numpy().view(np.uint64); ng = got["nsteps"].cpu().numpy().astype(np.uint32)
@@ -264,6 +264,78 @@ def test_transport_fp32_aggregate(B, name):
     # still overwhelmingly identical because both sides consume the same Philox draws in the same order
     got, ref, frac = compare_transport(B, geom, src, n, seed, 32, 0.97)
     print(f"{name} fp32 identical histories: {frac:.5f}")
+
+
+def _four_walls():
+    from paper_1209_5235_b200.workloads import _Builder
+    b = _Builder("four_walls")
+    world = b.place(-1, b.box(1000.0, 1000.0, 1000.0), "vacuum")
+    b.place(world, b.box(0.25, 0.25, 4.0), "lead")
+    wall_x, wall_y = b.box(50.0, 150.0, 900.0), b.box(50.0, 50.0, 900.0)
+    for solid, T in ((wall_x, (150.0, 0, 0)), (wall_x, (-150.0, 0, 0)), (wall_y, (0, 150.0, 0)), (wall_y, (0, -150.0, 0))):
+        b.place(world, solid, "lead", T=T)
+    return b.finish()
+
+
+def _pencil(E):
+    return W.Source(W.SRC_PENCIL, (0.0, 0.0, -500.0), (0.0, 0.0, 1.0), W.E_MONO, E)
+
+
+SECONDARY_CASES = {
+    # thick lead, 20 MeV: most primaries end in a pair event, so the annihilation photons need more than one batch of cap / 2 pairs
+    "lead_slab_20MeV": lambda: (W.homogeneous_slab("lead", half=(200.0, 200.0, 10.0), world_half=1000.0), _pencil(20.0), 20000, 3),
+    "four_walls": lambda: (_four_walls(), _pencil(8.0), 20000, 21),
+    "calorimeter": lambda: (W.calorimeter_geometry(10), W.calorimeter_source(), 20000, 2),
+    "phantom16_6MeV": lambda: (W.phantom_geometry(16, 2.0, 3), W.phantom_source(16, half_angle_deg=0.8), 20000, 3),
+    "detector": lambda: (W.detector_geometry(seed=4, n_phi=16, n_z=8, barrels=((200, 400), (450, 650))), W.detector_source(), 20000, 4),
+    "cmslike": lambda: (W.cms_like_geometry(), W.Source(W.SRC_ISOTROPIC, (0.0, 0.0, 0.0), (0, 0, 1.0), W.E_LOGUNIFORM, 0.1, 1000.0), 20000, 6),
+}
+
+
+@pytest.mark.parametrize("wavefront", [False, True])
+@pytest.mark.parametrize("name", list(SECONDARY_CASES))
+def test_secondary_photons_fp64_histories_identical(B, name, wavefront):
+    """pair events leave two annihilation photons (Philox stream tags 1 / 2), followed in batches of
+    their own after the primaries; per-photon hash and step count are sums over the primary and its secondaries.
+    wavefront: tail_photons = 1 and short passes, so the secondaries go through the lean passes, the compaction and the
+    interaction wavefront as well (default for this n: source pass, then one run-to-completion pass)."""
+    geom, src, n, seed = SECONDARY_CASES[name]()
+    opts = dict(secondaries=1, **(dict(steps_per_pass=5, tail_photons=1) if wavefront else {}))
+    got, ref, _ = compare_transport(B, geom, src, n, seed, 64, 0.999, opts=opts, oracle_opts=dict(secondaries=1))
+    s, r = got["stats"], ref["stats"]
+    assert s["n_pair"] == r["n_pair"] and s["n_pair"] > 100
+    # every photon ends exactly once; each pair event adds two photons
+    assert s["n_pe"] + s["n_pair"] + s["n_cut"] + s["n_escaped"] + s["n_stuck"] == n + 2 * s["n_pair"]
+    if name == "lead_slab_20MeV":
+        assert 2 * s["n_pair"] > n                                   # more than one batch of annihilation photons
+
+
+@pytest.mark.parametrize("name", ["lead_slab_20MeV", "calorimeter", "detector"])
+def test_secondary_photons_fp32_aggregate(B, name):
+    geom, src, n, seed = SECONDARY_CASES[name]()
+    got, ref, frac = compare_transport(B, geom, src, n, seed, 32, 0.97, opts=dict(secondaries=1), oracle_opts=dict(secondaries=1))
+    print(f"{name} fp32 with secondaries, identical histories: {frac:.5f}")
+
+
+def test_secondary_photons_without_per_photon_outputs_and_below_threshold(B):
+    geom, src, n, seed = SECONDARY_CASES["four_walls"]()
+    g1 = B.Geometry(geom, secondaries=1)
+    a = B.transport_run(g1, src, seed, n, 64, per_photon=True)
+    b = B.transport_run(g1, src, seed, n, 64)                        # the lean (untracked) kernels
+    assert np.allclose(a["edep"].cpu().numpy(), b["edep"].cpu().numpy(), rtol=1e-12, atol=1e-12)
+    for k in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons"):
+        assert a["stats"][k] == b["stats"][k], k
+    # below 2 me c^2 the option changes nothing
+    g0 = B.Geometry(geom)
+    c = B.transport_run(g0, _pencil(1.0), seed, 5000, 64, per_photon=True)
+    d = B.transport_run(g1, _pencil(1.0), seed, 5000, 64, per_photon=True)
+    assert np.array_equal(c["hash"].cpu().numpy(), d["hash"].cpu().numpy())
+    assert np.allclose(c["edep"].cpu().numpy(), d["edep"].cpu().numpy(), rtol=1e-12, atol=1e-12)      # fp64 atomics: order of the adds
+    assert d["stats"]["n_pair"] == 0 and d["stats"]["n_steps"] == c["stats"]["n_steps"]
+    # one photon (queue capacity 2): its pair, if any, still fits
+    e = B.transport_run(g1, _pencil(8.0), seed, 1, 64, per_photon=True)
+    r = oracle.OracleGeometry(geom, secondaries=1).transport(_pencil(8.0), seed, 1, 64, per_photon=True)
+    assert int(e["hash"].cpu().numpy().view(np.uint64)[0]) == int(r["hash"][0])
 
 
 def test_transport_is_independent_of_steps_per_pass_and_sharding(B):
