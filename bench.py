@@ -297,6 +297,8 @@ def run_ours(args):
         gopts["first_pass_steps"] = args.first_pass_steps
     if args.regroup_percent:
         gopts["regroup_percent"] = args.regroup_percent
+    if args.secondaries:
+        gopts["secondaries"] = 1
     geo = B.Geometry(wl.geometry, **gopts)
     transport = wl.source is not None
     dom = [0, 0.0]                                            # dominant kernel: steps taken in / summed duration of the lean step passes
@@ -428,7 +430,7 @@ def run_ours(args):
                 "config": {"workload": wl.name, "precision": precision, ("photons_per_gpu" if transport else "queries_per_gpu"): n,
                            "volumes": geo.n_places, "l2": "photon state queues (2 x %d MB) exceed the 126 MB L2; no explicit flush" % (n * (64 if precision == 32 else 112) // 10 ** 6)
                            if transport else "query arrays (%d MB) exceed the 126 MB L2" % (n * 6 * (4 if precision == 32 else 8) // 10 ** 6),
-                           "parallelism": f"dp{world} (photon-id ranges, replicated geometry)"},
+                           "parallelism": f"dp{world} (photon-id ranges, replicated geometry)", **({"secondaries": 1} if args.secondaries else {})},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
                 "units_per_step": units / args.steps / world}
         print(json.dumps(line))
@@ -451,10 +453,14 @@ def main():
     ap.add_argument("--tail-photons", type=int, default=0, help="diagnostics: override gn_opts.tail_photons")
     ap.add_argument("--first-pass-steps", type=int, default=0, help="diagnostics: override gn_opts.first_pass_steps")
     ap.add_argument("--regroup-percent", type=int, default=0, help="diagnostics: override gn_opts.regroup_percent")
+    ap.add_argument("--secondaries", action="store_true",
+                    help="variant (not BASELINE.json's workload): gn_opts.secondaries = 1, annihilation photons of pair events are transported; no cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-all-cores", action="store_true")
     ap.add_argument("--allow-short-warmup", action="store_true")
     args = ap.parse_args()
+    if args.secondaries:
+        args.no_cpu_baseline = True
     if args.config in (6, 7):
         return run_freepath(args)
     if args.impl == "reference":

@@ -427,6 +427,7 @@ extern "C" int gn_geometry_destroy(gn_geometry* geo) {
     for (void* p : geo->allocations) cudaFree(p);
     if (geo->ws_scratch) cudaFree(geo->ws_scratch);
     if (geo->ws_pinned) cudaFreeHost(geo->ws_pinned);
+    if (geo->ws_host_edep) cudaFree(geo->ws_host_edep);
     if (geo->ws_events_ok) for (cudaEvent_t e : geo->ws_events) if (e) cudaEventDestroy(e);
     delete geo;
     return GN_OK;

@@ -19,9 +19,11 @@ struct gn_geometry {
     // transport workspace (photon queues, counters, pinned read-back, events): grown on demand, reused by every
     // gn_transport_run on this handle, released by gn_geometry_destroy; runs on one handle are serialised
     mutable std::mutex ws_mutex;
+    mutable std::mutex host_mutex;            // held across a whole gn_transport_run_host call (its staging buffer is shared)
     mutable char* ws_scratch = nullptr;
     mutable size_t ws_bytes = 0;
     mutable void* ws_pinned = nullptr;
+    mutable double* ws_host_edep = nullptr;   // device staging of the tally for gn_transport_run_host (n_places doubles)
     mutable cudaEvent_t ws_events[8 + 48] = {};
     mutable bool ws_events_ok = false;
 };

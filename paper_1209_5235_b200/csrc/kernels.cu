@@ -1051,14 +1051,19 @@ extern "C" int gn_nav_query_host(const gn_geometry* geo, int precision, const vo
 extern "C" int gn_transport_run_host(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
                                      int64_t first_photon_id, int64_t n_photons, double* h_edep_out, gn_run_stats* h_stats_out) {
     if (!geo || !h_edep_out) return fail(GN_INVALID_ARGUMENT, "gn_transport_run_host: bad argument");
-    double* d = nullptr;
     const size_t bytes = sizeof(double) * (size_t)geo->n_places;
-    if (cudaMalloc((void**)&d, bytes) != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, "gn_transport_run_host: cudaMalloc"); }
+    double* d = nullptr;
+    std::lock_guard<std::mutex> host_lock(geo->host_mutex);
+    {   // the device staging buffer of the tally belongs to the handle (no allocation per call)
+        if (!geo->ws_host_edep && cudaMalloc((void**)&geo->ws_host_edep, bytes) != cudaSuccess) {
+            cudaGetLastError(); geo->ws_host_edep = nullptr;
+            return fail(GN_OUT_OF_MEMORY, "gn_transport_run_host: cudaMalloc");
+        }
+        d = geo->ws_host_edep;
+    }
     int rc = gn_transport_run(geo, precision, h_src, seed, first_photon_id, n_photons, d, h_stats_out, nullptr, nullptr, nullptr, nullptr);
-    cudaError_t e = cudaSuccess;
-    if (rc == GN_OK) e = cudaMemcpy(h_edep_out, d, bytes, cudaMemcpyDeviceToHost);
-    cudaFree(d);
     if (rc != GN_OK) return rc;
+    cudaError_t e = cudaMemcpy(h_edep_out, d, bytes, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(e, "gn_transport_run_host");
     return GN_OK;
 }
