@@ -124,6 +124,13 @@ class OracleGeometry:
                                                     _p(nrm), C.c_int(int(use_grid))), "nav_compute_step_normal")
         return step, nxt, nrm
 
+    def compute_safety(self, pos, vol, precision=64):
+        R = _real(precision)
+        pos = np.ascontiguousarray(pos, R); vol = np.ascontiguousarray(vol, np.int32)
+        out = np.empty(pos.shape[0], R)
+        _check(lib().oracle_nav_compute_safety(self._h, C.c_int(precision), _p(pos), _p(vol), C.c_int64(pos.shape[0]), _p(out)), "nav_compute_safety")
+        return out
+
     def transport(self, src, seed, n, precision=64, first_id=0, per_photon=False, use_grid=True):
         edep = np.zeros(self.n_places, np.float64); st = Stats()
         h = np.empty(n, np.uint64) if per_photon else None
@@ -156,7 +163,7 @@ class OracleGeometry:
 def solid_eval(stype, params, tol, what, pos, dirs=None, precision=64):
     """what: 'inside' | 'dist_in' | 'dist_out' for one solid on many points."""
     R = _real(precision)
-    code = {"inside": 0, "dist_in": 1, "dist_out": 2, "normal": 3}[what]
+    code = {"inside": 0, "dist_in": 1, "dist_out": 2, "normal": 3, "safety_in": 4, "safety_out": 5}[what]
     pos = np.ascontiguousarray(pos, R)
     dirs = np.ascontiguousarray(dirs if dirs is not None else np.zeros_like(pos), R)
     p5 = np.zeros(5, np.float64); p5[:len(params)] = params

@@ -19,7 +19,9 @@
  * conservation, chi^2 of sampled epsilon, slab transmission exp(-mu x), energy book-keeping,
  * Philox vs. cuRAND's host generator, uniform end points; orb closed forms / ray marching and the
  * attenuation-only free paths (the paper's own benchmark) vs. a sorted-chord closed form in numpy
- * (tests/test_oracle_freepath.py).
+ * (tests/test_oracle_freepath.py); secondary photons (tests/test_oracle_secondaries.py); isotropic safety: points
+ * built at a chosen distance off one face of every surface kind, lower bound against DistanceToIn / DistanceToOut in
+ * many directions, attained from inside box / tube / orb, never above a ComputeStep (tests/test_oracle_safety.py).
  * PARITY UNPINNED (defined only by SURVEY 8(c)/DESIGN.md, no independent truth exists):
  *   sigma_PE0 normalisation, the capped Bethe-Heitler form, A values, source frame convention,
  *   tolerances, tie-breaks, stuck guard, history hash.
@@ -108,10 +110,10 @@ template <class R> inline int classify(R D, R delta) {         /* S:C2 "Inside" 
 }
 
 /* BOX: s_i = |p_i| - h_i */
-template <class R> int box_inside(const SolidR<R>& s, const R p[3], R delta) {
-    R D = r_max(r_max(r_abs(p[0]) - s.a, r_abs(p[1]) - s.b), r_abs(p[2]) - s.c);
-    return classify(D, delta);
+template <class R> R box_outsideness(const SolidR<R>& s, const R p[3]) {
+    return r_max(r_max(r_abs(p[0]) - s.a, r_abs(p[1]) - s.b), r_abs(p[2]) - s.c);
 }
+template <class R> int box_inside(const SolidR<R>& s, const R p[3], R delta) { return classify(box_outsideness(s, p), delta); }
 
 /* one planar pair +-h along an axis, exit rule of S:C2: if moving outward and within the band -> 0,
  * else candidate (sign(v) h - p)/v.  Returns false when the answer is 0. */
@@ -154,7 +156,7 @@ template <class R> R box_dist_in(const SolidR<R>& s, const R p[3], const R v[3],
 }
 
 /* TUBE: rmin=a, rmax=b, hz=c; sector planes s_S = sS x - cS y, s_E = cE y - sE x */
-template <class R> int tube_inside(const SolidR<R>& s, const R p[3], R delta) {
+template <class R> R tube_outsideness(const SolidR<R>& s, const R p[3]) {
     R r = r_sqrt(p[0] * p[0] + p[1] * p[1]);
     R D = r_abs(p[2]) - s.c;
     D = r_max(D, r - s.b);
@@ -163,8 +165,9 @@ template <class R> int tube_inside(const SolidR<R>& s, const R p[3], R delta) {
         D = r_max(D, s.sS * p[0] - s.cS * p[1]);
         D = r_max(D, s.cE * p[1] - s.sE * p[0]);
     }
-    return classify(D, delta);
+    return D;
 }
+template <class R> int tube_inside(const SolidR<R>& s, const R p[3], R delta) { return classify(tube_outsideness(s, p), delta); }
 
 template <class R> R tube_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
     R best = r_inf<R>();
@@ -281,10 +284,11 @@ template <class R> R tube_dist_in(const SolidR<R>& s, const R p[3], const R v[3]
 
 /* ORB (radius a): s = |p| - r.  D:"orb solid" -- the sphere analogue of the S:C2 cylinder rules; the paper only
  * names the solid ("aluminium balls").  Sums are (x.x + y.y) + z.z, left to right. */
-template <class R> int orb_inside(const SolidR<R>& s, const R p[3], R delta) {
+template <class R> R orb_outsideness(const SolidR<R>& s, const R p[3]) {
     R rp = r_sqrt((p[0] * p[0] + p[1] * p[1]) + p[2] * p[2]);
-    return classify(rp - s.a, delta);
+    return rp - s.a;
 }
+template <class R> int orb_inside(const SolidR<R>& s, const R p[3], R delta) { return classify(orb_outsideness(s, p), delta); }
 template <class R> R orb_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
     R a = (v[0] * v[0] + v[1] * v[1]) + v[2] * v[2];
     R b = (p[0] * v[0] + p[1] * v[1]) + p[2] * v[2];
@@ -315,12 +319,12 @@ template <class R> R orb_dist_in(const SolidR<R>& s, const R p[3], const R v[3],
  * host, rounded once).  Surface radius u(z) = r0 + m z; s_z = |z| - hz; s_c = (r - u) cs (true distance to the cone).
  * Along a ray, f(t) = r(t)^2 - u(t)^2 = A t^2 + 2 B t + C with du = m v_z, A = (vx^2 + vy^2) - du^2,
  * B = (x vx + y vy) - u du, C = (x^2 + y^2) - u^2; B > 0 <=> moving outward at the surface. */
-template <class R> int cone_inside(const SolidR<R>& s, const R p[3], R delta) {
+template <class R> R cone_outsideness(const SolidR<R>& s, const R p[3]) {
     R r = r_sqrt(p[0] * p[0] + p[1] * p[1]);
     R u = s.a + s.b * p[2];
-    R D = r_max(r_abs(p[2]) - s.c, (r - u) * s.cS);
-    return classify(D, delta);
+    return r_max(r_abs(p[2]) - s.c, (r - u) * s.cS);
 }
+template <class R> int cone_inside(const SolidR<R>& s, const R p[3], R delta) { return classify(cone_outsideness(s, p), delta); }
 template <class R> R cone_dist_out(const SolidR<R>& s, const R p[3], const R v[3], R delta) {
     R best = r_inf<R>();
     if (!slab_out(p[2], v[2], s.c, delta, best)) return 0;            /* z planes */
@@ -426,6 +430,17 @@ template <class R> void solid_normal(const SolidR<R>& s, const R q[3], R n[3]) {
 }
 
 /* the "fork" on solid type */
+/* Isotropic safety (S:8(f) NEXT-4, D:reading 17): every s of S:C2 is the signed distance of p to ONE bounding surface's
+ * half-space / cylinder / sphere / cone (negative inside), and the solid is the intersection of those sets.  So for a
+ * point inside, min_i(-s_i) = -D is the distance to the nearest bounding surface (no boundary is nearer: a lower bound
+ * of the exit distance in EVERY direction; exact for box, tube and orb, a lower bound for the cone, whose (r - u) cs is
+ * the distance to the generator LINE); for a point outside, dist(p, intersection) >= max_i dist(p, set_i) = D. */
+template <class R> R solid_outsideness(const SolidR<R>& s, const R p[3]) {
+    return s.type == ORACLE_BOX ? box_outsideness(s, p) : (s.type == ORACLE_TUBE ? tube_outsideness(s, p) : (s.type == ORACLE_ORB ? orb_outsideness(s, p) : cone_outsideness(s, p)));
+}
+template <class R> R solid_safety_out(const SolidR<R>& s, const R p[3]) { return r_max(-solid_outsideness(s, p), (R)0); }
+template <class R> R solid_safety_in(const SolidR<R>& s, const R p[3]) { return r_max(solid_outsideness(s, p), (R)0); }
+
 template <class R> int solid_inside(const SolidR<R>& s, const R p[3], R delta) {
     return s.type == ORACLE_BOX ? box_inside(s, p, delta) : (s.type == ORACLE_TUBE ? tube_inside(s, p, delta) : (s.type == ORACLE_ORB ? orb_inside(s, p, delta) : cone_inside(s, p, delta)));
 }
@@ -488,6 +503,19 @@ template <class R> struct Navigator {
             if (found < 0) return cur;
             cur = found;
         }
+    }
+    /* Isotropic safety of point x in volume vol (S:8(f) NEXT-4, D:reading 17): plain linear scan -- the smaller of
+     * SafetyToOut of vol's own solid and SafetyToIn of every daughter of vol, in index order.  No boundary of vol or of
+     * one of its daughters is nearer than this in any direction.  vol = -1 -> 0. */
+    R safety(int vol, const R x[3]) const {
+        if (vol < 0) return 0;
+        R p[3]; local_point(vol, x, p);
+        R best = solid_safety_out(S[g.solid[vol]], p);
+        for (int d : g.daughters[vol]) {
+            R q[3]; local_point(d, x, q);
+            best = r_min(best, solid_safety_in(S[g.solid[d]], q));
+        }
+        return best;
     }
     int locate(const R x[3], const R* w) const {
         if (!occupies(0, x, w)) return -1;
@@ -978,6 +1006,16 @@ template <class R> int run_transport(const Geo& g, const oracle_source_t* src, u
     return ORACLE_OK;
 }
 
+template <class R> int run_safety(const Geo& g, const void* pos, const int32_t* vol_in, int64_t n, void* out) {
+    Navigator<R> nav(g, false);
+    const R* P = (const R*)pos; R* O = (R*)out;
+    for (int64_t i = 0; i < n; ++i) {
+        if (vol_in[i] < -1 || vol_in[i] >= (int32_t)g.parent.size()) return ORACLE_INVALID_ARGUMENT;
+        O[i] = nav.safety(vol_in[i], P + 3 * i);
+    }
+    return ORACLE_OK;
+}
+
 template <class R> int run_solid_eval(const SolidD& sd, double tol, int what, const void* pos, const void* dir, int64_t n, void* out) {
     SolidR<R> s = round_solid<R>(sd);
     R delta = (R)tol / 2;
@@ -986,6 +1024,8 @@ template <class R> int run_solid_eval(const SolidD& sd, double tol, int what, co
         if (what == 0) O[i] = (R)solid_inside(s, P + 3 * i, delta);
         else if (what == 1) O[i] = solid_dist_in(s, P + 3 * i, D + 3 * i, delta);
         else if (what == 3) solid_normal(s, P + 3 * i, O + 3 * i);            /* out: n x 3 */
+        else if (what == 4) O[i] = solid_safety_in(s, P + 3 * i);
+        else if (what == 5) O[i] = solid_safety_out(s, P + 3 * i);
         else O[i] = solid_dist_out(s, P + 3 * i, D + 3 * i, delta);
     }
     return ORACLE_OK;
@@ -1135,6 +1175,14 @@ int oracle_nav_compute_step(const void* geo, int precision, const void* pos, con
     const Geo& g = *(const Geo*)geo;
     if (precision == 64) return run_step<double>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, use_grid != 0);
     if (precision == 32) return run_step<float>(g, pos, dir, vol_in, max_step, n, step_out, next_vol_out, use_grid != 0);
+    return ORACLE_INVALID_ARGUMENT;
+}
+
+int oracle_nav_compute_safety(const void* geo, int precision, const void* pos, const int32_t* vol_in, int64_t n, void* safety_out) {
+    if (!geo || n < 0 || (n > 0 && (!pos || !vol_in || !safety_out))) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    if (precision == 64) return run_safety<double>(g, pos, vol_in, n, safety_out);
+    if (precision == 32) return run_safety<float>(g, pos, vol_in, n, safety_out);
     return ORACLE_INVALID_ARGUMENT;
 }
 

@@ -79,6 +79,9 @@ int oracle_nav_compute_step(const void* geo, int precision, const void* pos, con
 /* ComputeStep with the surface normal ("what is the normal of the boundary surface at that point?"): as
  * oracle_nav_compute_step, plus normal_out n x 3 Real: outward unit normal, global frame, of the solid whose surface ends
  * the step (own solid on exit, the entered daughter otherwise); (0,0,0) when no boundary lies within max_step. */
+/* isotropic safety (S:8(f) NEXT-4, D:reading 17): lower bound, valid in every direction, of the distance from pos[i] (a point
+ * of volume vol_in[i]) to the nearest boundary of that volume's solid or of one of its daughters; linear scan; vol -1 -> 0 */
+int oracle_nav_compute_safety(const void* geo, int precision, const void* pos, const int32_t* vol_in, int64_t n, void* safety_out);
 int oracle_nav_compute_step_normal(const void* geo, int precision, const void* pos, const void* dir, const int32_t* vol_in,
                                    const void* max_step, int64_t n, void* step_out, int32_t* next_vol_out, void* normal_out, int use_grid);
 
