@@ -148,6 +148,19 @@ int gn_nav_compute_step_normal(const gn_geometry* geo, int precision, const void
                                void* d_step_out, int32_t* d_next_vol_out, void* d_normal_out, void* cuda_stream);
 
 /*
+ * gn_nav_compute_safety -- isotropic safety distance (the boundary problem of PAPER.md L124-125 without a
+ * direction): a lower bound, valid in EVERY direction, of the distance from d_pos[i] to the nearest boundary of volume
+ * d_vol_in[i]'s own solid or of one of its daughters -- no gn_nav_compute_step from that point is shorter.
+ *   = min( max(-D_vol(p), 0), min over daughters d of max(D_d(p_d), 0) ),  D = the outsideness of SURVEY 8(c) C2 (the largest
+ *   signed distance to one bounding plane / cylinder / sphere / cone of the solid, negative inside); from inside it is the exact
+ *   distance to the nearest bounding surface for box, tube and orb (reading 17).
+ *   d_pos n x 3 Real (device), d_vol_in n int32 (as returned by gn_nav_locate; -1 or out of range gives 0),
+ *   d_safety_out n Real (device, caller-owned).  Asynchronous on cuda_stream.  Daughters are scanned linearly.
+ */
+int gn_nav_compute_safety(const gn_geometry* geo, int precision, const void* d_pos, const int32_t* d_vol_in, int64_t n,
+                          void* d_safety_out, void* cuda_stream);
+
+/*
  * gn_transport_run -- PAPER.md Algorithm 1 (L55-76) for photons first_photon_id .. first_photon_id + n - 1,
  * each with its own Philox4x32-10 stream keyed by (seed, photon id).
  *   d_edep_out    gn_geometry_num_places doubles [MeV]; ZEROED by the callee, then accumulated (fp64 atomics)

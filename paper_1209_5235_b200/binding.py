@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "libgammanav.so")
 _lib = None
 
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",
-           "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_nav_compute_step_normal", "gn_transport_run", "gn_nav_query_host",
+           "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_nav_compute_step_normal", "gn_nav_compute_safety", "gn_transport_run", "gn_nav_query_host",
            "gn_transport_run_host", "gn_free_path_run", "gn_free_path_run_host", "gn_selftest_arith", "gn_last_error", "gn_version")
 
 
@@ -66,6 +66,7 @@ def lib():
         L.gn_geometry_voxel_info.argtypes = [C.c_void_p, C.c_void_p]
         L.gn_nav_locate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.gn_nav_compute_step.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.gn_nav_compute_safety.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.gn_nav_compute_step_normal.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_transport_run.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
@@ -202,6 +203,20 @@ def nav_compute_step_normal(geo: Geometry, pos, dirs, vol, max_step=None, precis
                                             C.c_void_p(step.data_ptr()), C.c_void_p(nxt.data_ptr()), C.c_void_p(nrm.data_ptr()), _stream_ptr(torch)),
            "gn_nav_compute_step_normal")
     return step, nxt, nrm
+
+
+def nav_compute_safety(geo: Geometry, pos, vol, precision=None):
+    """gn_nav_compute_safety on device tensors -> safety (n,) Real."""
+    torch = _torch()
+    precision = precision or (32 if pos.dtype == torch.float32 else 64)
+    dt = _real_dtype(torch, precision)
+    if pos.dtype != dt or vol.dtype != torch.int32 or not (pos.is_cuda and vol.is_cuda):
+        raise GammaNavError("nav_compute_safety: tensors must be CUDA, Real / int32")
+    pos = pos.contiguous(); vol = vol.contiguous(); n = pos.shape[0]
+    out = torch.empty(n, dtype=dt, device=pos.device)
+    _check(lib().gn_nav_compute_safety(geo._h, precision, C.c_void_p(pos.data_ptr()), C.c_void_p(vol.data_ptr()), C.c_int64(n),
+                                       C.c_void_p(out.data_ptr()), _stream_ptr(torch)), "gn_nav_compute_safety")
+    return out
 
 
 def transport_run(geo: Geometry, source, seed, n_photons, precision=32, first_photon_id=0, per_photon=False, edep=None):

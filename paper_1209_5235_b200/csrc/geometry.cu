@@ -395,6 +395,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     }
     Uploader up{geo};
     const int* d_dlist = up.put(dlist);
+    { std::vector<int> dfirst(V); for (size_t i = 0; i < V; ++i) dfirst[i] = kids[i].x; geo->v32.dfirst = geo->v64.dfirst = up.put(dfirst); }
     const int2* d_cells = up.put(cells); const int* d_cand = up.put(cand);
     GeoView<float>& a = geo->v32; GeoView<double>& b = geo->v64;
     a.dlist = b.dlist = d_dlist; a.cells = b.cells = d_cells; a.cand = b.cand = d_cand;

@@ -158,6 +158,38 @@ __global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLO
     }
 }
 
+// Isotropic safety (reading 17): min of SafetyToOut of the volume's own solid and SafetyToIn of
+// each of its daughters, SafetyToOut / In = max(-D, 0) / max(D, 0) with D the outsideness of C2.  Plain scan of the daughter
+// list, one thread per query (lanes of a warp in the same mother read the same daughters: broadcast loads from L1 / L2).
+template <class R>
+__global__ void __launch_bounds__(NAV_THREADS) safety_kernel(GeoView<R> g, const R* __restrict__ pos, const int32_t* __restrict__ vol_in,
+                                                             int64_t n, R* __restrict__ safety_out) {
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
+    __syncthreads();
+    const NavCtx<R>* c = &tab.ctx;
+    const V3<R> w0{0, 0, 1};
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        const int vol = vol_in[i];
+        R best = 0;
+        if (vol >= 0 && vol < g.n_nodes) {
+            const NodeRec<R> nd = load_node(g.node, vol);
+            V3<R> p, v;
+            to_local<R, true>(c->rot, vol, nd, x, w0, p, v);
+            best = rmax(-outsideness(c->solids[nd.info & NODE_SOLID_MASK], p), (R)0);
+            const int first = __ldg(&g.dfirst[vol]);
+            for (int k = 0; k < nd.ndau; ++k) {
+                const int d = __ldg(&g.dlist[first + k]);
+                const NodeRec<R> dn = load_node(g.node, d);
+                to_local<R, true>(c->rot, d, dn, x, w0, p, v);
+                best = rmin(best, rmax(outsideness(c->solids[dn.info & NODE_SOLID_MASK], p), (R)0));
+            }
+        }
+        safety_out[i] = best;
+    }
+}
+
 // ComputeStep + surface normal of the boundary crossed
 template <class R, bool FLAT>
 __global__ void __launch_bounds__(NAV_THREADS) step_normal_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
@@ -975,6 +1007,18 @@ extern "C" int gn_nav_compute_step_normal(const gn_geometry* geo, int precision,
     if (precision == 32) return step_normal_impl<float>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, d_normal_out, (cudaStream_t)cuda_stream);
     if (precision == 64) return step_normal_impl<double>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, d_normal_out, (cudaStream_t)cuda_stream);
     return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step_normal: precision must be 32 or 64");
+}
+
+extern "C" int gn_nav_compute_safety(const gn_geometry* geo, int precision, const void* d_pos, const int32_t* d_vol_in, int64_t n,
+                                     void* d_safety_out, void* cuda_stream) {
+    if (!geo || n < 0 || (n > 0 && (!d_pos || !d_vol_in || !d_safety_out))) return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_safety: bad argument");
+    if (precision != 32 && precision != 64) return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_safety: precision must be 32 or 64");
+    if (n == 0) return GN_OK;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (precision == 32) safety_kernel<float><<<nav_grid(n), NAV_THREADS, 0, s>>>(geo->v32, (const float*)d_pos, d_vol_in, n, (float*)d_safety_out);
+    else safety_kernel<double><<<nav_grid(n), NAV_THREADS, 0, s>>>(geo->v64, (const double*)d_pos, d_vol_in, n, (double*)d_safety_out);
+    GN_CUDA(cudaGetLastError(), "gn_nav_compute_safety launch");
+    return GN_OK;
 }
 
 template <class R> int free_path_impl(const gn_geometry* geo, const void* pos, const void* dir, const void* Y, int64_t n, double mu_mass,

@@ -56,6 +56,7 @@ template <class R> struct GeoView {
     const NodeRec<R>* node;
     const R* rot;
     const int* dlist;
+    const int* dfirst;    // node -> offset of its daughters in dlist (every node, voxelised or not; the safety scan)
     const SolidRec<R>* solids;
     const MatRec<R>* mats;
     const double* rho;    // density per material [g/cm3] (attenuation-only mode: mu = rho * mu_mass)

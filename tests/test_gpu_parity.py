@@ -107,6 +107,37 @@ def test_nav_bit_exact(B, name, precision):
     assert len(np.unique(ref)) > min(4, geom.n_places - 1) and (ref == -1).any()
 
 
+@pytest.mark.parametrize("name", list(GEOMS))
+@pytest.mark.parametrize("precision", [64, 32])
+def test_safety_bit_exact(B, name, precision):
+    """isotropic safety distance -- canonical arithmetic only (+ - * sqrt max |.|), so 0 ulp against the
+    oracle's linear scan; and no ComputeStep of the CUDA path from the same point is shorter."""
+    geom = GEOMS[name]()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    rng = np.random.default_rng(202)
+    n = 20011 if name == "phantom12" else 50021         # several blocks and a ragged tail (the oracle scans every daughter)
+    R = np.float64 if precision == 64 else np.float32
+    p = query_points(geom, rng, n).astype(R); v = unit(rng, n).astype(R)
+    tp, tv = cuda(p), cuda(v)
+    vol = B.nav_locate(g, tp, None)
+    ref_vol = og.locate(p, None, precision)
+    assert np.array_equal(vol.cpu().numpy(), ref_vol)
+    s = B.nav_compute_safety(g, tp, vol).cpu().numpy()
+    ref = og.compute_safety(p, ref_vol, precision)
+    assert np.array_equal(s, ref)
+    assert np.all(s[ref_vol < 0] == 0) and (s > 0).mean() > 0.5 and np.isfinite(s).all()
+    # arbitrary (wrong) volumes are still the same function on both sides; -1 and out-of-range give 0
+    wrong = rng.integers(-1, geom.n_places, n).astype(np.int32)
+    assert np.array_equal(B.nav_compute_safety(g, tp, cuda(wrong)).cpu().numpy(), og.compute_safety(p, wrong, precision))
+    # lower bound of every step from the same point (the volume a step starts in depends on the direction on surfaces)
+    vol_d = B.nav_locate(g, tp, tv)
+    step, _ = B.nav_compute_step(g, tp, tv, vol_d)
+    same = (vol_d == vol).cpu().numpy() & (ref_vol >= 0)
+    slack = 1e-9 if precision == 64 else 1e-3
+    assert np.all(step.cpu().numpy()[same] >= s[same] - slack)
+    assert B.nav_compute_safety(g, tp[:0], vol[:0]).numel() == 0
+
+
 def test_voxel_walk_matches_linear_scan_oracle(B):
     """The sparse lattice puts 64 solids in a voxelised vacuum world: ComputeStep from the mother walks the
     grid; the oracle's ComputeStep is the plain linear scan over all daughters."""
