@@ -58,7 +58,10 @@ typedef struct {
                                   (me c^2 each, isotropic axis, Philox stream tags 1 / 2 of the parent's id) are transported
                                   from the vertex; their steps, events, hashes and step counts are added to
                                   the parent's.  0 (default): a pair event deposits all of E locally (BASELINE.json config 1) */
-    int32_t reserved;          /* 0 */
+    int32_t refill;            /* 1: the paper's own scheduling remedy ("filling the empty places with new
+                                  particles") as one persistent kernel per batch: each lane follows its photon to the end and
+                                  then takes the next photon id from a device counter.  Same per-photon results as the default
+                                  wavefront passes (0); cannot be combined with secondaries */
 } gn_opts;
 
 /* Photon source.  axis need not be normalised. */

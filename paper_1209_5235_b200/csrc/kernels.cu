@@ -700,6 +700,127 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
 }
 
+// The paper's own remedy for threads whose particle has finished (stream compaction "and filling the empty places
+// with new particles ... some speedup"), as a persistent kernel (gn_opts.refill): every lane follows
+// its photon to the end, interactions in line, and a lane whose photon is gone takes the next photon id from a device
+// counter (one warp-aggregated atomic per refill) until the batch is used up.  Same arithmetic per photon as the
+// wavefront passes -- Philox streams are keyed by photon id, so which lane follows which photon changes nothing.
+template <class R, bool TRACK, bool FLAT>
+__global__ void __launch_bounds__(TR_THREADS)
+transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, unsigned* __restrict__ next,
+                 double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp) {
+    __shared__ BlockTables<R> tab;
+    __shared__ MatRec<R> sh_mats[MAX_SMEM_MATS];
+    __shared__ SourceDev<R> sh_src;
+    __shared__ EnergyFactors<R> sh_mono;
+    __shared__ unsigned long long sh_cnt[8];
+    __shared__ double sh_en[4];
+    stage_tables(g, tab);
+    const MatRec<R>* mats = g.mats;
+    if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
+    if (threadIdx.x == 0) { sh_src = src; if (src.energy_kind == 0) sh_mono = energy_factors(src.e0); }
+    if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
+    if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
+    __syncthreads();
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
+    const int lane = threadIdx.x & 31;
+    const SecIO<R> nosec{nullptr, nullptr, nullptr, nullptr, nullptr};
+
+    bool alive = false, exhausted = false;
+    V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0, gPE = 0, gKN = 0, L2k = 0;
+    uint32_t idx = 0, misc = 0, ctr = 0; int above = 0;
+    uint64_t h = 0;
+    int vol = -1; NodeRec<R> nd = {};
+    unsigned c_steps = 0, c_phot = 0, c_esc = 0, c_stuck = 0, c_compton = 0, c_pe = 0, c_pair = 0, c_cut = 0;
+    double e_src = 0.0, e_esc = 0.0, e_stuck = 0.0;
+#pragma unroll 1
+    for (;;) {
+        // ---- refill: lanes without a photon take the next ids ---------------------------------------------------
+        const unsigned want = __ballot_sync(0xffffffffu, !alive && !exhausted);
+        if (want) {
+            const int leader = __ffs(want) - 1;
+            unsigned base = 0;
+            if (lane == leader) base = atomicAdd(next, (unsigned)__popc(want));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (!alive && !exhausted) {
+                const unsigned i = base + __popc(want & ((1u << lane) - 1u));
+                if (i >= n_src || base >= n_src) exhausted = true;
+                else {
+                    idx = i; misc = 0; h = 0xcbf29ce484222325ull;
+                    BirthIO<R> b;
+                    birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, seed, first_id + i);
+                    x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
+                    gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
+                    ++c_phot; e_src += (double)E;
+                    vol = nav.locate(x, w, nd);
+                    if (vol < 0) { ++c_esc; e_esc += (double)E; if (TRACK) history_out(pp, nosec, idx, h, 0u, E); }
+                    else alive = true;
+                }
+            }
+        }
+        if (!__any_sync(0xffffffffu, alive || !exhausted)) break;
+        // ---- one step of Algorithm 1 (A1-A9) for every lane that has a photon -----------------------------------------
+        double dep_d = 0.0; bool has_dep = false; int dep_vol = 0;
+        if (alive) {
+            const MatRec<R> m = mats[nd.mat];
+            const R muPE = m.aPE * gPE, muC = m.aC * gKN;
+            const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
+            const R muP = (above && P > 0) ? m.aP * P : (R)0;
+            const R mu = (muPE + muC) + muP;
+            const R s_int = mu > 0 ? rdiv(Y, mu) : rinf<R>();
+            const int vol_before = vol;
+            R step; V3<R> xn;
+            nav.compute_step(vol, nd, x, w, s_int, step, xn);
+            ++c_steps; misc += 0x100u;
+            const bool inter = step == rinf<R>();
+            const R len = inter ? s_int : step;
+            uint32_t zs = misc & 0xffu;
+            zs = (len <= g.delta) ? zs + 1 : 0;
+            misc = (misc & ~0xffu) | (zs & 0xffu);
+            int ev;
+            if (inter) {
+                x = advance(x, w, s_int);
+                InteractIO<R> io;
+                io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
+                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + idx, 0u, false);
+                ev = io.ev; ctr = io.j;
+                dep_d = (double)io.dep; has_dep = true; dep_vol = vol;
+                if (ev == EV_COMPTON || ev == EV_CUT) {
+                    E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
+                    ++c_compton;
+                    if (ev == EV_CUT) { ++c_cut; alive = false; }
+                    else { Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above; }
+                } else {
+                    if (ev == EV_PE) ++c_pe; else ++c_pair;
+                    alive = false;
+                }
+            } else {
+                x = xn;
+                Y = rmax(Y - step * mu, (R)0);
+                ev = EV_BOUNDARY;
+                if (vol < 0) { ev = EV_ESCAPE; alive = false; ++c_esc; e_esc += (double)E; }
+            }
+            if (alive && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; alive = false; ++c_stuck; e_stuck += (double)E; }
+            if (TRACK) {
+                fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
+                if (!alive) history_out(pp, nosec, idx, h, misc >> 8, E);
+            }
+        }
+        if (__any_sync(0xffffffffu, has_dep)) warp_tally(edep, &sh_en[EN_DEPOSITED], dep_vol, dep_d, has_dep);
+    }
+    // ---- statistics -----------------------------------------------------------------------------------------------
+    {
+        const unsigned v[8] = {c_steps, c_compton, c_pe, c_pair, c_cut, c_esc, c_stuck, c_phot};      // ST_* order
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { unsigned t = warp_sum(v[q]); if (lane == 0 && t) atomicAdd(&sh_cnt[q], (unsigned long long)t); }
+        double a = warp_sum(e_esc), b2 = warp_sum(e_stuck), c2 = warp_sum(e_src);
+        if (lane == 0) { if (a != 0.0) atomicAdd(&sh_en[EN_ESCAPED], a); if (b2 != 0.0) atomicAdd(&sh_en[EN_STUCK], b2); if (c2 != 0.0) atomicAdd(&sh_en[EN_SOURCE], c2); }
+    }
+    __syncthreads();
+    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+}
+
 // -------------------------------------------------------------------------------------------------------
 // host side
 // -------------------------------------------------------------------------------------------------------
@@ -815,6 +936,8 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     const int K = geo->opts.steps_per_pass;
     const int K0 = std::min(K, geo->opts.first_pass_steps);      // first pass: short, sheds photons that miss
     const bool secondaries = geo->opts.secondaries > 0;        // NEXT-3: pair events leave two annihilation photons
+    const bool refill = geo->opts.refill > 0;                  // NEXT-4: persistent kernel, finished lanes take fresh photons
+    if (refill && secondaries) return fail(GN_INVALID_ARGUMENT, "gn_transport_run: gn_opts.refill and gn_opts.secondaries cannot be combined");
     const size_t cap = (size_t)std::min<int64_t>(std::max<int64_t>(n_photons, 2), TR_BATCH);
     const size_t qb = cap * sizeof(PhotonRec<R>);
     const size_t hb = (track && !d_hash) ? cap * 8 : 0;       // the hash array doubles as per-photon state between passes
@@ -927,6 +1050,25 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         const uint32_t n0 = (uint32_t)std::min<int64_t>((int64_t)cap, n_photons - done);
         const uint64_t fid = (uint64_t)(first_id + done);
         PerPhotonOut pp{d_hash ? d_hash + done : tmp_hash, d_nsteps ? d_nsteps + done : nullptr, d_efinal ? d_efinal + done : nullptr};
+        if (refill) {                                        // one persistent launch per batch: as many blocks as fit on the chip
+            unsigned* d_next = (unsigned*)((char*)d_stats + 256);
+            int per_sm = 0, sms = 0;
+            auto kern = track ? (geo->coherent ? transport_refill<R, true, false> : transport_refill<R, true, true>)
+                              : (geo->coherent ? transport_refill<R, false, false> : transport_refill<R, false, true>);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TR_THREADS, 0);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, geo->device);
+            const unsigned blocks = std::min<unsigned>((n0 + TR_THREADS - 1) / TR_THREADS, (unsigned)std::max(1, per_sm * sms));
+            cudaMemsetAsync(d_next, 0, sizeof(unsigned), s);
+            cudaEventRecord(ev0, s);
+            kern<<<blocks, TR_THREADS, 0, s>>>(g, src, seed, fid, n0, d_next, d_edep, d_stats, pp);
+            cudaEventRecord(ev1, s);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+            if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run refill"); break; }
+            { float ms = 0.f; if (cudaEventElapsedTime(&ms, ev0, ev1) == cudaSuccess) kernel_ms += ms; }
+            ++passes; ++launches;
+            continue;
+        }
         if (secondaries) cudaMemsetAsync(d_npairs, 0, sizeof(unsigned), s);
         run_batch(n0, fid, pp, SecIO<R>{d_pairs, d_npairs, nullptr, nullptr, nullptr});
         if (!secondaries || rc != GN_OK) continue;
