@@ -299,6 +299,8 @@ def run_ours(args):
         gopts["regroup_percent"] = args.regroup_percent
     if args.secondaries:
         gopts["secondaries"] = 1
+    if args.refill:
+        gopts["refill"] = 1
     geo = B.Geometry(wl.geometry, **gopts)
     transport = wl.source is not None
     dom = [0, 0.0]                                            # dominant kernel: steps taken in / summed duration of the lean step passes
@@ -430,7 +432,7 @@ def run_ours(args):
                 "config": {"workload": wl.name, "precision": precision, ("photons_per_gpu" if transport else "queries_per_gpu"): n,
                            "volumes": geo.n_places, "l2": "photon state queues (2 x %d MB) exceed the 126 MB L2; no explicit flush" % (n * (64 if precision == 32 else 112) // 10 ** 6)
                            if transport else "query arrays (%d MB) exceed the 126 MB L2" % (n * 6 * (4 if precision == 32 else 8) // 10 ** 6),
-                           "parallelism": f"dp{world} (photon-id ranges, replicated geometry)", **({"secondaries": 1} if args.secondaries else {})},
+                           "parallelism": f"dp{world} (photon-id ranges, replicated geometry)", **({"secondaries": 1} if args.secondaries else {}), **({"refill": 1} if args.refill else {})},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
                 "units_per_step": units / args.steps / world}
         print(json.dumps(line))
@@ -455,6 +457,8 @@ def main():
     ap.add_argument("--regroup-percent", type=int, default=0, help="diagnostics: override gn_opts.regroup_percent")
     ap.add_argument("--secondaries", action="store_true",
                     help="variant (not BASELINE.json's workload): gn_opts.secondaries = 1, annihilation photons of pair events are transported; no cpu_baseline leg")
+    ap.add_argument("--refill", action="store_true",
+                    help="variant: gn_opts.refill = 1, the paper's refill scheduling (PAPER.md L195) as one persistent kernel instead of the wavefront passes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-all-cores", action="store_true")
     ap.add_argument("--allow-short-warmup", action="store_true")

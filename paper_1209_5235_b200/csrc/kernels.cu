@@ -267,6 +267,7 @@ constexpr int TR_WARPS = TR_THREADS / 32;
 #ifndef TR_MIN_BLOCKS_BOX
 #define TR_MIN_BLOCKS_BOX 6      // box-only fp32 step pass: 80 registers (no spills), 24 warps / SM
 #endif
+constexpr int REFILL_BATCH = 8;       // empty lanes that trigger a warp's refill (persistent refill kernel)
 constexpr int INTERACT_BATCH = 8;     // parked lanes that trigger a warp's interaction phase
 enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
 enum : int { FATE_ALIVE = 0, FATE_ABSORBED = 1, FATE_ESCAPED = 2, FATE_STUCK = 3, FATE_NONE = 4 };
@@ -702,7 +703,7 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
 
 // The paper's own remedy for threads whose particle has finished (stream compaction "and filling the empty places
 // with new particles ... some speedup"), as a persistent kernel (gn_opts.refill): every lane follows
-// its photon to the end, interactions in line, and a lane whose photon is gone takes the next photon id from a device
+// its photon to the end (interactions batched per warp, as in the tail pass), and a lane whose photon is gone takes the next photon id from a device
 // counter (one warp-aggregated atomic per refill) until the batch is used up.  Same arithmetic per photon as the
 // wavefront passes -- Philox streams are keyed by photon id, so which lane follows which photon changes nothing.
 template <class R, bool TRACK, bool FLAT>
@@ -726,7 +727,7 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     const int lane = threadIdx.x & 31;
     const SecIO<R> nosec{nullptr, nullptr, nullptr, nullptr, nullptr};
 
-    bool alive = false, exhausted = false;
+    bool alive = false, exhausted = false, pending = false;      // pending: parked at its interaction point
     V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0, gPE = 0, gKN = 0, L2k = 0;
     uint32_t idx = 0, misc = 0, ctr = 0; int above = 0;
     uint64_t h = 0;
@@ -736,8 +737,9 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
 #pragma unroll 1
     for (;;) {
         // ---- refill: lanes without a photon take the next ids ---------------------------------------------------
+        // (batched like the interactions: birth + locate of a few lanes stalls the rest of the warp)
         const unsigned want = __ballot_sync(0xffffffffu, !alive && !exhausted);
-        if (want) {
+        if (want && (__popc(want) >= REFILL_BATCH || !__any_sync(0xffffffffu, alive))) {
             const int leader = __ffs(want) - 1;
             unsigned base = 0;
             if (lane == leader) base = atomicAdd(next, (unsigned)__popc(want));
@@ -759,9 +761,44 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
             }
         }
         if (!__any_sync(0xffffffffu, alive || !exhausted)) break;
-        // ---- one step of Algorithm 1 (A1-A9) for every lane that has a photon -----------------------------------------
-        double dep_d = 0.0; bool has_dep = false; int dep_vol = 0;
-        if (alive) {
+        // ---- interaction phase (A6-A9): lanes parked at their interaction points, batched per warp as in the tail pass ----
+        const unsigned pen = __ballot_sync(0xffffffffu, alive && pending);
+        const unsigned act = __ballot_sync(0xffffffffu, alive && !pending);
+        if (pen && (act == 0 || __popc(pen) >= INTERACT_BATCH)) {
+            double dep_d = 0.0;
+            const bool was = alive && pending;
+            if (was) {
+                const MatRec<R> m = mats[nd.mat];
+                const R muPE = m.aPE * gPE, muC = m.aC * gKN;
+                const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
+                const R muP = (above && P > 0) ? m.aP * P : (R)0;
+                const R mu = (muPE + muC) + muP;
+                InteractIO<R> io;
+                io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
+                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + idx, 0u, false);
+                int ev = io.ev; ctr = io.j;
+                dep_d = (double)io.dep;
+                if (ev == EV_COMPTON || ev == EV_CUT) {
+                    E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
+                    ++c_compton;
+                    if (ev == EV_CUT) { ++c_cut; alive = false; }
+                    else { Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above; }
+                } else {
+                    if (ev == EV_PE) ++c_pe; else ++c_pair;
+                    alive = false;
+                }
+                if (alive && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; alive = false; ++c_stuck; e_stuck += (double)E; }
+                if (TRACK) {
+                    fnv_word(h, (uint32_t)vol); fnv_word(h, (uint32_t)ev);
+                    if (!alive) history_out(pp, nosec, idx, h, misc >> 8, E);
+                }
+                pending = false;
+            }
+            warp_tally(edep, &sh_en[EN_DEPOSITED], vol, dep_d, was);
+            continue;
+        }
+        // ---- one navigation step (A1-A5) for every travelling lane ----------------------------------------------------
+        if (alive && !pending) {
             const MatRec<R> m = mats[nd.mat];
             const R muPE = m.aPE * gPE, muC = m.aC * gKN;
             const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
@@ -777,36 +814,21 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
             uint32_t zs = misc & 0xffu;
             zs = (len <= g.delta) ? zs + 1 : 0;
             misc = (misc & ~0xffu) | (zs & 0xffu);
-            int ev;
             if (inter) {
                 x = advance(x, w, s_int);
-                InteractIO<R> io;
-                io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
-                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + idx, 0u, false);
-                ev = io.ev; ctr = io.j;
-                dep_d = (double)io.dep; has_dep = true; dep_vol = vol;
-                if (ev == EV_COMPTON || ev == EV_CUT) {
-                    E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
-                    ++c_compton;
-                    if (ev == EV_CUT) { ++c_cut; alive = false; }
-                    else { Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above; }
-                } else {
-                    if (ev == EV_PE) ++c_pe; else ++c_pair;
-                    alive = false;
-                }
+                pending = true;
             } else {
                 x = xn;
                 Y = rmax(Y - step * mu, (R)0);
-                ev = EV_BOUNDARY;
+                int ev = EV_BOUNDARY;
                 if (vol < 0) { ev = EV_ESCAPE; alive = false; ++c_esc; e_esc += (double)E; }
-            }
-            if (alive && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; alive = false; ++c_stuck; e_stuck += (double)E; }
-            if (TRACK) {
-                fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
-                if (!alive) history_out(pp, nosec, idx, h, misc >> 8, E);
+                if (alive && (misc & 0xffu) >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; alive = false; ++c_stuck; e_stuck += (double)E; }
+                if (TRACK) {
+                    fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev);
+                    if (!alive) history_out(pp, nosec, idx, h, misc >> 8, E);
+                }
             }
         }
-        if (__any_sync(0xffffffffu, has_dep)) warp_tally(edep, &sh_en[EN_DEPOSITED], dep_vol, dep_d, has_dep);
     }
     // ---- statistics -----------------------------------------------------------------------------------------------
     {

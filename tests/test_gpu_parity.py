@@ -369,6 +369,29 @@ def test_secondary_photons_without_per_photon_outputs_and_below_threshold(B):
     assert int(e["hash"].cpu().numpy().view(np.uint64)[0]) == int(r["hash"][0])
 
 
+@pytest.mark.parametrize("name", list(TRANSPORT_CASES))
+def test_refill_kernel_same_histories(B, name):
+    """SURVEY 8(f) NEXT-4 / PAPER.md L195: the persistent refill kernel (gn_opts.refill) follows the same photons with the
+    same Philox streams as the wavefront passes -- identical fp64 histories against the oracle, same statistics as the default path."""
+    geom, src, n, seed = TRANSPORT_CASES[name]()
+    got, ref, frac = compare_transport(B, geom, src, n, seed, 64, 0.999, opts=dict(refill=1))
+    assert got["stats"]["n_kernel_launches"] == 1
+    d = B.transport_run(B.Geometry(geom), src, seed, n, 64, per_photon=True)
+    assert np.array_equal(d["hash"].cpu().numpy(), got["hash"].cpu().numpy())
+    for k in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons"):
+        assert d["stats"][k] == got["stats"][k], k
+    assert np.allclose(d["edep"].cpu().numpy(), got["edep"].cpu().numpy(), rtol=1e-12, atol=1e-12)
+    # fp32, untracked kernels, more photons than lanes on the chip (every lane refills many times)
+    g = B.Geometry(geom, refill=1)
+    a = B.transport_run(g, src, seed, 400000, 32)
+    b = B.transport_run(B.Geometry(geom), src, seed, 400000, 32)
+    for k in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons"):
+        assert a["stats"][k] == b["stats"][k], k
+    assert np.allclose(a["edep"].cpu().numpy(), b["edep"].cpu().numpy(), rtol=1e-9, atol=1e-9)
+    with pytest.raises(Exception):
+        B.transport_run(B.Geometry(geom, refill=1, secondaries=1), src, seed, 100, 64)
+
+
 def test_transport_is_independent_of_steps_per_pass_and_sharding(B):
     import torch
     geom, src, n, seed = TRANSPORT_CASES["phantom16"]()
