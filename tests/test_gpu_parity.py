@@ -363,6 +363,12 @@ def test_secondary_photons_without_per_photon_outputs_and_below_threshold(B):
     assert np.array_equal(c["hash"].cpu().numpy(), d["hash"].cpu().numpy())
     assert np.allclose(c["edep"].cpu().numpy(), d["edep"].cpu().numpy(), rtol=1e-12, atol=1e-12)      # fp64 atomics: order of the adds
     assert d["stats"]["n_pair"] == 0 and d["stats"]["n_steps"] == c["stats"]["n_steps"]
+    # sharding by photon-id ranges (the multi-GPU split): secondaries follow their parents' ids
+    lo = B.transport_run(g1, src, seed, 7000, 64, first_photon_id=0, per_photon=True)
+    hi = B.transport_run(g1, src, seed, n - 7000, 64, first_photon_id=7000, per_photon=True)
+    assert np.array_equal(np.concatenate([lo["hash"].cpu().numpy(), hi["hash"].cpu().numpy()]), a["hash"].cpu().numpy())
+    assert np.array_equal(np.concatenate([lo["nsteps"].cpu().numpy(), hi["nsteps"].cpu().numpy()]), a["nsteps"].cpu().numpy())
+    assert np.allclose((lo["edep"] + hi["edep"]).cpu().numpy(), a["edep"].cpu().numpy(), rtol=1e-12, atol=1e-12)
     # one photon (queue capacity 2): its pair, if any, still fits
     e = B.transport_run(g1, _pencil(8.0), seed, 1, 64, per_photon=True)
     r = oracle.OracleGeometry(geom, secondaries=1).transport(_pencil(8.0), seed, 1, 64, per_photon=True)
