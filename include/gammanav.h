@@ -171,6 +171,11 @@ int gn_nav_compute_safety(const gn_geometry* geo, int precision, const void* d_p
  *   d_hash_out    n uint64 history hashes (FNV-1a-64 over (volume, event) per step), or NULL
  *   d_nsteps_out  n uint32 steps per photon, or NULL
  *   d_efinal_out  n doubles: photon energy when it terminated, or NULL
+ * With gn_opts.secondaries = 1 a photon's hash and step count are the sums (wrapping, order-independent) over itself and the
+ * two annihilation photons of its pair event, d_efinal_out stays the primary's own energy at its end, and the counters of
+ * h_stats_out count every photon followed except n_photons / e_source (primaries only); scratch grows by one pair-vertex
+ * list (16 / 32 B per photon of a batch).  gn_opts.refill = 1 runs the same histories in one persistent kernel per batch
+ * (no queues are used); combining it with secondaries returns GN_INVALID_ARGUMENT.
  * Scratch (two photon-state queues, 2 x min(n, 2^24) x 64 B in fp32 / 112 B in fp64, plus counters) belongs to
  * the geometry handle: grown on demand, reused by later runs, released by gn_geometry_destroy.  Runs on one
  * handle are serialised (internal mutex); use one handle per stream for concurrent runs.
