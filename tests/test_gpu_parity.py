@@ -455,6 +455,31 @@ def test_batching_across_the_queue_capacity(B):
     assert got["stats"]["n_photons"] == n and int(got["nsteps"].sum().item()) == got["stats"]["n_steps"]
 
 
+def test_batching_across_the_queue_capacity_with_secondaries(B):
+    """Two batches of primaries, each followed by its own batches of annihilation photons (the pair-vertex list is reused
+    per batch; 20 MeV in lead: more pairs than half a queue, so the secondaries of the first batch need two chunks)."""
+    geom, src, _, seed = SECONDARY_CASES["lead_slab_20MeV"]()
+    g = B.Geometry(geom, secondaries=1)
+    n = (1 << 24) + 30000
+    got = B.transport_run(g, src, seed, n, 64, per_photon=True)
+    og = oracle.OracleGeometry(geom, secondaries=1)
+    first = (1 << 24) - 15000
+    ref = og.transport(src, seed, 30000, 64, first_id=first, per_photon=True)
+    hg = got["hash"][first:first + 30000].cpu().numpy().view(np.uint64)
+    ng = got["nsteps"][first:first + 30000].cpu().numpy().astype(np.uint32)
+    assert ((hg == ref["hash"]) & (ng == ref["nsteps"])).mean() >= 0.999
+    s = got["stats"]
+    assert s["n_photons"] == n and 2 * s["n_pair"] > n and int(got["nsteps"].to(torch_int64()).sum().item()) == s["n_steps"]
+    assert s["n_pe"] + s["n_pair"] + s["n_cut"] + s["n_escaped"] + s["n_stuck"] == n + 2 * s["n_pair"]
+    book = float(got["edep"].sum()) + s["e_escaped"] + s["e_stuck"]
+    assert abs(book / s["e_source"] - 1) < 1e-9
+
+
+def torch_int64():
+    import torch
+    return torch.int64
+
+
 # ---- BASELINE.json full-size geometries, in the launch configuration bench.py times ---------------------------
 def test_config3_full_size_sampled(B):
     """Config 3 as bench.py runs it (64^3 voxels, 1e7 photons, fp32): oracle on a sampled id range; book-keeping,
