@@ -739,7 +739,7 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
         // ---- refill: lanes without a photon take the next ids ---------------------------------------------------
         // (batched like the interactions: birth + locate of a few lanes stalls the rest of the warp)
         const unsigned want = __ballot_sync(0xffffffffu, !alive && !exhausted);
-        if (want && (__popc(want) >= REFILL_BATCH || !__any_sync(0xffffffffu, alive))) {
+        if (want && (FLAT || __popc(want) >= REFILL_BATCH || !__any_sync(0xffffffffu, alive))) {      // general geometries: warps are thin anyway, refill at once
             const int leader = __ffs(want) - 1;
             unsigned base = 0;
             if (lane == leader) base = atomicAdd(next, (unsigned)__popc(want));
@@ -1014,6 +1014,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     // parents' pair vertices), passes until none is left; ends with a stream synchronise
     auto run_batch = [&](uint32_t n0, uint64_t fid, PerPhotonOut pp, SecIO<R> sec) {
         PhotonRec<R>* in = qb_; PhotonRec<R>* out = qa;
+        const int k_first = sec.in ? K : K0;                      // annihilation photons are born inside the detector: no short first pass
         cudaMemsetAsync(d_ctr, 0, cb, s);
         if (sorted) cudaMemsetAsync(d_kctr, 0, kb, s);
         cudaEventRecord(ev0, s);
@@ -1033,8 +1034,8 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
             // FLAT = general geometry (any solid, rotations, long candidate lists); !FLAT = unrotated boxes only (geo->coherent)
             if (p == 0) {
-                if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup, sec);
-                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K0, regroup, sec, SortIO{d_kctr + 1, d_keys, nullptr});
+                if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, k_first, regroup, sec);
+                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, k_first, regroup, sec, SortIO{d_kctr + 1, d_keys, nullptr});
             } else if (last) {
                 if (geo->coherent) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec);
                 else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec, SortIO{nullptr, nullptr, d_perm});
