@@ -21,13 +21,23 @@ def _free_port():
     s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close(); return p
 
 
-def _worker(rank, world, port, q):
+def _case(secondaries):
+    """config 1 as it stands, or -- secondaries -- its geometry under an 8 MeV beam with the annihilation photons followed
+    (a photon's secondaries stay on the rank that owns its id)."""
+    wl = W.config(1)
+    if not secondaries:
+        return wl.geometry, wl.source, {}
+    return wl.geometry, W.Source(W.SRC_PENCIL, (0.0, 0.0, -500.0), (0.0, 0.0, 1.0), W.E_MONO, 8.0), dict(secondaries=1)
+
+
+def _worker(rank, world, port, q, secondaries=False):
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     wl = W.config(1)
-    og = oracle.OracleGeometry(wl.geometry)
+    geom, source, opts = _case(secondaries)
+    og = oracle.OracleGeometry(geom, **opts)
     first, count = shard_range(N, rank, world)
-    r = og.transport(wl.source, wl.seed, count, 64, first_id=first)
+    r = og.transport(source, wl.seed, count, 64, first_id=first)
     edep, stats = allreduce_tally(torch.from_numpy(r["edep"]), r["stats"])
     if rank == 0:
         q.put((edep.numpy().copy(), stats))
@@ -36,11 +46,12 @@ def _worker(rank, world, port, q):
 
 
 @pytest.mark.timeout(180)
-def test_two_rank_sharded_run_equals_single_run():
+@pytest.mark.parametrize("secondaries", [False, True])
+def test_two_rank_sharded_run_equals_single_run(secondaries):
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, secondaries)) for r in range(2)]
     for p in procs:
         p.start()
     edep, stats = q.get(timeout=150)
@@ -48,8 +59,11 @@ def test_two_rank_sharded_run_equals_single_run():
         p.join(timeout=60)
         assert p.exitcode == 0
     wl = W.config(1)
-    ref = oracle.OracleGeometry(wl.geometry).transport(wl.source, wl.seed, N, 64)
+    geom, source, opts = _case(secondaries)
+    ref = oracle.OracleGeometry(geom, **opts).transport(source, wl.seed, N, 64)
     assert np.allclose(edep, ref["edep"], rtol=1e-12, atol=0)
-    for k in ("n_steps", "n_compton", "n_pe", "n_escaped", "n_photons"):
+    for k in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_photons"):
         assert stats[k] == ref["stats"][k]
+    if secondaries:
+        assert stats["n_pair"] > 50
     assert abs(stats["e_source"] - ref["stats"]["e_source"]) < 1e-9
