@@ -45,6 +45,8 @@ def lib():
         L.oracle_sigma_pe.restype = C.c_double; L.oracle_sigma_pe.argtypes = [C.c_double, C.c_double, C.c_double]
         L.oracle_uniform_from_lane.restype = C.c_double; L.oracle_uniform_from_lane.argtypes = [C.c_uint64, C.c_int]
         L.oracle_draw.restype = C.c_double; L.oracle_draw.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_int]
+        L.oracle_fnv1a_bytes.restype = C.c_uint64; L.oracle_fnv1a_bytes.argtypes = [C.c_void_p, C.c_int64]
+        L.oracle_history_hash.restype = C.c_uint64; L.oracle_history_hash.argtypes = [C.c_void_p, C.c_int64]
         _lib = L
     return _lib
 
@@ -131,18 +133,44 @@ class OracleGeometry:
         _check(lib().oracle_nav_compute_safety(self._h, C.c_int(precision), _p(pos), _p(vol), C.c_int64(pos.shape[0]), _p(out)), "nav_compute_safety")
         return out
 
-    def transport(self, src, seed, n, precision=64, first_id=0, per_photon=False, use_grid=True):
+    def transport(self, src, seed, n, precision=64, first_id=0, per_photon=False, use_grid=True, tally=False):
+        """tally=True adds per volume the sum of the squared deposits and the number of deposits (edep_sq, n_dep)."""
         edep = np.zeros(self.n_places, np.float64); st = Stats()
         h = np.empty(n, np.uint64) if per_photon else None
         ns = np.empty(n, np.uint32) if per_photon else None
         ef = np.empty(n, np.float64) if per_photon else None
+        sq = np.zeros(self.n_places, np.float64) if tally else None
+        nd = np.zeros(self.n_places, np.uint32) if tally else None
         cs = _csource(src)
-        _check(lib().oracle_transport_run(self._h, C.c_int(precision), C.byref(cs), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n),
-                                          _p(edep), C.byref(st), _p(h), _p(ns), _p(ef), C.c_int(int(use_grid))), "transport_run")
+        _check(lib().oracle_transport_run_tally(self._h, C.c_int(precision), C.byref(cs), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n),
+                                                _p(edep), _p(sq), _p(nd), C.byref(st), _p(h), _p(ns), _p(ef), C.c_int(int(use_grid))), "transport_run")
         out = {"edep": edep, "stats": st.as_dict()}
         if per_photon:
             out.update(hash=h, nsteps=ns, efinal=ef)
+        if tally:
+            out.update(edep_sq=sq, n_dep=nd)
         return out
+
+    OP_NAMES = ("add", "mul", "div", "sqrt", "cmp", "fma", "trans", "flops")
+
+    def transport_count_ops(self, src, seed, n, first_id=0):
+        """Operation counts of n histories (S:8(d) instrumented oracle) -> (dict of counts, stats)."""
+        c = np.zeros(8, np.uint64); st = Stats(); cs = _csource(src)
+        _check(lib().oracle_transport_count_ops(self._h, C.byref(cs), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n), _p(c), C.byref(st)), "transport_count_ops")
+        return dict(zip(self.OP_NAMES, (int(v) for v in c))), st.as_dict()
+
+    def nav_count_ops(self, pos, dirs):
+        """Operation counts of len(pos) navigation queries (locate, then ComputeStep)."""
+        pos = np.ascontiguousarray(pos, np.float64); dirs = np.ascontiguousarray(dirs, np.float64)
+        c = np.zeros(8, np.uint64)
+        _check(lib().oracle_nav_count_ops(self._h, _p(pos), _p(dirs), C.c_int64(pos.shape[0]), _p(c)), "nav_count_ops")
+        return dict(zip(self.OP_NAMES, (int(v) for v in c)))
+
+    def composed_transforms(self, precision=64):
+        """Global->local (M row-major, T) of every node as stored for `precision` (test hook, S:C0)."""
+        M = np.empty((self.n_places, 9)); T = np.empty((self.n_places, 3))
+        _check(lib().oracle_composed_transforms(self._h, C.c_int(precision), _p(M), _p(T)), "composed_transforms")
+        return M, T
 
     def free_path(self, pos, dirs, Y, mu_mass, precision=64, use_grid=True):
         """The paper's benchmark (Algorithm 2 phase 5): T_i from (x0, w, Y)_i, attenuation only.  -> (T, nsteps)."""
@@ -190,6 +218,25 @@ def pair_directions(seed, first_id, n, precision=64):
     w1 = np.empty((n, 3), np.float64); w2 = np.empty((n, 3), np.float64)
     _check(lib().oracle_pair_directions(C.c_int(precision), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n), _p(w1), _p(w2)), "pair_directions")
     return w1, w2
+
+
+def fnv1a_bytes(data: bytes) -> int:
+    """FNV-1a-64 of a byte string through the oracle's own byte step (test hook for the history hash, S:C9)."""
+    buf = np.frombuffer(bytes(data), np.uint8) if len(data) else np.zeros(0, np.uint8)
+    return int(lib().oracle_fnv1a_bytes(_p(np.ascontiguousarray(buf)) if len(buf) else None, C.c_int64(len(buf))))
+
+
+def history_hash(words) -> int:
+    """History hash of a list of 32-bit words (vol_before, event, vol_before, event, ...)."""
+    w = np.ascontiguousarray(np.asarray(words, dtype=np.int64) & 0xffffffff, np.uint32)
+    return int(lib().oracle_history_hash(_p(w) if len(w) else None, C.c_int64(len(w))))
+
+
+def source_frame(src, precision=64):
+    """(a, e1, e2) of a source as rounded to `precision` (D:reading 4)."""
+    out = np.empty(9); cs = _csource(src)
+    _check(lib().oracle_source_frame(C.byref(cs), C.c_int(precision), _p(out)), "source_frame")
+    return out.reshape(3, 3)
 
 
 def philox(counter, key):

@@ -50,6 +50,52 @@ template <class R> inline R r_abs(R a) { return std::fabs(a); }
 template <class R> inline R r_sqrt(R a) { return std::sqrt(a); }
 template <class R> inline R r_max(R a, R b) { return a > b ? a : b; }
 template <class R> inline R r_min(R a, R b) { return a < b ? a : b; }
+/* transcendental functions (physics only; navigation never calls them, S:C0) */
+template <class R> inline R r_log(R a) { return std::log(a); }
+template <class R> inline R r_exp(R a) { return std::exp(a); }
+template <class R> inline R r_cos(R a) { return std::cos(a); }
+template <class R> inline R r_sin(R a) { return std::sin(a); }
+template <class R> inline R r_pow(R a, R b) { return std::pow(a, b); }
+
+/* ---- operation counter (S:8(d) "instrumented oracle") -------------------------------------------------
+ * Counted is a third `Real`: a double whose every operation also bumps a counter, so that one run of the SAME
+ * templates gives the algorithmic flops of the workload: + - * / sqrt, compare / min / max / |.| = 1 each,
+ * fma = 2, every transcendental = 1 (S:8(d): "a deliberately low count").  Values are plain fp64, so a counted
+ * run follows exactly the fp64 histories.  Unary minus, copies and integer index arithmetic are not counted. */
+struct OpCounts { uint64_t add, mul, div, sqrt, cmp, fma, trans; };
+OpCounts g_ops = {0, 0, 0, 0, 0, 0, 0};
+struct Counted {
+    double v;
+    Counted() = default;
+    Counted(double x) : v(x) {}
+    explicit operator double() const { return v; }
+    Counted operator-() const { return Counted(-v); }
+    friend Counted operator+(Counted a, Counted b) { ++g_ops.add; return Counted(a.v + b.v); }
+    friend Counted operator-(Counted a, Counted b) { ++g_ops.add; return Counted(a.v - b.v); }
+    friend Counted operator*(Counted a, Counted b) { ++g_ops.mul; return Counted(a.v * b.v); }
+    friend Counted operator/(Counted a, Counted b) { ++g_ops.div; return Counted(a.v / b.v); }
+    friend bool operator<(Counted a, Counted b) { ++g_ops.cmp; return a.v < b.v; }
+    friend bool operator>(Counted a, Counted b) { ++g_ops.cmp; return a.v > b.v; }
+    friend bool operator<=(Counted a, Counted b) { ++g_ops.cmp; return a.v <= b.v; }
+    friend bool operator>=(Counted a, Counted b) { ++g_ops.cmp; return a.v >= b.v; }
+    friend bool operator==(Counted a, Counted b) { ++g_ops.cmp; return a.v == b.v; }
+    friend bool operator!=(Counted a, Counted b) { ++g_ops.cmp; return a.v != b.v; }
+};
+template <> inline Counted r_inf<Counted>() { return Counted(std::numeric_limits<double>::infinity()); }
+template <> inline Counted r_fma<Counted>(Counted a, Counted b, Counted c) { ++g_ops.fma; return Counted(std::fma(a.v, b.v, c.v)); }
+template <> inline Counted r_abs<Counted>(Counted a) { ++g_ops.cmp; return Counted(std::fabs(a.v)); }
+template <> inline Counted r_sqrt<Counted>(Counted a) { ++g_ops.sqrt; return Counted(std::sqrt(a.v)); }
+template <> inline Counted r_log<Counted>(Counted a) { ++g_ops.trans; return Counted(std::log(a.v)); }
+template <> inline Counted r_exp<Counted>(Counted a) { ++g_ops.trans; return Counted(std::exp(a.v)); }
+template <> inline Counted r_cos<Counted>(Counted a) { ++g_ops.trans; return Counted(std::cos(a.v)); }
+template <> inline Counted r_sin<Counted>(Counted a) { ++g_ops.trans; return Counted(std::sin(a.v)); }
+template <> inline Counted r_pow<Counted>(Counted a, Counted b) { ++g_ops.trans; return Counted(std::pow(a.v, b.v)); }
+/* the type in which the energy-dependent factors of mu are evaluated (D:"mu factorisation": fp64 in both precision modes) */
+template <class R> struct Wide { typedef double type; };
+template <> struct Wide<Counted> { typedef Counted type; };
+/* operations done in plain double inside an accelerator (grid index arithmetic): counted by hand */
+template <class R> inline void note_ops(uint64_t, uint64_t) {}
+template <> inline void note_ops<Counted>(uint64_t adds, uint64_t muls) { g_ops.add += adds; g_ops.mul += muls; }
 
 /* ---- geometry store ------------------------------------------------------------------- */
 struct SolidD {            /* as given (fp64) */
@@ -81,6 +127,7 @@ struct Geo {
     std::vector<XformR<double>> x64; std::vector<XformR<float>> x32;
     std::vector<SolidR<double>> s64; std::vector<SolidR<float>> s32;
     std::vector<MaterialR<double>> m64; std::vector<MaterialR<float>> m32;
+    std::vector<XformR<Counted>> xc; std::vector<SolidR<Counted>> sc; std::vector<MaterialR<Counted>> mc;   /* copies of the fp64 tables for the operation counter */
     std::vector<int> grid_of;                /* node -> index in grids or -1 */
     std::vector<Grid> grids;
     double tol64, tol32, sigma_pe0, e_cut; int stuck_limit, grid_min, secondaries;
@@ -92,6 +139,12 @@ template <> struct Sel<double> {
     static const std::vector<SolidR<double>>& s(const Geo& g) { return g.s64; }
     static const std::vector<MaterialR<double>>& m(const Geo& g) { return g.m64; }
     static double tol(const Geo& g) { return g.tol64; }
+};
+template <> struct Sel<Counted> {
+    static const std::vector<XformR<Counted>>& x(const Geo& g) { return g.xc; }
+    static const std::vector<SolidR<Counted>>& s(const Geo& g) { return g.sc; }
+    static const std::vector<MaterialR<Counted>>& m(const Geo& g) { return g.mc; }
+    static Counted tol(const Geo& g) { return Counted(g.tol64); }
 };
 template <> struct Sel<float> {
     static const std::vector<XformR<float>>& x(const Geo& g) { return g.x32; }
@@ -490,6 +543,7 @@ template <class R> struct Navigator {
                 const Grid& G = g.grids[gi];
                 R p[3]; local_point(cur, x, p);
                 int c[3];
+                note_ops<R>(3, 3);                       /* (p - gmin) * inv_w per axis, in plain double below */
                 for (int k = 0; k < 3; ++k) {
                     double f = std::floor(((double)p[k] - G.gmin[k]) * G.inv_w[k]);
                     c[k] = (int)std::min(std::max(f, 0.0), (double)(G.n[k] - 1));
@@ -574,13 +628,14 @@ template <class R> struct Navigator {
 
 /* ---- physics (S:C6) -------------------------------------------------------------------- */
 /* Klein-Nishina total cross-section per electron, cm^2 */
-double sigma_kn(double k) {
-    double l = std::log(1.0 + 2.0 * k);
-    double t1 = (1.0 + k) / (k * k) * (2.0 * (1.0 + k) / (1.0 + 2.0 * k) - l / k);
-    double t2 = l / (2.0 * k);
-    double t3 = (1.0 + 3.0 * k) / ((1.0 + 2.0 * k) * (1.0 + 2.0 * k));
-    return 2.0 * kPi * kRe * kRe * (t1 + t2 - t3);
+template <class W> W sigma_kn_over_2pire2(W k) {          /* sigma_KN / (2 pi r_e^2), S:C6 closed form */
+    W l = r_log<W>(W(1.0) + W(2.0) * k);
+    W t1 = (W(1.0) + k) / (k * k) * (W(2.0) * (W(1.0) + k) / (W(1.0) + W(2.0) * k) - l / k);
+    W t2 = l / (W(2.0) * k);
+    W t3 = (W(1.0) + W(3.0) * k) / ((W(1.0) + W(2.0) * k) * (W(1.0) + W(2.0) * k));
+    return t1 + t2 - t3;
 }
+double sigma_kn(double k) { return 2.0 * kPi * kRe * kRe * sigma_kn_over_2pire2<double>(k); }
 double pair_cap(double Z) { return (28.0 / 9.0) * std::log(183.0 * std::pow(Z, -1.0 / 3.0)) - 2.0 / 27.0; }
 double sigma_pair(double k, double Z) {
     if (!(k > 2.0)) return 0.0;
@@ -596,12 +651,14 @@ double sigma_pe(double E, double Z, double s0_barn) {
  * the sum are in Real.  In fp64 mode this is the closed form of S:C6 evaluated in a fixed order. */
 template <class R> struct EnergyFactors { R gPE, gKN, L2k; bool above_pair; };
 template <class R> EnergyFactors<R> energy_factors(R E) {
-    double e = (double)E, k = e / kMeC2;
+    typedef typename Wide<R>::type W;
+    W e = W((double)E), k = e / W(kMeC2);
     EnergyFactors<R> f;
-    f.gPE = (R)std::pow(0.1 / e, 3.5);
-    f.gKN = (R)(sigma_kn(k) / (2.0 * kPi * kRe * kRe));
-    f.L2k = (R)std::log(2.0 * k);
-    f.above_pair = k > 2.0;
+    f.gPE = (R)(double)r_pow<W>(W(0.1) / e, W(3.5));
+    const W two_pi_re2(2.0 * kPi * kRe * kRe);
+    f.gKN = (R)(double)((two_pi_re2 * sigma_kn_over_2pire2<W>(k)) / two_pi_re2);      /* sigma_KN(k) / (2 pi r_e^2), as D:reading 1 writes it */
+    f.L2k = (R)(double)r_log<W>(W(2.0) * k);
+    f.above_pair = k > W(2.0);
     return f;
 }
 template <class R> void mu_partials(const MaterialR<R>& m, const EnergyFactors<R>& f, R mu[3]) {
@@ -627,6 +684,7 @@ void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
 template <class R> R uniform_from_lane(uint64_t lane);
 template <> double uniform_from_lane<double>(uint64_t lane) { return (double)((lane >> 11) + 1) * 0x1p-53; }
 template <> float uniform_from_lane<float>(uint64_t lane) { return (float)((lane >> 40) + 1) * 0x1p-24f; }
+template <> Counted uniform_from_lane<Counted>(uint64_t lane) { ++g_ops.mul; return Counted((double)((lane >> 11) + 1) * 0x1p-53); }
 
 struct Stream {      /* draw j of photon id: lane (j mod 2) of block j/2; tag 0 = the primary, 1 / 2 = its annihilation photons */
     uint64_t seed, id; uint32_t j; uint32_t tag = 0;
@@ -645,7 +703,7 @@ struct Stream {      /* draw j of photon id: lane (j mod 2) of block j/2; tag 0 
 template <class R> int kn_sample(R E, Stream& rng, R& eps, R& cost, R& sint2) {
     R k = E / (R)kMeC2;
     R eps0 = (R)1 / ((R)1 + (R)2 * k);
-    R a1 = -std::log(eps0);
+    R a1 = -r_log(eps0);
     R eps0sq = eps0 * eps0;
     R a2 = ((R)1 - eps0sq) / (R)2;
     int trials = 0;
@@ -653,7 +711,7 @@ template <class R> int kn_sample(R E, Stream& rng, R& eps, R& cost, R& sint2) {
         ++trials;
         R u1 = rng.u<R>(), u2 = rng.u<R>(), u3 = rng.u<R>();
         R e, e2;
-        if (u1 < a1 / (a1 + a2)) { e = std::exp(-a1 * u2); e2 = e * e; }
+        if (u1 < a1 / (a1 + a2)) { e = r_exp(-a1 * u2); e2 = e * e; }
         else { e2 = eps0sq + ((R)1 - eps0sq) * u2; e = r_sqrt(e2); }
         R t = ((R)1 - e) / (k * e);
         R s2 = t * ((R)2 - t);
@@ -662,7 +720,7 @@ template <class R> int kn_sample(R E, Stream& rng, R& eps, R& cost, R& sint2) {
 }
 /* direction update */
 template <class R> void rotate_dir(R w[3], R cost, R sint, R phi) {
-    R cp = std::cos(phi), sp = std::sin(phi);
+    R cp = r_cos(phi), sp = r_sin(phi);
     R u = w[0], v = w[1], ww = w[2];
     R s2 = u * u + v * v;
     R n[3];
@@ -712,28 +770,32 @@ template <class R> void sample_source(const SourceR<R>& s, Stream& rng, R x[3], 
     for (int i = 0; i < 3; ++i) { x[i] = s.o[i]; w[i] = s.a[i]; }
     if (s.kind == ORACLE_SRC_GAUSS_PENCIL) {
         R u0 = rng.u<R>(), u1 = rng.u<R>();
-        R r = s.sigma * r_sqrt((R)-2 * std::log(u0));
+        R r = s.sigma * r_sqrt((R)-2 * r_log(u0));
         R phi = twopi * u1;
-        R gx = r * std::cos(phi), gy = r * std::sin(phi);
+        R gx = r * r_cos(phi), gy = r * r_sin(phi);
         for (int i = 0; i < 3; ++i) x[i] = s.o[i] + (gx * s.e1[i] + gy * s.e2[i]);
     } else if (s.kind == ORACLE_SRC_CONE || s.kind == ORACLE_SRC_ISOTROPIC) {
         R u0 = rng.u<R>(), u1 = rng.u<R>();
         R ct = (s.kind == ORACLE_SRC_CONE) ? (R)1 - u0 * ((R)1 - s.cos_half) : (R)1 - (R)2 * u0;
         R st = r_sqrt(r_max(((R)1 - ct) * ((R)1 + ct), (R)0));
         R phi = twopi * u1;
-        R cx = st * std::cos(phi), cy = st * std::sin(phi);
+        R cx = st * r_cos(phi), cy = st * r_sin(phi);
         R n[3];
         for (int i = 0; i < 3; ++i) n[i] = (cx * s.e1[i] + cy * s.e2[i]) + ct * s.a[i];
         R nn = r_sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
         for (int i = 0; i < 3; ++i) w[i] = n[i] / nn;
     }
-    if (s.energy_kind == ORACLE_E_LOGUNIFORM) E = std::exp(s.ln_e0 + rng.u<R>() * s.ln_ratio);
+    if (s.energy_kind == ORACLE_E_LOGUNIFORM) E = r_exp(s.ln_e0 + rng.u<R>() * s.ln_ratio);
     else E = s.e0;
 }
 
 /* ---- transport loop (Algorithm 1 generalised, S:C9) ---------------------------- */
+/* History hash (S:C9): FNV-1a, 64 bit -- offset basis 0xcbf29ce484222325, per byte h = (h xor byte) * 0x100000001b3 mod 2^64 --
+ * over the bytes of the 32-bit words (vol_before, event) of every step, least significant byte first. */
+const uint64_t kFnvOffset = 0xcbf29ce484222325ull, kFnvPrime = 0x100000001b3ull;
+inline void fnv_byte(uint64_t& h, uint8_t b) { h ^= b; h *= kFnvPrime; }
 inline void fnv_word(uint64_t& h, uint32_t w) {
-    for (int i = 0; i < 4; ++i) { h ^= (w >> (8 * i)) & 0xffu; h *= 0x100000001b3ull; }
+    for (int i = 0; i < 4; ++i) fnv_byte(h, (uint8_t)((w >> (8 * i)) & 0xffu));
 }
 enum { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
 
@@ -741,6 +803,17 @@ enum { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_E
  * Returns the history hash and the step count; E holds the energy at the end.  With g.secondaries (S:8(f) NEXT-3,
  * D:reading 16) a pair event deposits E - 2 me c^2 and the two annihilation photons are followed right after the parent. */
 template <class R> struct History { uint64_t h; uint32_t ns; };
+
+/* per-volume tally (S:8(a) A9): edep[vol] += deposit.  Optionally also the number of deposits and the sum of their squares
+ * per volume, from which a test estimates the Monte Carlo error of a group of volumes (S:C10 "3 sigma_MC"). */
+struct Tally {
+    double* edep; double* edep_sq; uint32_t* n_dep;
+    void add(int vol, double dep) const {
+        edep[vol] += dep;
+        if (edep_sq) edep_sq[vol] += dep * dep;
+        if (n_dep) n_dep[vol] += 1;
+    }
+};
 
 template <class R>
 void pair_directions(uint64_t seed, uint64_t id, R w1[3], R w2[3], Stream& s1) {
@@ -751,21 +824,21 @@ void pair_directions(uint64_t seed, uint64_t id, R w1[3], R w2[3], Stream& s1) {
     R ct = (R)1 - (R)2 * u0;
     R st = r_sqrt(r_max(((R)1 - ct) * ((R)1 + ct), (R)0));
     R phi = twopi * u1;
-    w1[0] = st * std::cos(phi); w1[1] = st * std::sin(phi); w1[2] = ct;
+    w1[0] = st * r_cos(phi); w1[1] = st * r_sin(phi); w1[2] = ct;
     for (int i = 0; i < 3; ++i) w2[i] = -w1[i];
 }
 
 template <class R>
 History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t id, Stream& rng, R x[3], R w[3], R& E,
-                 double* edep, oracle_stats_t& st) {
+                 const Tally& edep, oracle_stats_t& st) {
     const std::vector<MaterialR<R>>& mats = Sel<R>::m(g);
     const R twopi = (R)6.283185307179586;
-    uint64_t h = 0xcbf29ce484222325ull; uint32_t ns = 0;
+    uint64_t h = kFnvOffset; uint32_t ns = 0;
     int vol = nav.locate(x, w);
     bool alive = true;
     if (vol < 0) { st.n_escaped++; st.e_escaped += (double)E; alive = false; }
     R Y = 0; EnergyFactors<R> ef{};
-    if (alive) { Y = -std::log(rng.u<R>()); ef = energy_factors(E); }           /* Alg.1 steps 1-2 */
+    if (alive) { Y = -r_log(rng.u<R>()); ef = energy_factors(E); }           /* Alg.1 steps 1-2 */
     int zero_steps = 0;
     bool annihilate = false;
     while (alive) {
@@ -781,7 +854,7 @@ History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t 
             for (int i = 0; i < 3; ++i) x[i] = r_fma(s_int, w[i], x[i]);
             R t = rng.u<R>() * mu;
             if (t < mu3[0]) {                                                   /* photoelectric */
-                edep[vol] += (double)E; st.e_deposited += (double)E; st.n_pe++; ev = EV_PE; alive = false;
+                edep.add(vol, (double)E); st.e_deposited += (double)E; st.n_pe++; ev = EV_PE; alive = false;
             } else if (t < mu3[0] + mu3[1] || !(mu3[2] > 0)) {                  /* Compton */
                 R eps, cost, s2; kn_sample(E, rng, eps, cost, s2);
                 R Ep = eps * E;
@@ -791,11 +864,11 @@ History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t 
                 st.n_compton++; ev = EV_COMPTON;
                 E = Ep;
                 if (Ep < (R)g.e_cut) { dep = dep + Ep; st.n_cut++; ev = EV_CUT; alive = false; }
-                edep[vol] += (double)dep; st.e_deposited += (double)dep;
-                if (alive) { ef = energy_factors(E); Y = -std::log(rng.u<R>()); }
+                edep.add(vol, (double)dep); st.e_deposited += (double)dep;
+                if (alive) { ef = energy_factors(E); Y = -r_log(rng.u<R>()); }
             } else {                                                            /* pair */
                 R dep = g.secondaries ? E - (R)(2.0 * kMeC2) : E;               /* local deposit: all of E, or the pair's kinetic energy */
-                edep[vol] += (double)dep; st.e_deposited += (double)dep; st.n_pair++; ev = EV_PAIR; alive = false;
+                edep.add(vol, (double)dep); st.e_deposited += (double)dep; st.n_pair++; ev = EV_PAIR; alive = false;
                 annihilate = g.secondaries != 0;
             }
         } else {                                                                /* boundary */
@@ -827,7 +900,7 @@ History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t 
 
 template <class R>
 void transport_photon(const Geo& g, const Navigator<R>& nav, const SourceR<R>& src, uint64_t seed, uint64_t id,
-                      double* edep, oracle_stats_t& st, uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out) {
+                      const Tally& edep, oracle_stats_t& st, uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out) {
     Stream rng{seed, id, 0, 0};
     R x[3], w[3], E;
     sample_source(src, rng, x, w, E);
@@ -994,7 +1067,7 @@ template <class R> int run_step_normal(const Geo& g, const void* pos, const void
     return ORACLE_OK;
 }
 template <class R> int run_transport(const Geo& g, const oracle_source_t* src, uint64_t seed, int64_t first, int64_t n,
-                                     double* edep, oracle_stats_t* st, uint64_t* hash, uint32_t* ns, double* ef, bool grid) {
+                                     const Tally& edep, oracle_stats_t* st, uint64_t* hash, uint32_t* ns, double* ef, bool grid) {
     SourceR<R> s;
     if (!make_source(*src, s)) return ORACLE_INVALID_ARGUMENT;
     Navigator<R> nav(g, grid);
@@ -1123,6 +1196,17 @@ int oracle_geometry_create(const double* materials, int32_t n_mats, const int32_
     g->secondaries = (opts && opts->secondaries > 0) ? 1 : 0;
     for (const SolidD& s : g->solids) { g->s64.push_back(round_solid<double>(s)); g->s32.push_back(round_solid<float>(s)); }
     for (const MaterialD& m : g->mats) { g->m64.push_back(round_material<double>(m, g->sigma_pe0)); g->m32.push_back(round_material<float>(m, g->sigma_pe0)); }
+    /* operation counter: the fp64 tables again, element by element, in the counting type */
+    g->xc.resize(n_places);
+    for (int i = 0; i < n_places; ++i) {
+        for (int k = 0; k < 9; ++k) g->xc[i].M[k] = Counted(g->x64[i].M[k]);
+        for (int k = 0; k < 3; ++k) g->xc[i].T[k] = Counted(g->x64[i].T[k]);
+    }
+    for (const SolidR<double>& s : g->s64) {
+        SolidR<Counted> c; c.type = s.type; c.a = s.a; c.b = s.b; c.c = s.c; c.sector = s.sector; c.cS = s.cS; c.sS = s.sS; c.cE = s.cE; c.sE = s.sE;
+        g->sc.push_back(c);
+    }
+    for (const MaterialR<double>& m : g->m64) { MaterialR<Counted> c; c.aPE = m.aPE; c.aC = m.aC; c.aP = m.aP; c.capZ = m.capZ; g->mc.push_back(c); }
     g->grid_of.assign(n_places, -1);
     for (int i = 0; i < n_places; ++i) if ((int)g->daughters[i].size() >= g->grid_min) build_grid(*g, i);
     *out = g;
@@ -1198,11 +1282,78 @@ int oracle_nav_compute_step_normal(const void* geo, int precision, const void* p
 int oracle_transport_run(const void* geo, int precision, const oracle_source_t* src, uint64_t seed, int64_t first_id,
                          int64_t n_photons, double* edep_out, oracle_stats_t* stats_out, uint64_t* hash_out,
                          uint32_t* nsteps_out, double* efinal_out, int use_grid) {
+    return oracle_transport_run_tally(geo, precision, src, seed, first_id, n_photons, edep_out, nullptr, nullptr, stats_out, hash_out, nsteps_out,
+                                      efinal_out, use_grid);
+}
+
+int oracle_transport_run_tally(const void* geo, int precision, const oracle_source_t* src, uint64_t seed, int64_t first_id,
+                               int64_t n_photons, double* edep_out, double* edep_sq_out, uint32_t* n_dep_out, oracle_stats_t* stats_out,
+                               uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out, int use_grid) {
     if (!geo || !src || !edep_out || n_photons < 0 || first_id < 0) return ORACLE_INVALID_ARGUMENT;
     const Geo& g = *(const Geo*)geo;
-    if (precision == 64) return run_transport<double>(g, src, seed, first_id, n_photons, edep_out, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
-    if (precision == 32) return run_transport<float>(g, src, seed, first_id, n_photons, edep_out, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
+    const Tally tally{edep_out, edep_sq_out, n_dep_out};
+    if (precision == 64) return run_transport<double>(g, src, seed, first_id, n_photons, tally, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
+    if (precision == 32) return run_transport<float>(g, src, seed, first_id, n_photons, tally, stats_out, hash_out, nsteps_out, efinal_out, use_grid != 0);
     return ORACLE_INVALID_ARGUMENT;
+}
+
+/* ---- operation counts (S:8(d)): the same templates run in the counting type ------------------------------- */
+static void ops_out(uint64_t c[8]) {
+    c[0] = g_ops.add; c[1] = g_ops.mul; c[2] = g_ops.div; c[3] = g_ops.sqrt; c[4] = g_ops.cmp; c[5] = g_ops.fma; c[6] = g_ops.trans;
+    c[7] = g_ops.add + g_ops.mul + g_ops.div + g_ops.sqrt + g_ops.cmp + 2 * g_ops.fma + g_ops.trans;      /* flops: fma = 2, the rest 1 */
+}
+int oracle_transport_count_ops(const void* geo, const oracle_source_t* src, uint64_t seed, int64_t first_id, int64_t n_photons,
+                               uint64_t counts_out[8], oracle_stats_t* stats_out) {
+    if (!geo || !src || !counts_out || n_photons < 0 || first_id < 0) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    std::vector<double> edep(g.parent.size(), 0.0);
+    const Tally tally{edep.data(), nullptr, nullptr};
+    g_ops = OpCounts{0, 0, 0, 0, 0, 0, 0};
+    int rc = run_transport<Counted>(g, src, seed, first_id, n_photons, tally, stats_out, nullptr, nullptr, nullptr, true);
+    ops_out(counts_out);
+    return rc;
+}
+int oracle_nav_count_ops(const void* geo, const double* pos, const double* dir, int64_t n, uint64_t counts_out[8]) {
+    if (!geo || !counts_out || n < 0 || (n > 0 && (!pos || !dir))) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    Navigator<Counted> nav(g, true);
+    g_ops = OpCounts{0, 0, 0, 0, 0, 0, 0};
+    for (int64_t i = 0; i < n; ++i) {                       /* one config-5 query: locate, then ComputeStep */
+        Counted x[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]}, w[3] = {dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        int vol = nav.locate(x, w);
+        Counted step; int next;
+        nav.compute_step(vol, x, w, r_inf<Counted>(), step, next);
+    }
+    ops_out(counts_out);
+    return ORACLE_OK;
+}
+
+/* ---- test hooks for the history hash and the set-up arithmetic ------------------------------------------------ */
+uint64_t oracle_fnv1a_bytes(const uint8_t* bytes, int64_t n) {
+    uint64_t h = kFnvOffset;
+    for (int64_t i = 0; i < n; ++i) fnv_byte(h, bytes[i]);
+    return h;
+}
+uint64_t oracle_history_hash(const uint32_t* words, int64_t n_words) {
+    uint64_t h = kFnvOffset;
+    for (int64_t i = 0; i < n_words; ++i) fnv_word(h, words[i]);
+    return h;
+}
+int oracle_source_frame(const oracle_source_t* src, int precision, double frame_out[9]) {
+    if (!src || !frame_out) return ORACLE_INVALID_ARGUMENT;
+    if (precision == 64) { SourceR<double> s; if (!make_source(*src, s)) return ORACLE_INVALID_ARGUMENT; for (int i = 0; i < 3; ++i) { frame_out[i] = s.a[i]; frame_out[3 + i] = s.e1[i]; frame_out[6 + i] = s.e2[i]; } }
+    else if (precision == 32) { SourceR<float> s; if (!make_source(*src, s)) return ORACLE_INVALID_ARGUMENT; for (int i = 0; i < 3; ++i) { frame_out[i] = s.a[i]; frame_out[3 + i] = s.e1[i]; frame_out[6 + i] = s.e2[i]; } }
+    else return ORACLE_INVALID_ARGUMENT;
+    return ORACLE_OK;
+}
+int oracle_composed_transforms(const void* geo, int precision, double* M_out, double* T_out) {
+    if (!geo || !M_out || !T_out) return ORACLE_INVALID_ARGUMENT;
+    const Geo& g = *(const Geo*)geo;
+    for (size_t i = 0; i < g.parent.size(); ++i) {
+        for (int k = 0; k < 9; ++k) M_out[9 * i + k] = precision == 32 ? (double)g.x32[i].M[k] : g.x64[i].M[k];
+        for (int k = 0; k < 3; ++k) T_out[3 * i + k] = precision == 32 ? (double)g.x32[i].T[k] : g.x64[i].T[k];
+    }
+    return ORACLE_OK;
 }
 
 int oracle_free_path_run(const void* geo, int precision, const void* pos, const void* dir, const void* Y, int64_t n,

@@ -91,6 +91,28 @@ int oracle_transport_run(const void* geo, int precision, const oracle_source_t* 
                          int64_t first_id, int64_t n_photons, double* edep_out, oracle_stats_t* stats_out,
                          uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out, int use_grid);
 
+/* as oracle_transport_run, plus per volume (n_places each, ACCUMULATED INTO, may be NULL): edep_sq_out = sum of the squares of
+ * the deposits, n_dep_out = number of deposits -- the Monte Carlo error of a group of volumes for S:C10's "1e-3 + 3 sigma_MC" */
+int oracle_transport_run_tally(const void* geo, int precision, const oracle_source_t* src, uint64_t seed, int64_t first_id,
+                               int64_t n_photons, double* edep_out, double* edep_sq_out, uint32_t* n_dep_out, oracle_stats_t* stats_out,
+                               uint64_t* hash_out, uint32_t* nsteps_out, double* efinal_out, int use_grid);
+
+/* Operation counts of the algorithm on a real workload (S:8(d) "instrumented oracle"): the same templates run in a
+ * counting type (fp64 values).  counts_out = {add/sub, mul, div, sqrt, compare/min/max/abs, fma, transcendental,
+ * flops = sum with fma counted twice}.  Transport: photons first_id.. (the locate grid is used; ComputeStep is the plain
+ * linear scan); nav: n config-5 queries (locate, then ComputeStep), pos / dir n x 3 doubles. */
+int oracle_transport_count_ops(const void* geo, const oracle_source_t* src, uint64_t seed, int64_t first_id, int64_t n_photons,
+                               uint64_t counts_out[8], oracle_stats_t* stats_out);
+int oracle_nav_count_ops(const void* geo, const double* pos, const double* dir, int64_t n, uint64_t counts_out[8]);
+
+/* test hooks: the history hash (S:C9) of a byte string / of a list of 32-bit words (vol_before, event, ...); the source
+ * frame (a, e1, e2; D:reading 4) and the composed global->local transforms (M row-major 9, T 3 per node; S:C0) as rounded
+ * to the given precision */
+uint64_t oracle_fnv1a_bytes(const uint8_t* bytes, int64_t n);
+uint64_t oracle_history_hash(const uint32_t* words, int64_t n_words);
+int oracle_source_frame(const oracle_source_t* src, int precision, double frame_out[9]);
+int oracle_composed_transforms(const void* geo, int precision, double* M_out, double* T_out);
+
 /* The paper's own benchmark (Algorithm 2 phase 5): free path T_i of particle i from (x0, w, Y)_i by
  * Algorithm 1 with attenuation only, mu = rho * mu_mass (Eq. 9; mu_mass in cm^2/g, 0.06146 for Al at
  * 1 MeV).  pos/dir: n x 3 Real, Y: n Real, T_out: n Real (+inf: left the world), nsteps_out: n or NULL. */
