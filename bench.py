@@ -378,13 +378,17 @@ def run_ours(args):
         R = np.float32 if precision == 32 else np.float64
         hp = torch.empty((m, 3), dtype=rdt).pin_memory(); hd = torch.empty((m, 3), dtype=rdt).pin_memory()
         hp.copy_(pos[:m]); hd.copy_(dirs[:m])
-        B.nav_query_host(geo, hp.numpy()[:1024], hd.numpy()[:1024], precision)
+        hout = (torch.empty(m, dtype=torch.int32).pin_memory().numpy(), torch.empty(m, dtype=rdt).pin_memory().numpy(),
+                torch.empty(m, dtype=torch.int32).pin_memory().numpy())
+        B.nav_query_host(geo, hp.numpy(), hd.numpy(), precision, out=hout)          # untimed: sizes the handle's staging area
+        reps = 3
         t0 = time.perf_counter()
-        B.nav_query_host(geo, hp.numpy(), hd.numpy(), precision)
-        dt = time.perf_counter() - t0
+        for _ in range(reps):
+            B.nav_query_host(geo, hp.numpy(), hd.numpy(), precision, out=hout)
+        dt = (time.perf_counter() - t0) / reps
         rs = 4 if precision == 32 else 8
         e2e = {"value": world * m / dt, "unit": "ComputeStep queries/s", "h2d_bytes_per_step": 6 * rs * m, "d2h_bytes_per_step": (8 + rs) * m,
-               "note": f"{m} queries from pinned host memory per call"}
+               "note": f"{m} queries per call, inputs from and results to page-locked host memory, chunks of 2^22 on two streams"}
 
     if rank == 0:
         peak, peak_src = measured_peaks()

@@ -16,8 +16,11 @@
  * Positions / directions at the ABI are row-major n x 3 (x0 y0 z0 x1 ...).
  * Every function returns GN_OK (0) or a negative gn_status; nothing throws or aborts, and outputs are
  * untouched on failure.  gn_last_error() gives a human-readable string for the calling thread's last failure.
- * All nav calls are asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream);
- * gn_transport_run synchronises the stream before it fills the host stats.
+ * All nav calls are asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream).  gn_transport_run is
+ * host-synchronous: the stream only orders it against earlier work; the call waits for survivor counts while it
+ * enqueues its passes, synchronises the stream at the end of every batch (and once more per batch of annihilation
+ * photons with gn_opts.secondaries) and returns when the tally and the statistics are complete.
+ * Every call runs on the device the geometry was created on; the caller's current device is restored on return.
  */
 #ifndef GAMMANAV_H
 #define GAMMANAV_H
@@ -48,7 +51,9 @@ typedef struct {
     double sigma_pe0;          /* photoelectric cross-section of Z = 82 at 0.1 MeV [barn/atom]; default 1750 */
     double e_cut;              /* photons below this energy are absorbed locally [MeV]; default 0.010 */
     int32_t voxel_min_daughters; /* mothers with at least this many daughters get a voxel grid; default 8 */
-    int32_t stuck_limit;       /* consecutive steps of length <= tol/2 before a photon is killed; default 8 */
+    int32_t stuck_limit;       /* consecutive steps of length <= tol/2 before a photon is killed; default 8, at most 255
+                                  (gn_geometry_create returns GN_INVALID_ARGUMENT above that: the per-photon counter has 8 bits;
+                                  the per-photon step count has 24 bits and wraps at 2^24 steps of one photon) */
     int32_t steps_per_pass;    /* K: steps a photon takes per wavefront pass before it is re-queued; default 16 */
     int32_t first_pass_steps;  /* K0: steps in the pass that also generates the photons (sheds photons that miss early); default 1 */
     int32_t tail_photons;      /* once at most this many photons are left, one last pass runs them to completion; default 148 * 512 */
@@ -84,8 +89,8 @@ typedef struct {
     double kernel_ms;          /* duration of the whole kernel sequence of the run (source pass, step passes, interaction
                                   passes, tail), CUDA events on the launching stream */
     double step_pass_ms;       /* sum of the launch durations of the lean wavefront step passes (the dominant kernel), one
-                                  CUDA-event pair per launch (first 24 passes of each batch) */
-    uint64_t n_steps_step_pass;/* steps taken inside those passes */
+                                  CUDA-event pair per launch; only the first 64 such passes of each batch are timed */
+    uint64_t n_steps_step_pass;/* steps taken inside exactly those timed passes (later lean passes count in n_steps only) */
 } gn_run_stats;
 
 /*
@@ -198,7 +203,10 @@ int gn_transport_run(const gn_geometry* geo, int precision, const gn_source* h_s
 int gn_free_path_run(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, const void* d_Y,
                      int64_t n, double mu_mass_cm2_g, void* d_T_out, uint32_t* d_nsteps_out, void* cuda_stream);
 
-/* Host-buffer convenience wrappers (the "end to end" path: copies host<->device inside the call). */
+/* Host-buffer wrappers (the "end to end" path: copies host<->device inside the call).  The query arrays are processed in
+ * chunks of 2^22 on two internal streams with a device staging area owned by the handle, so that uploads, kernels and
+ * downloads of neighbouring chunks overlap when the caller's buffers are page-locked (pageable buffers work, serially).
+ * Synchronous: results are complete on return.  Calls on one handle are serialised. */
 int gn_nav_query_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, int64_t n,
                       int32_t* h_vol_out, void* h_step_out, int32_t* h_next_vol_out);
 int gn_free_path_run_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, const void* h_Y, int64_t n,
@@ -214,6 +222,26 @@ int gn_transport_run_host(const gn_geometry* geo, int precision, const gn_source
  * argument index of each (all ones when none).  Synchronous; default stream.
  */
 int gn_selftest_arith(int64_t n_div_pairs, uint64_t h_out[4]);
+
+/*
+ * gn_selftest_pipe_peak -- FP32 (precision 32: FFMA) or FP64 (64: DFMA) pipe peak of the current device by a register-
+ * resident fused-multiply-add kernel (8 independent chains per thread, one block of 1024 threads per SM): the flops leg of the
+ * per-step roofline.  h_out[0] = TFLOP/s (fma = 2 flops), [1] = SM clock during the run [MHz],
+ * [2] = kernel time [ms], [3] = number of SMs.  Synchronous; default stream.
+ */
+int gn_selftest_pipe_peak(int precision, double h_out[4]);
+
+/*
+ * Host-only hooks (no device needed): the fp64 set-up arithmetic of the library, exposed so that tests can compare it with
+ * an independent implementation of the same definitions.
+ *   gn_host_source_frame: frame_out = a (axis / |axis|), e1, e2, as rounded to `precision`
+ *   gn_host_compose_transforms: for every placement the composed global -> local rotation M (row-major 9 doubles) and
+ *   translation T (3 doubles) of SURVEY 8(c) C0 (M = R_global^T, p_local = M (x - T)); same validation and status codes as
+ *   gn_geometry_create
+ */
+int gn_host_source_frame(const gn_source* h_src, int precision, double frame_out[9]);
+int gn_host_compose_transforms(const int32_t* h_placements, int32_t n_places, const double* h_transforms, int32_t n_transforms,
+                               double* h_M_out, double* h_T_out);
 
 const char* gn_last_error(void);
 const char* gn_version(void);

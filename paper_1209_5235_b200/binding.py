@@ -17,7 +17,8 @@ _lib = None
 
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",
            "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_nav_compute_step_normal", "gn_nav_compute_safety", "gn_transport_run", "gn_nav_query_host",
-           "gn_transport_run_host", "gn_free_path_run", "gn_free_path_run_host", "gn_selftest_arith", "gn_last_error", "gn_version")
+           "gn_transport_run_host", "gn_free_path_run", "gn_free_path_run_host", "gn_selftest_arith", "gn_selftest_pipe_peak",
+           "gn_host_source_frame", "gn_host_compose_transforms", "gn_last_error", "gn_version")
 
 
 class GammaNavError(RuntimeError):
@@ -72,6 +73,9 @@ def lib():
                                        C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_nav_query_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_selftest_arith.argtypes = [C.c_int64, C.c_void_p]
+        L.gn_selftest_pipe_peak.argtypes = [C.c_int, C.c_void_p]
+        L.gn_host_source_frame.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.gn_host_compose_transforms.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         L.gn_free_path_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p]
         L.gn_free_path_run.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_transport_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
@@ -268,11 +272,18 @@ def free_path_run_host(geo: Geometry, pos: np.ndarray, dirs: np.ndarray, Y: np.n
     return T, ns
 
 
-def nav_query_host(geo: Geometry, pos: np.ndarray, dirs: np.ndarray, precision=64):
-    """gn_nav_query_host: host numpy buffers in, host numpy out (locate + compute_step, copies inside)."""
+def nav_query_host(geo: Geometry, pos: np.ndarray, dirs: np.ndarray, precision=64, out=None):
+    """gn_nav_query_host: host numpy buffers in, host numpy out (locate + compute_step, copies inside).
+    out = (vol int32 (n,), step Real (n,), next int32 (n,)) numpy arrays to fill (page-locked ones let the copies overlap)."""
     R = np.float32 if precision == 32 else np.float64
     pos = _np(pos, R); dirs = _np(dirs, R); n = pos.shape[0]
-    vol = np.empty(n, np.int32); step = np.empty(n, R); nxt = np.empty(n, np.int32)
+    if out is not None:
+        vol, step, nxt = out
+        if vol.dtype != np.int32 or nxt.dtype != np.int32 or step.dtype != R or min(vol.size, step.size, nxt.size) < n or \
+                not (vol.flags.c_contiguous and step.flags.c_contiguous and nxt.flags.c_contiguous):
+            raise GammaNavError("nav_query_host: out must be contiguous (int32, Real, int32) arrays of at least n elements")
+    else:
+        vol = np.empty(n, np.int32); step = np.empty(n, R); nxt = np.empty(n, np.int32)
     _check(lib().gn_nav_query_host(geo._h, precision, pos.ctypes.data_as(C.c_void_p), dirs.ctypes.data_as(C.c_void_p), C.c_int64(n),
                                    vol.ctypes.data_as(C.c_void_p), step.ctypes.data_as(C.c_void_p), nxt.ctypes.data_as(C.c_void_p)), "gn_nav_query_host")
     return vol, step, nxt
@@ -292,3 +303,27 @@ def selftest_arith(n_div_pairs=1 << 30):
     out = (C.c_uint64 * 4)()
     _check(lib().gn_selftest_arith(C.c_int64(n_div_pairs), out), "gn_selftest_arith")
     return {"sqrt_mismatches": out[0], "div_mismatches": out[1], "first_bad_sqrt": out[2], "first_bad_div": out[3]}
+
+
+def selftest_pipe_peak(precision=32):
+    """gn_selftest_pipe_peak: FFMA / DFMA pipe peak of the current device (the flops leg of the roofline)."""
+    _torch()
+    out = (C.c_double * 4)()
+    _check(lib().gn_selftest_pipe_peak(int(precision), out), "gn_selftest_pipe_peak")
+    return {"tflops": out[0], "sm_mhz": out[1], "ms": out[2], "sms": int(out[3])}
+
+
+def host_source_frame(source, precision=64):
+    """gn_host_source_frame (host-only hook): rows a, e1, e2 of the source frame as rounded to `precision`."""
+    out = np.empty(9, np.float64); cs = _csource(source)
+    _check(lib().gn_host_source_frame(C.byref(cs), int(precision), out.ctypes.data_as(C.c_void_p)), "gn_host_source_frame")
+    return out.reshape(3, 3)
+
+
+def host_compose_transforms(geom):
+    """gn_host_compose_transforms (host-only hook): composed global->local (M (n, 9), T (n, 3)) of every placement, fp64."""
+    pl = _np(geom.placements, np.int32); tr = _np(geom.transforms, np.float64)
+    M = np.empty((pl.shape[0], 9), np.float64); T = np.empty((pl.shape[0], 3), np.float64)
+    _check(lib().gn_host_compose_transforms(pl.ctypes.data_as(C.c_void_p), C.c_int32(pl.shape[0]), tr.ctypes.data_as(C.c_void_p), C.c_int32(tr.shape[0]),
+                                            M.ctypes.data_as(C.c_void_p), T.ctypes.data_as(C.c_void_p)), "gn_host_compose_transforms")
+    return M, T

@@ -8,6 +8,7 @@
 #include <string>
 #include <vector>
 #include "geometry.h"
+#include "hostmath.h"
 
 namespace gn {
 
@@ -104,6 +105,47 @@ template <class R> MatRec<R> make_mat_rec(double Z, double A, double rho, double
     return o;
 }
 
+// One solid from its type code and five parameters (gammanav.h).  What is stored is what the device formulas of
+// nav.cuh read: half-lengths / radii as given; for a phi sector the cosines and sines of its two bounding planes;
+// for a cone the mid radius, the slope dr/dz and 1 / sqrt(1 + slope^2).
+int parse_solid(int type, const double* q, HostSolid& out, const char** why) {
+    out = HostSolid{};
+    out.type = type;
+    switch (type) {
+    case GN_BOX:
+        out.a = q[0]; out.b = q[1]; out.c = q[2];
+        if (out.a > 0 && out.b > 0 && out.c > 0) return GN_OK;
+        *why = "box half-lengths must be positive"; return GN_INVALID_ARGUMENT;
+    case GN_ORB:
+        out.a = q[0];
+        if (out.a > 0) return GN_OK;
+        *why = "orb radius must be positive"; return GN_INVALID_ARGUMENT;
+    case GN_CONE: {
+        const double r_low = q[0], r_high = q[1], half = q[2];
+        if (!(r_low >= 0 && r_high >= 0 && r_low + r_high > 0 && half > 0)) { *why = "cone needs r1, r2 >= 0, r1 + r2 > 0, hz > 0"; return GN_INVALID_ARGUMENT; }
+        out.a = (r_low + r_high) / 2;
+        out.b = (r_high - r_low) / (2 * half);
+        out.c = half;
+        out.cS = 1 / std::sqrt(1 + out.b * out.b);
+        out.rbound = std::max(r_low, r_high);
+        return GN_OK;
+    }
+    case GN_TUBE: {
+        out.a = q[0]; out.b = q[1]; out.c = q[2]; out.sphi = q[3]; out.dphi = q[4];
+        if (!(out.a >= 0 && out.b > out.a && out.c > 0)) { *why = "tube needs 0 <= rmin < rmax, hz > 0"; return GN_INVALID_ARGUMENT; }
+        if (out.dphi >= 2 * kPi) return GN_OK;                        // full tube: no phi planes
+        if (!(out.dphi > 0) || out.dphi > kPi) { *why = "tube sector must have 0 < dphi <= pi (or a full tube)"; return GN_UNSUPPORTED_SOLID; }
+        const double phi_end = out.sphi + out.dphi;
+        out.sector = true;
+        out.cS = std::cos(out.sphi); out.sS = std::sin(out.sphi);
+        out.cE = std::cos(phi_end); out.sE = std::sin(phi_end);
+        return GN_OK;
+    }
+    default:
+        *why = "unknown solid type"; return GN_UNSUPPORTED_SOLID;
+    }
+}
+
 struct HostGrid { int n[3]; double gmin[3], w[3]; int cell_base; };
 
 }  // namespace
@@ -130,58 +172,29 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     }
     std::vector<HostSolid> solids(n_solids);
     for (int i = 0; i < n_solids; ++i) {
-        const double* p = h_solid_params + 5 * (size_t)i;
-        HostSolid& s = solids[i];
-        s.type = h_solid_type[i]; s.sector = false; s.cS = s.sS = s.cE = s.sE = 0; s.sphi = s.dphi = 0;
-        s.a = p[0]; s.b = p[1]; s.c = p[2];
-        if (s.type == GN_BOX) {
-            if (!(s.a > 0 && s.b > 0 && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: box half-lengths must be positive");
-        } else if (s.type == GN_CONE) {       // r1 (at -hz), r2 (at +hz), hz -> a = r0, b = slope, c = hz, cS = 1/sqrt(1 + slope^2)
-            const double r1 = p[0], r2 = p[1], hz = p[2];
-            if (!(r1 >= 0 && r2 >= 0 && r1 + r2 > 0 && hz > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: cone needs r1, r2 >= 0, r1 + r2 > 0, hz > 0");
-            s.a = (r1 + r2) / 2; s.b = (r2 - r1) / (2 * hz); s.c = hz;
-            s.cS = 1 / std::sqrt(1 + s.b * s.b);
-            s.rbound = r1 > r2 ? r1 : r2;
-        } else if (s.type == GN_ORB) {
-            s.b = s.c = 0;
-            if (!(s.a > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: orb radius must be positive");
-        } else if (s.type == GN_TUBE) {
-            s.sphi = p[3]; s.dphi = p[4];
-            if (!(s.a >= 0 && s.b > s.a && s.c > 0)) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: tube needs 0 <= rmin < rmax, hz > 0");
-            if (s.dphi < 2 * kPi) {
-                if (!(s.dphi > 0) || s.dphi > kPi) return fail(GN_UNSUPPORTED_SOLID, "gn_geometry_create: tube sector must have 0 < dphi <= pi (or a full tube)");
-                s.sector = true;
-                s.cS = std::cos(s.sphi); s.sS = std::sin(s.sphi);
-                s.cE = std::cos(s.sphi + s.dphi); s.sE = std::sin(s.sphi + s.dphi);
-            }
-        } else return fail(GN_UNSUPPORTED_SOLID, "gn_geometry_create: unknown solid type");
+        const char* why = nullptr;
+        const int rc = parse_solid(h_solid_type[i], h_solid_params + 5 * (size_t)i, solids[i], &why);
+        if (rc != GN_OK) return fail(rc, std::string("gn_geometry_create: ") + why);
     }
     const size_t V = (size_t)n_places;
     std::vector<int4> node(V);
     std::vector<double> Rg(9 * V), Tg(3 * V);
     std::vector<int> kid_count(V, 0);
     for (size_t i = 0; i < V; ++i) {
-        int p = h_placements[4 * i], s = h_placements[4 * i + 1], m = h_placements[4 * i + 2], t = h_placements[4 * i + 3];
-        if (s < 0 || s >= n_solids || m < 0 || m >= n_mats || t < 0 || t >= n_transforms)
-            return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: placement index out of range");
-        if ((i == 0 && p != -1) || (i > 0 && (p < 0 || (size_t)p >= i)))
-            return fail(GN_BAD_TREE, "gn_geometry_create: node 0 must be the world and parent < child");
-        const double* Rl = h_transforms + 12 * (size_t)t; const double* Tl = Rl + 9;
-        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) {
-            double dot = Rl[3 * a] * Rl[3 * b] + Rl[3 * a + 1] * Rl[3 * b + 1] + Rl[3 * a + 2] * Rl[3 * b + 2];
-            if (std::fabs(dot - (a == b ? 1.0 : 0.0)) > 1e-9) return fail(GN_BAD_TREE, "gn_geometry_create: rotation not orthonormal");
-        }
-        node[i] = make_int4(p, s, m, -1);
-        double* R = &Rg[9 * i]; double* T = &Tg[3 * i];
-        if (p < 0) { std::memcpy(R, Rl, 9 * sizeof(double)); std::memcpy(T, Tl, 3 * sizeof(double)); }
-        else {
-            // C0: Rg = Rg_parent R, Tg = Rg_parent T + Tg_parent, left to right, fp64
-            const double* Rp = &Rg[9 * (size_t)p]; const double* Tp = &Tg[3 * (size_t)p];
-            for (int a = 0; a < 3; ++a) {
-                for (int b = 0; b < 3; ++b) R[3 * a + b] = (Rp[3 * a] * Rl[b] + Rp[3 * a + 1] * Rl[3 + b]) + Rp[3 * a + 2] * Rl[6 + b];
-                T[a] = ((Rp[3 * a] * Tl[0] + Rp[3 * a + 1] * Tl[1]) + Rp[3 * a + 2] * Tl[2]) + Tp[a];
-            }
-            kid_count[p]++;
+        const int p = h_placements[4 * i], sol = h_placements[4 * i + 1], mat = h_placements[4 * i + 2];
+        if (sol < 0 || sol >= n_solids || mat < 0 || mat >= n_mats) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: placement index out of range");
+        node[i] = make_int4(p, sol, mat, -1);
+    }
+    {
+        std::vector<Affine> global;
+        const int st = compose_tree(h_placements, n_places, h_transforms, n_transforms, global);     // hostmath.h (C0)
+        if (st == 1) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: placement index out of range");
+        if (st == 2) return fail(GN_BAD_TREE, "gn_geometry_create: node 0 must be the world and parent < child");
+        if (st == 3) return fail(GN_BAD_TREE, "gn_geometry_create: rotation not orthonormal");
+        for (size_t i = 0; i < V; ++i) {
+            std::memcpy(&Rg[9 * i], global[i].R.m, 9 * sizeof(double));
+            Tg[3 * i] = global[i].T.x; Tg[3 * i + 1] = global[i].T.y; Tg[3 * i + 2] = global[i].T.z;
+            if (node[i].x >= 0) kid_count[node[i].x]++;
         }
     }
     // daughters in index order (CSR)
@@ -190,19 +203,19 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     { int acc = 0; for (size_t i = 0; i < V; ++i) { kids[i] = make_int2(acc, 0); acc += kid_count[i]; } }
     for (size_t i = 1; i < V; ++i) { int p = node[i].x; dlist[kids[p].x + kids[p].y] = (int)i; kids[p].y++; }
 
-    {
-        // the library's stream-ordered scratch (query sort) comes from the device's default memory pool: keep freed blocks
-        // in the pool instead of returning them to the driver at every synchronisation
-        cudaMemPool_t pool = nullptr; int dev = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) {
-            unsigned long long keep = ~0ull;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
-        cudaGetLastError();
-    }
     gn_geometry* geo = new gn_geometry();
     geo->n_places = n_places; geo->n_solids = n_solids; geo->n_mats = n_mats;
     cudaGetDevice(&geo->device);
+    {   // stream-ordered scratch of the query sort: a pool of the handle's own that keeps freed blocks (the device's default
+        // pool and its release threshold are the application's, not this library's)
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned; props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice; props.location.id = geo->device;
+        if (cudaMemPoolCreate(&geo->pool, &props) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(geo->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        } else { cudaGetLastError(); geo->pool = nullptr; }
+    }
     gn_opts o{}; if (h_opts) o = *h_opts;
     const HostSolid& ws = solids[node[0].y];
     double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == GN_ORB ? ws.a : (ws.type == GN_CONE ? std::max(ws.rbound, ws.c) : std::max(ws.b, ws.c)));
@@ -212,6 +225,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     if (!(o.e_cut > 0)) o.e_cut = 0.010;
     if (o.voxel_min_daughters <= 0) o.voxel_min_daughters = 8;
     if (o.stuck_limit <= 0) o.stuck_limit = 8;
+    if (o.stuck_limit > 255) { gn_geometry_destroy(geo); return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: stuck_limit must be <= 255 (the per-photon counter of consecutive short steps has 8 bits)"); }
     if (o.steps_per_pass <= 0) o.steps_per_pass = 16;
     if (o.first_pass_steps <= 0) o.first_pass_steps = 1;
     if (o.tail_photons <= 0) o.tail_photons = 148 * 512;
@@ -430,6 +444,9 @@ extern "C" int gn_geometry_destroy(gn_geometry* geo) {
     if (geo->ws_pinned) cudaFreeHost(geo->ws_pinned);
     if (geo->ws_host_edep) cudaFree(geo->ws_host_edep);
     if (geo->ws_events_ok) for (cudaEvent_t e : geo->ws_events) if (e) cudaEventDestroy(e);
+    if (geo->hp_buf) cudaFree(geo->hp_buf);
+    if (geo->hp_streams_ok) for (cudaStream_t st : geo->hp_stream) if (st) cudaStreamDestroy(st);
+    if (geo->pool) cudaMemPoolDestroy(geo->pool);
     delete geo;
     return GN_OK;
 }
@@ -447,3 +464,19 @@ extern "C" int gn_geometry_voxel_info(const gn_geometry* geo, int64_t info[4]) {
 namespace gn { const char* last_error_cstr(); }
 extern "C" const char* gn_last_error(void) { return gn::last_error_cstr(); }
 extern "C" const char* gn_version(void) { return "gammanav 0.1 (sm_100a)"; }
+
+// host-only hook (no device needed): the composed global -> local transforms the store would hold, M = R_global^T (row-major)
+// and T_global per node, for tests that compare them with an independent composition
+extern "C" int gn_host_compose_transforms(const int32_t* h_placements, int32_t n_places, const double* h_transforms, int32_t n_transforms,
+                                          double* h_M_out, double* h_T_out) {
+    if (!h_placements || !h_transforms || !h_M_out || !h_T_out || n_places <= 0 || n_transforms <= 0)
+        return fail(GN_INVALID_ARGUMENT, "gn_host_compose_transforms: bad argument");
+    std::vector<Affine> global;
+    const int st = compose_tree(h_placements, n_places, h_transforms, n_transforms, global);
+    if (st != 0) return fail(st == 1 ? GN_INVALID_ARGUMENT : GN_BAD_TREE, "gn_host_compose_transforms: bad placement tree");
+    for (int32_t i = 0; i < n_places; ++i) {
+        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) h_M_out[9 * (size_t)i + 3 * a + b] = global[i].R.m[3 * b + a];
+        h_T_out[3 * (size_t)i] = global[i].T.x; h_T_out[3 * (size_t)i + 1] = global[i].T.y; h_T_out[3 * (size_t)i + 2] = global[i].T.z;
+    }
+    return GN_OK;
+}

@@ -6,6 +6,8 @@
 #include "store.h"
 #include "../../include/gammanav.h"
 
+#define GN_TIMED_PASSES 64      // lean step passes of a batch that are timed one by one
+
 struct gn_geometry {
     gn::GeoView<float> v32{};
     gn::GeoView<double> v64{};
@@ -24,8 +26,15 @@ struct gn_geometry {
     mutable size_t ws_bytes = 0;
     mutable void* ws_pinned = nullptr;
     mutable double* ws_host_edep = nullptr;   // device staging of the tally for gn_transport_run_host (n_places doubles)
-    mutable cudaEvent_t ws_events[8 + 48] = {};
+    mutable cudaEvent_t ws_events[8 + 2 * GN_TIMED_PASSES] = {};
     mutable bool ws_events_ok = false;
+    // host-buffer entry points: two streams and a two-slot device staging area, so that the copies of one chunk overlap
+    // the kernels of the other
+    mutable cudaStream_t hp_stream[2] = {};
+    mutable bool hp_streams_ok = false;
+    mutable char* hp_buf = nullptr;
+    mutable size_t hp_bytes = 0;
+    cudaMemPool_t pool = nullptr;             // stream-ordered scratch (query sort) of this handle
 };
 
 namespace gn {

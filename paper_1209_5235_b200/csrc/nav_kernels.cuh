@@ -1,0 +1,218 @@
+// nav_kernels.cuh -- navigation kernels (locate, ComputeStep, surface normal, safety, the paper's free-path benchmark) and
+// their launchers, templated on the precision; instantiated in nav_f32.cu / nav_f64.cu.
+#pragma once
+#include "common.cuh"
+#include "impl.h"
+
+namespace gn {
+
+// -------------------------------------------------------------------------------------------------------
+// navigation kernels: pure maps over queries
+// -------------------------------------------------------------------------------------------------------
+template <class R, bool HAS_DIR, bool FLAT>
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : 3) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+                                                             int64_t n, int32_t* __restrict__ vol_out) {
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
+    __syncthreads();
+    Navigator<R, HAS_DIR, FLAT> nav(g, &tab.ctx);
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        V3<R> w{0, 0, 0};
+        if (HAS_DIR) { w.x = dir[3 * i]; w.y = dir[3 * i + 1]; w.z = dir[3 * i + 2]; }
+        NodeRec<R> nd;
+        vol_out[i] = nav.locate(x, w, nd);
+    }
+}
+
+template <class R, bool FLAT>
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLOCKS : 3) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+                                                           const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
+                                                           int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out,
+                                                           const uint32_t* __restrict__ perm) {
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
+    __syncthreads();
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = perm ? (int64_t)perm[t] : t;                     // work order: queries grouped by volume key (sort_queries)
+        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        int vol = vol_in[i];
+        R step = rinf<R>(); int next = -1;
+        if (vol >= 0 && vol < g.n_nodes) {
+            NodeRec<R> nd = nav.node(vol);
+            V3<R> xn;
+            nav.compute_step(vol, nd, x, w, max_step ? max_step[i] : rinf<R>(), step, xn);
+            next = vol;
+        }
+        step_out[i] = step; next_out[i] = next;
+    }
+}
+
+// Isotropic safety (reading 17): min of SafetyToOut of the volume's own solid and SafetyToIn of
+// each of its daughters, SafetyToOut / In = max(-D, 0) / max(D, 0) with D the outsideness of C2.  Plain scan of the daughter
+// list, one thread per query (lanes of a warp in the same mother read the same daughters: broadcast loads from L1 / L2).
+template <class R>
+__global__ void __launch_bounds__(NAV_THREADS) safety_kernel(GeoView<R> g, const R* __restrict__ pos, const int32_t* __restrict__ vol_in,
+                                                             int64_t n, R* __restrict__ safety_out) {
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
+    __syncthreads();
+    const NavCtx<R>* c = &tab.ctx;
+    const V3<R> w0{0, 0, 1};
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        const int vol = vol_in[i];
+        R best = 0;
+        if (vol >= 0 && vol < g.n_nodes) {
+            const NodeRec<R> nd = load_node(g.node, vol);
+            V3<R> p, v;
+            to_local<R, true>(c->rot, vol, nd, x, w0, p, v);
+            best = rmax(-outsideness(c->solids[nd.info & NODE_SOLID_MASK], p), (R)0);
+            const int first = __ldg(&g.dfirst[vol]);
+            for (int k = 0; k < nd.ndau; ++k) {
+                const int d = __ldg(&g.dlist[first + k]);
+                const NodeRec<R> dn = load_node(g.node, d);
+                to_local<R, true>(c->rot, d, dn, x, w0, p, v);
+                best = rmin(best, rmax(outsideness(c->solids[dn.info & NODE_SOLID_MASK], p), (R)0));
+            }
+        }
+        safety_out[i] = best;
+    }
+}
+
+// ComputeStep + surface normal of the boundary crossed
+template <class R, bool FLAT>
+__global__ void __launch_bounds__(NAV_THREADS) step_normal_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+                                                                  const int32_t* __restrict__ vol_in, const R* __restrict__ max_step, int64_t n,
+                                                                  R* __restrict__ step_out, int32_t* __restrict__ next_out, R* __restrict__ normal_out) {
+    __shared__ BlockTables<R> tab;
+    stage_tables(g, tab);
+    __syncthreads();
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        int vol = vol_in[i];
+        R step = rinf<R>(); int next = -1; V3<R> ng{0, 0, 0};
+        if (vol >= 0 && vol < g.n_nodes) {
+            NodeRec<R> nd = nav.node(vol);
+            nav.compute_step_normal(vol, nd, x, w, max_step ? max_step[i] : rinf<R>(), step, ng);
+            next = vol;
+        }
+        step_out[i] = step; next_out[i] = next;
+        normal_out[3 * i] = ng.x; normal_out[3 * i + 1] = ng.y; normal_out[3 * i + 2] = ng.z;
+    }
+}
+
+// -------------------------------------------------------------------------------------------------------
+// the paper's own benchmark: Algorithm 1 with attenuation only, one thread per particle
+// -------------------------------------------------------------------------------------------------------
+template <class R, bool FLAT>
+__global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+                                                                const R* __restrict__ Yin, int64_t n, double mu_mass,
+                                                                R* __restrict__ T_out, uint32_t* __restrict__ nsteps_out) {
+    __shared__ BlockTables<R> tab;
+    __shared__ R sh_mu[MAX_SMEM_MATS];
+    stage_tables(g, tab);
+    // Eq. 9: mu = rho mu_mass, here in 1/mm; fp64, rounded once to Real
+    for (int i = threadIdx.x; i < g.n_mats && i < MAX_SMEM_MATS; i += blockDim.x) sh_mu[i] = (R)(g.rho[i] * mu_mass / 10.0);
+    __syncthreads();
+    Navigator<R, true, FLAT> nav(g, &tab.ctx);
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        const V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        NodeRec<R> nd;
+        int vol = nav.locate(x, w, nd);
+        R t = 0, Yrem = Yin[i], T = rinf<R>();
+        uint32_t ns = 0; int zero_steps = 0;
+        while (vol >= 0) {
+            const R mu = nd.mat < MAX_SMEM_MATS ? sh_mu[nd.mat] : (R)(g.rho[nd.mat] * mu_mass / 10.0);
+            const R s_int = mu > 0 ? rdiv(Yrem, mu) : rinf<R>();        // remaining part of Eq. 7
+            R step; V3<R> xn;
+            nav.compute_step(vol, nd, x, w, s_int, step, xn);             // "next intersection"
+            ++ns;
+            if (step == rinf<R>()) { T = t + s_int; break; }               // S_j >= Y inside this volume (L76)
+            x = xn;
+            t = t + step;
+            Yrem = rmax(Yrem - step * mu, (R)0);                           // S_j update (L71)
+            zero_steps = (step <= g.delta) ? zero_steps + 1 : 0;
+            if (vol >= 0 && zero_steps >= g.stuck_limit) break;
+        }
+        T_out[i] = T;
+        if (nsteps_out) nsteps_out[i] = ns;
+    }
+}
+
+template <class R> int locate_impl(const gn_geometry* geo, const void* pos, const void* dir, int64_t n, int32_t* out, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    // geometries whose lanes do different things per node visit (tubes, rotations, long candidate lists) use the flat
+    // one-visit-per-iteration search, coherent ones (voxel phantoms) the nested climb / descend loops
+    if (geo->coherent) {
+        if (dir) locate_kernel<R, true, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
+        else locate_kernel<R, false, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
+    } else {
+        if (dir) locate_kernel<R, true, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
+        else locate_kernel<R, false, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
+    }
+    GN_CUDA(cudaGetLastError(), "gn_nav_locate launch");
+    return GN_OK;
+}
+template <class R> int step_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
+                                 int64_t n, void* step, int32_t* next, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    if (geo->coherent) {
+        step_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, nullptr);
+        GN_CUDA(cudaGetLastError(), "gn_nav_compute_step launch");
+        return GN_OK;
+    }
+    // general geometry: group the queries by volume key first (large batches only; stream-ordered scratch)
+    uint32_t* perm = nullptr;
+    char* scratch = nullptr;
+    if (n >= (1 << 16) && n < (1ll << 32)) {
+        const size_t bytes = 256 + (size_t)n + 4 * (size_t)n + 64;
+        if (geo->pool && cudaMallocFromPoolAsync((void**)&scratch, bytes, geo->pool, s) == cudaSuccess) {
+            unsigned long long* totals = (unsigned long long*)scratch; unsigned long long* cursors = totals + 16;
+            uint8_t* keys = (uint8_t*)(scratch + 256);
+            perm = (uint32_t*)(scratch + 256 + (((size_t)n + 63) & ~(size_t)63));
+            cudaMemsetAsync(scratch, 0, 256, s);
+            sort_keys_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), vol, n, keys, totals);
+            sort_scatter_kernel<<<nav_grid((n + 3) / 4), NAV_THREADS, 0, s>>>(keys, n, totals, cursors, perm, nullptr);
+        } else { cudaGetLastError(); scratch = nullptr; }                     // no scratch: run in arrival order
+    }
+    step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, perm);
+    cudaError_t e = cudaGetLastError();
+    if (scratch) cudaFreeAsync(scratch, s);
+    GN_CUDA(e, "gn_nav_compute_step launch");
+    return GN_OK;
+}
+
+template <class R> int step_normal_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
+                                        int64_t n, void* step, int32_t* next, void* normal, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    if (geo->coherent) step_normal_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, (R*)normal);
+    else step_normal_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, (R*)normal);
+    GN_CUDA(cudaGetLastError(), "gn_nav_compute_step_normal launch");
+    return GN_OK;
+}
+
+template <class R> int safety_impl(const gn_geometry* geo, const void* pos, const int32_t* vol, int64_t n, void* out, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    safety_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, vol, n, (R*)out);
+    GN_CUDA(cudaGetLastError(), "gn_nav_compute_safety launch");
+    return GN_OK;
+}
+
+template <class R> int free_path_impl(const gn_geometry* geo, const void* pos, const void* dir, const void* Y, int64_t n, double mu_mass,
+                                      void* T, uint32_t* ns, cudaStream_t s) {
+    if (n == 0) return GN_OK;
+    const int64_t blocks = (n + NAV_THREADS - 1) / NAV_THREADS;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(blocks, 148 * 64));
+    if (geo->coherent) free_path_kernel<R, false><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
+    else free_path_kernel<R, true><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
+    GN_CUDA(cudaGetLastError(), "gn_free_path_run launch");
+    return GN_OK;
+}
+
+}  // namespace gn

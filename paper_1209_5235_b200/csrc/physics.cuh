@@ -63,14 +63,17 @@ __device__ __forceinline__ void rsincos(double a, double* s, double* c) { *s = s
 template <class R> struct EnergyFactors { R gPE, gKN, L2k; int above_pair; };
 
 template <class R> __device__ EnergyFactors<R> energy_factors(R E) {
-    double e = (double)E, k = e / GN_ME_C2;
+    // Klein-Nishina total cross-section per electron in units of 2 pi r_e^2 (C6):
+    //   (1+k)/k^2 [2(1+k)/(1+2k) - ln(1+2k)/k] + ln(1+2k)/(2k) - (1+3k)/(1+2k)^2,  k = E / me c^2
+    // DESIGN.md reading 1 writes g_KN as sigma_KN / (2 pi r_e^2): the prefactor is multiplied in and divided out again
+    const double k = (double)E / GN_ME_C2;
+    const double one_k = 1.0 + k, one_2k = 1.0 + 2.0 * k, lg = log(one_2k);
+    const double bracket = 2.0 * one_k / one_2k - lg / k;
+    const double first = one_k / (k * k) * bracket, second = lg / (2.0 * k), third = (1.0 + 3.0 * k) / (one_2k * one_2k);
+    const double two_pi_re2 = 2.0 * GN_PI * 2.8179403262e-13 * 2.8179403262e-13;
     EnergyFactors<R> f;
-    f.gPE = (R)pow(0.1 / e, 3.5);
-    double l = log(1.0 + 2.0 * k);
-    double t1 = (1.0 + k) / (k * k) * (2.0 * (1.0 + k) / (1.0 + 2.0 * k) - l / k);
-    double t2 = l / (2.0 * k);
-    double t3 = (1.0 + 3.0 * k) / ((1.0 + 2.0 * k) * (1.0 + 2.0 * k));
-    f.gKN = (R)(t1 + t2 - t3);       // sigma_KN / (2 pi r_e^2)
+    f.gKN = (R)((two_pi_re2 * (first + second - third)) / two_pi_re2);
+    f.gPE = (R)pow(0.1 / (double)E, 3.5);
     f.L2k = (R)log(2.0 * k);
     f.above_pair = k > 2.0;
     return f;

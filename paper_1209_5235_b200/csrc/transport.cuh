@@ -20,238 +20,12 @@
 //     small in registers and instruction cache;
 //   * solids, voxel-grid headers and material factors are staged in shared memory; node records and voxel
 //     cells stay in L2.
-#include <cstdio>
-#include <cstring>
-#include <mutex>
-#include <string>
-#include "geometry.h"
-#include "nav.cuh"
+#pragma once
+#include "common.cuh"
+#include "impl.h"
 #include "physics.cuh"
 
 namespace gn {
-
-constexpr int NAV_THREADS = 256;
-#ifndef NAV_LOCATE_MIN_BLOCKS
-#define NAV_LOCATE_MIN_BLOCKS 8
-#endif
-#ifndef NAV_STEP_MIN_BLOCKS
-#define NAV_STEP_MIN_BLOCKS 8      // ComputeStep kernels are latency-bound at ~10 of 32 lanes: full occupancy (32 registers, spills) wins
-#endif
-constexpr int MAX_SMEM_SOLIDS = 32;
-constexpr int MAX_SMEM_GRIDS = 8;
-constexpr int MAX_SMEM_MATS = 32;
-
-// per-block copies of the small tables + the pointer block the out-of-line navigation helpers read
-template <class R> struct BlockTables {
-    SolidRec<R> solids[MAX_SMEM_SOLIDS];
-    GridRec<R> grids[MAX_SMEM_GRIDS];
-    NavCtx<R> ctx;
-};
-template <class R> __device__ __forceinline__ void stage_tables(const GeoView<R>& g, BlockTables<R>& t) {
-    const bool ss = g.n_solids <= MAX_SMEM_SOLIDS, sg = g.n_grids <= MAX_SMEM_GRIDS;
-    if (ss) for (int i = threadIdx.x; i < g.n_solids; i += blockDim.x) t.solids[i] = g.solids[i];
-    if (sg) for (int i = threadIdx.x; i < g.n_grids; i += blockDim.x) t.grids[i] = g.grids[i];
-    if (threadIdx.x == 0) {
-        t.ctx.node = g.node; t.ctx.rot = g.rot; t.ctx.dlist = g.dlist; t.ctx.cells = g.cells; t.ctx.cand = g.cand;
-        t.ctx.solids = ss ? t.solids : g.solids; t.ctx.grids = sg ? t.grids : g.grids; t.ctx.delta = g.delta;
-    }
-}
-
-// -------------------------------------------------------------------------------------------------------
-// navigation kernels: pure maps over queries
-// -------------------------------------------------------------------------------------------------------
-template <class R, bool HAS_DIR, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : 3) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
-                                                             int64_t n, int32_t* __restrict__ vol_out) {
-    __shared__ BlockTables<R> tab;
-    stage_tables(g, tab);
-    __syncthreads();
-    Navigator<R, HAS_DIR, FLAT> nav(g, &tab.ctx);
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
-        V3<R> w{0, 0, 0};
-        if (HAS_DIR) { w.x = dir[3 * i]; w.y = dir[3 * i + 1]; w.z = dir[3 * i + 2]; }
-        NodeRec<R> nd;
-        vol_out[i] = nav.locate(x, w, nd);
-    }
-}
-
-// Sort of the navigation queries by volume key (SURVEY 8(a) A10 applied to A11): queries arrive in arbitrary order, so in
-// a geometry with mixed solids the lanes of a warp would do different things (world: box exit + scan of the barrels;
-// sector: tube exit; ...).  Two small kernels build a work order -- a counting sort of the query indices by key = (solid
-// type of the current volume, has daughters) -- and step_kernel runs through it; outputs go back to the original slots.
-// Which query lands where inside its key's segment depends on block scheduling; the results do not.
-constexpr int SORT_KEYS = 9;              // 4 solid types x {leaf, mother} + "no volume"
-constexpr int SORT_TILE = 1024;
-template <class R>
-__global__ void __launch_bounds__(NAV_THREADS) sort_keys_kernel(GeoView<R> g, const int32_t* __restrict__ vol_in, int64_t n,
-                                                                uint8_t* __restrict__ keys, unsigned long long* __restrict__ totals) {
-    __shared__ unsigned sh[SORT_KEYS];
-    if (threadIdx.x < SORT_KEYS) sh[threadIdx.x] = 0;
-    __syncthreads();
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const int v = vol_in[i];
-        int key = SORT_KEYS - 1;
-        if (v >= 0 && v < g.n_nodes) {
-            const int4 h = __ldg(reinterpret_cast<const int4*>(g.node + v));          // {parent, info, mat, ndau}
-            key = 2 * __ldg(&g.solids[h.y & NODE_SOLID_MASK].type) + (h.w > 0 ? 1 : 0);
-        }
-        keys[i] = (uint8_t)key;
-        atomicAdd(&sh[key], 1u);
-    }
-    __syncthreads();
-    if (threadIdx.x < SORT_KEYS && sh[threadIdx.x]) atomicAdd(&totals[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
-}
-__global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const uint8_t* __restrict__ keys, int64_t n, const unsigned long long* __restrict__ totals,
-                                                                   unsigned long long* __restrict__ cursors, uint32_t* __restrict__ perm,
-                                                                   const unsigned* __restrict__ n_ptr) {
-    __shared__ unsigned sh_cnt[SORT_KEYS];
-    __shared__ unsigned long long sh_base[SORT_KEYS];
-    if (n_ptr) n = (int64_t)*n_ptr;                                          // count known only on the device (transport passes)
-    const int64_t n_tiles = (n + SORT_TILE - 1) / SORT_TILE;
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        if (threadIdx.x < SORT_KEYS) sh_cnt[threadIdx.x] = 0;
-        __syncthreads();
-        int key[SORT_TILE / NAV_THREADS]; unsigned rank[SORT_TILE / NAV_THREADS];
-#pragma unroll
-        for (int q = 0; q < SORT_TILE / NAV_THREADS; ++q) {
-            const int64_t i = tile * SORT_TILE + q * NAV_THREADS + threadIdx.x;
-            key[q] = i < n ? keys[i] : -1;
-            rank[q] = key[q] >= 0 ? atomicAdd(&sh_cnt[key[q]], 1u) : 0u;
-        }
-        __syncthreads();
-        if (threadIdx.x < SORT_KEYS) {
-            unsigned long long seg = 0;                                        // start of this key's segment
-            for (int k = 0; k < (int)threadIdx.x; ++k) seg += totals[k];
-            sh_base[threadIdx.x] = seg + (sh_cnt[threadIdx.x] ? atomicAdd(&cursors[threadIdx.x], (unsigned long long)sh_cnt[threadIdx.x]) : 0ull);
-        }
-        __syncthreads();
-#pragma unroll
-        for (int q = 0; q < SORT_TILE / NAV_THREADS; ++q)
-            if (key[q] >= 0) perm[sh_base[key[q]] + rank[q]] = (uint32_t)(tile * SORT_TILE + q * NAV_THREADS + threadIdx.x);
-        __syncthreads();
-    }
-}
-
-template <class R, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLOCKS : 3) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
-                                                           const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
-                                                           int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out,
-                                                           const uint32_t* __restrict__ perm) {
-    __shared__ BlockTables<R> tab;
-    stage_tables(g, tab);
-    __syncthreads();
-    Navigator<R, true, FLAT> nav(g, &tab.ctx);
-    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t i = perm ? (int64_t)perm[t] : t;                     // work order: queries grouped by volume key (sort_queries)
-        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
-        V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
-        int vol = vol_in[i];
-        R step = rinf<R>(); int next = -1;
-        if (vol >= 0 && vol < g.n_nodes) {
-            NodeRec<R> nd = nav.node(vol);
-            V3<R> xn;
-            nav.compute_step(vol, nd, x, w, max_step ? max_step[i] : rinf<R>(), step, xn);
-            next = vol;
-        }
-        step_out[i] = step; next_out[i] = next;
-    }
-}
-
-// Isotropic safety (reading 17): min of SafetyToOut of the volume's own solid and SafetyToIn of
-// each of its daughters, SafetyToOut / In = max(-D, 0) / max(D, 0) with D the outsideness of C2.  Plain scan of the daughter
-// list, one thread per query (lanes of a warp in the same mother read the same daughters: broadcast loads from L1 / L2).
-template <class R>
-__global__ void __launch_bounds__(NAV_THREADS) safety_kernel(GeoView<R> g, const R* __restrict__ pos, const int32_t* __restrict__ vol_in,
-                                                             int64_t n, R* __restrict__ safety_out) {
-    __shared__ BlockTables<R> tab;
-    stage_tables(g, tab);
-    __syncthreads();
-    const NavCtx<R>* c = &tab.ctx;
-    const V3<R> w0{0, 0, 1};
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
-        const int vol = vol_in[i];
-        R best = 0;
-        if (vol >= 0 && vol < g.n_nodes) {
-            const NodeRec<R> nd = load_node(g.node, vol);
-            V3<R> p, v;
-            to_local<R, true>(c->rot, vol, nd, x, w0, p, v);
-            best = rmax(-outsideness(c->solids[nd.info & NODE_SOLID_MASK], p), (R)0);
-            const int first = __ldg(&g.dfirst[vol]);
-            for (int k = 0; k < nd.ndau; ++k) {
-                const int d = __ldg(&g.dlist[first + k]);
-                const NodeRec<R> dn = load_node(g.node, d);
-                to_local<R, true>(c->rot, d, dn, x, w0, p, v);
-                best = rmin(best, rmax(outsideness(c->solids[dn.info & NODE_SOLID_MASK], p), (R)0));
-            }
-        }
-        safety_out[i] = best;
-    }
-}
-
-// ComputeStep + surface normal of the boundary crossed
-template <class R, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS) step_normal_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
-                                                                  const int32_t* __restrict__ vol_in, const R* __restrict__ max_step, int64_t n,
-                                                                  R* __restrict__ step_out, int32_t* __restrict__ next_out, R* __restrict__ normal_out) {
-    __shared__ BlockTables<R> tab;
-    stage_tables(g, tab);
-    __syncthreads();
-    Navigator<R, true, FLAT> nav(g, &tab.ctx);
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
-        V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
-        int vol = vol_in[i];
-        R step = rinf<R>(); int next = -1; V3<R> ng{0, 0, 0};
-        if (vol >= 0 && vol < g.n_nodes) {
-            NodeRec<R> nd = nav.node(vol);
-            nav.compute_step_normal(vol, nd, x, w, max_step ? max_step[i] : rinf<R>(), step, ng);
-            next = vol;
-        }
-        step_out[i] = step; next_out[i] = next;
-        normal_out[3 * i] = ng.x; normal_out[3 * i + 1] = ng.y; normal_out[3 * i + 2] = ng.z;
-    }
-}
-
-// -------------------------------------------------------------------------------------------------------
-// the paper's own benchmark: Algorithm 1 with attenuation only, one thread per particle
-// -------------------------------------------------------------------------------------------------------
-template <class R, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
-                                                                const R* __restrict__ Yin, int64_t n, double mu_mass,
-                                                                R* __restrict__ T_out, uint32_t* __restrict__ nsteps_out) {
-    __shared__ BlockTables<R> tab;
-    __shared__ R sh_mu[MAX_SMEM_MATS];
-    stage_tables(g, tab);
-    // Eq. 9: mu = rho mu_mass, here in 1/mm; fp64, rounded once to Real
-    for (int i = threadIdx.x; i < g.n_mats && i < MAX_SMEM_MATS; i += blockDim.x) sh_mu[i] = (R)(g.rho[i] * mu_mass / 10.0);
-    __syncthreads();
-    Navigator<R, true, FLAT> nav(g, &tab.ctx);
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
-        const V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
-        NodeRec<R> nd;
-        int vol = nav.locate(x, w, nd);
-        R t = 0, Yrem = Yin[i], T = rinf<R>();
-        uint32_t ns = 0; int zero_steps = 0;
-        while (vol >= 0) {
-            const R mu = nd.mat < MAX_SMEM_MATS ? sh_mu[nd.mat] : (R)(g.rho[nd.mat] * mu_mass / 10.0);
-            const R s_int = mu > 0 ? rdiv(Yrem, mu) : rinf<R>();        // remaining part of Eq. 7
-            R step; V3<R> xn;
-            nav.compute_step(vol, nd, x, w, s_int, step, xn);             // "next intersection"
-            ++ns;
-            if (step == rinf<R>()) { T = t + s_int; break; }               // S_j >= Y inside this volume (L76)
-            x = xn;
-            t = t + step;
-            Yrem = rmax(Yrem - step * mu, (R)0);                           // S_j update (L71)
-            zero_steps = (step <= g.delta) ? zero_steps + 1 : 0;
-            if (vol >= 0 && zero_steps >= g.stuck_limit) break;
-        }
-        T_out[i] = T;
-        if (nsteps_out) nsteps_out[i] = ns;
-    }
-}
 
 // -------------------------------------------------------------------------------------------------------
 // transport
@@ -330,9 +104,13 @@ template <class R> __device__ __forceinline__ void history_out(const PerPhotonOu
     }
 }
 
+// history hash: FNV-1a-64, one 32-bit word = its four bytes, least significant first
 __device__ __forceinline__ void fnv_word(uint64_t& h, uint32_t w) {
-#pragma unroll
-    for (int i = 0; i < 4; ++i) { h ^= (w >> (8 * i)) & 0xffu; h *= 0x100000001b3ull; }
+    const uint64_t prime = 0x100000001b3ull;
+    h = (h ^ (uint64_t)(w & 0xffu)) * prime;
+    h = (h ^ (uint64_t)((w >> 8) & 0xffu)) * prime;
+    h = (h ^ (uint64_t)((w >> 16) & 0xffu)) * prime;
+    h = (h ^ (uint64_t)(w >> 24)) * prime;
 }
 
 template <class T> __device__ __forceinline__ T warp_sum(T v) {
@@ -342,7 +120,7 @@ template <class T> __device__ __forceinline__ T warp_sum(T v) {
 }
 
 // warp-aggregated tally: one fp64 atomic per distinct volume per warp
-__device__ __noinline__ void warp_tally(double* __restrict__ edep, double* sh_dep_total, int vol, double dep, bool has) {
+static __device__ __noinline__ void warp_tally(double* __restrict__ edep, double* sh_dep_total, int vol, double dep, bool has) {
     const int lane = threadIdx.x & 31;
     {   // book-keeping total: one shared atomic per warp
         double tot = has ? dep : 0.0;
@@ -443,7 +221,7 @@ template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
 __global__ void __launch_bounds__(TR_THREADS, (sizeof(R) == 4 && !PHYS) ? (FROM_SOURCE ? TR_MIN_BLOCKS_SRC : (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX)) : 1)
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
-               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio, SecIO<R> sec) {
+               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio, SecIO<R> sec, int timed) {
     // input: pass 0 generates n_src photons; later passes read the survivors of the previous pass, whose count is
     // known only on the device (front + back of cin)
     unsigned n_front = n_src, n_in = n_src;
@@ -576,8 +354,8 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             const bool inter = step == rinf<R>();                              // S_j >= Y: the photon interacts in vol
             const R len = inter ? s_int : step;
             uint32_t zs = misc & 0xffu;
-            zs = (len <= g.delta) ? zs + 1 : 0;
-            misc = (misc & ~0xffu) | (zs & 0xffu);
+            zs = (len <= g.delta) ? min(zs + 1u, 255u) : 0u;                  // saturates: stuck_limit <= 255 is enforced at create time
+            misc = (misc & ~0xffu) | zs;
             if (inter) {
                 x = advance(x, w, s_int);
                 pending = true;
@@ -638,7 +416,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     __syncthreads();
     if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
-    if (!FROM_SOURCE && !PHYS && threadIdx.x == 12 && sh_cnt[ST_STEPS]) atomicAdd(&stats->lean_steps, sh_cnt[ST_STEPS]);
+    if (!FROM_SOURCE && !PHYS && timed && threadIdx.x == 12 && sh_cnt[ST_STEPS]) atomicAdd(&stats->lean_steps, sh_cnt[ST_STEPS]);
     if (FLAT && sio.kout && threadIdx.x >= 32 && threadIdx.x < 32 + SORT_KEYS && sh_key[threadIdx.x - 32]) atomicAdd(&sio.kout->tot[threadIdx.x - 32], (unsigned long long)sh_key[threadIdx.x - 32]);
 }
 
@@ -812,8 +590,8 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
             const bool inter = step == rinf<R>();
             const R len = inter ? s_int : step;
             uint32_t zs = misc & 0xffu;
-            zs = (len <= g.delta) ? zs + 1 : 0;
-            misc = (misc & ~0xffu) | (zs & 0xffu);
+            zs = (len <= g.delta) ? min(zs + 1u, 255u) : 0u;                  // saturates: stuck_limit <= 255 is enforced at create time
+            misc = (misc & ~0xffu) | zs;
             if (inter) {
                 x = advance(x, w, s_int);
                 pending = true;
@@ -843,104 +621,19 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
 }
 
-// -------------------------------------------------------------------------------------------------------
-// host side
-// -------------------------------------------------------------------------------------------------------
-static int cuda_fail(cudaError_t e, const char* where) {
-    return fail(GN_CUDA_ERROR, std::string(where) + ": " + cudaGetErrorString(e));
-}
-#define GN_CUDA(call, where) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(e__, where); } while (0)
-
-static int nav_grid(int64_t n) {
-    int64_t blocks = (n + NAV_THREADS - 1) / NAV_THREADS;
-    const int64_t cap = 148 * 64;                 // grid-stride beyond this; multiple of the SM count
-    return (int)std::max<int64_t>(1, std::min(blocks, cap));
-}
-
-template <class R> const GeoView<R>& view(const gn_geometry* g);
-template <> const GeoView<float>& view<float>(const gn_geometry* g) { return g->v32; }
-template <> const GeoView<double>& view<double>(const gn_geometry* g) { return g->v64; }
-
-template <class R> int locate_impl(const gn_geometry* geo, const void* pos, const void* dir, int64_t n, int32_t* out, cudaStream_t s) {
-    if (n == 0) return GN_OK;
-    // geometries whose lanes do different things per node visit (tubes, rotations, long candidate lists) use the flat
-    // one-visit-per-iteration search, coherent ones (voxel phantoms) the nested climb / descend loops
-    if (geo->coherent) {
-        if (dir) locate_kernel<R, true, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
-        else locate_kernel<R, false, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
-    } else {
-        if (dir) locate_kernel<R, true, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
-        else locate_kernel<R, false, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
-    }
-    GN_CUDA(cudaGetLastError(), "gn_nav_locate launch");
-    return GN_OK;
-}
-template <class R> int step_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
-                                 int64_t n, void* step, int32_t* next, cudaStream_t s) {
-    if (n == 0) return GN_OK;
-    if (geo->coherent) {
-        step_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, nullptr);
-        GN_CUDA(cudaGetLastError(), "gn_nav_compute_step launch");
-        return GN_OK;
-    }
-    // general geometry: group the queries by volume key first (large batches only; stream-ordered scratch)
-    uint32_t* perm = nullptr;
-    char* scratch = nullptr;
-    if (n >= (1 << 16) && n < (1ll << 32)) {
-        const size_t bytes = 256 + (size_t)n + 4 * (size_t)n + 64;
-        if (cudaMallocAsync((void**)&scratch, bytes, s) == cudaSuccess) {
-            unsigned long long* totals = (unsigned long long*)scratch; unsigned long long* cursors = totals + 16;
-            uint8_t* keys = (uint8_t*)(scratch + 256);
-            perm = (uint32_t*)(scratch + 256 + (((size_t)n + 63) & ~(size_t)63));
-            cudaMemsetAsync(scratch, 0, 256, s);
-            sort_keys_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), vol, n, keys, totals);
-            sort_scatter_kernel<<<nav_grid((n + 3) / 4), NAV_THREADS, 0, s>>>(keys, n, totals, cursors, perm, nullptr);
-        } else { cudaGetLastError(); scratch = nullptr; }                     // no scratch: run in arrival order
-    }
-    step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, perm);
-    cudaError_t e = cudaGetLastError();
-    if (scratch) cudaFreeAsync(scratch, s);
-    GN_CUDA(e, "gn_nav_compute_step launch");
-    return GN_OK;
-}
-
-template <class R> bool make_source(const gn_source& s, SourceDev<R>& o) {
-    // a = axis / |axis|; h = unit vector of the smallest |a_i| (ties x < y < z);
-    // e1 = normalise(h - (h.a) a); e2 = a x e1 -- fp64 on the host, rounded once to Real.
-    double n = std::sqrt(s.axis[0] * s.axis[0] + s.axis[1] * s.axis[1] + s.axis[2] * s.axis[2]);
-    if (!(n > 0) || !(s.e0 > 0)) return false;
-    double a[3] = {s.axis[0] / n, s.axis[1] / n, s.axis[2] / n};
-    int m = 0;
-    if (std::fabs(a[1]) < std::fabs(a[m])) m = 1;
-    if (std::fabs(a[2]) < std::fabs(a[m])) m = 2;
-    double hv[3] = {0, 0, 0}; hv[m] = 1;
-    double ha = a[m];
-    double e1[3] = {hv[0] - ha * a[0], hv[1] - ha * a[1], hv[2] - ha * a[2]};
-    double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
-    for (int i = 0; i < 3; ++i) e1[i] /= n1;
-    double e2[3] = {a[1] * e1[2] - a[2] * e1[1], a[2] * e1[0] - a[0] * e1[2], a[0] * e1[1] - a[1] * e1[0]};
-    o.kind = s.kind; o.energy_kind = s.energy_kind;
-    for (int i = 0; i < 3; ++i) { o.o[i] = (R)s.origin[i]; o.a[i] = (R)a[i]; o.e1[i] = (R)e1[i]; o.e2[i] = (R)e2[i]; }
-    o.sigma = (R)s.sigma; o.cos_half = (R)std::cos(s.half_angle); o.e0 = (R)s.e0; o.ln_e0 = 0; o.ln_ratio = 0;
-    if (s.energy_kind == GN_E_LOGUNIFORM) {
-        if (!(s.e1 >= s.e0)) return false;
-        o.ln_e0 = (R)std::log(s.e0); o.ln_ratio = (R)std::log(s.e1 / s.e0);
-    } else if (s.energy_kind != GN_E_MONO) return false;
-    return s.kind >= GN_SRC_PENCIL && s.kind <= GN_SRC_ISOTROPIC;
-}
-
 constexpr int64_t TR_BATCH = 1ll << 24;     // photons per batch (bounds scratch at 2 x 16.8 M x 64 B = 2.1 GB in fp32)
 constexpr int TR_MAX_PASSES = 4096;         // device counters per batch; the last one always runs to completion
 constexpr int TR_LAG = 2;                   // the host looks at survivor counts that are this many passes old
 constexpr int K_UNLIMITED = 0x7fffffff;
-constexpr int TR_TIMED = 24;                // lean step passes per batch timed one by one (CUDA events around the launch)
+constexpr int TR_TIMED = GN_TIMED_PASSES;   // lean step passes per batch timed one by one (CUDA events around the launch)
 
 template <class R, bool SRC, bool PHYS, bool FLAT>
 static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, const SourceDev<R>& src, uint64_t seed, uint64_t first_id,
                         uint32_t n_src, const PassCounters* cin, PassCounters* cout, const PhotonRec<R>* qin, PhotonRec<R>* qout, uint32_t cap,
-                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct, SecIO<R> sec, SortIO sio = SortIO{nullptr, nullptr, nullptr}) {
-    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio, sec);
-    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio, sec);
+                        double* edep, DevStats* stats, PerPhotonOut pp, int K, int regroup_pct, SecIO<R> sec, SortIO sio = SortIO{nullptr, nullptr, nullptr},
+                        int timed = 0) {
+    if (track) transport_pass<R, SRC, true, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio, sec, timed);
+    else transport_pass<R, SRC, false, PHYS, FLAT><<<blocks, TR_THREADS, 0, s>>>(g, src, seed, first_id, n_src, cin, cout, qin, qout, cap, edep, stats, pp, K, regroup_pct, sio, sec, timed);
 }
 template <class R>
 static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, uint64_t seed, uint64_t first_id, const PassCounters* cin,
@@ -949,11 +642,9 @@ static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const G
     else interact_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
 }
 
-template <class R>
-int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed, int64_t first_id, int64_t n_photons,
+template <class R, bool FLAT>
+int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t seed, int64_t first_id, int64_t n_photons,
                    double* d_edep, gn_run_stats* h_stats, uint64_t* d_hash, uint32_t* d_nsteps, double* d_efinal, cudaStream_t s) {
-    SourceDev<R> src;
-    if (!make_source(*h_src, src)) return fail(GN_INVALID_ARGUMENT, "gn_transport_run: bad source (axis, energies or kind)");
     const bool track = d_hash || d_nsteps || d_efinal;
     const int K = geo->opts.steps_per_pass;
     const int K0 = std::min(K, geo->opts.first_pass_steps);      // first pass: short, sheds photons that miss
@@ -964,7 +655,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
     const size_t qb = cap * sizeof(PhotonRec<R>);
     const size_t hb = (track && !d_hash) ? cap * 8 : 0;       // the hash array doubles as per-photon state between passes
     const size_t cb = sizeof(PassCounters) * (TR_MAX_PASSES + 2);
-    const bool sorted = !geo->coherent;                        // general geometries: work order of every pass sorted by volume key
+    const bool sorted = FLAT;                                  // general geometries: work order of every pass sorted by volume key
     const size_t kb = sorted ? sizeof(KeyCounters) * (TR_MAX_PASSES + 2) : 0;
     const size_t sb = sorted ? ((cap + 255) & ~(size_t)255) + 4 * cap : 0;      // keys + perm
     const size_t pb = secondaries ? cap * sizeof(PairVtx<R>) + 16 : 0;          // pair vertices of a batch + their count
@@ -1032,21 +723,21 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
             }
             const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
             const unsigned blocks = (ub + TR_THREADS - 1) / TR_THREADS;
-            // FLAT = general geometry (any solid, rotations, long candidate lists); !FLAT = unrotated boxes only (geo->coherent)
             if (p == 0) {
-                if (geo->coherent) launch_pass<R, true, false, false>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, k_first, regroup, sec);
-                else launch_pass<R, true, false, true>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, k_first, regroup, sec, SortIO{d_kctr + 1, d_keys, nullptr});
+                launch_pass<R, true, false, FLAT>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, k_first, regroup, sec,
+                                                  sorted ? SortIO{d_kctr + 1, d_keys, nullptr} : SortIO{nullptr, nullptr, nullptr});
             } else if (last) {
-                if (geo->coherent) launch_pass<R, false, true, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec);
-                else launch_pass<R, false, true, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec, SortIO{nullptr, nullptr, d_perm});
-            }
-            else {
-                // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass
+                launch_pass<R, false, true, FLAT>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec,
+                                                  sorted ? SortIO{nullptr, nullptr, d_perm} : SortIO{nullptr, nullptr, nullptr});
+            } else {
+                // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass; the
+                // first TR_TIMED lean passes of a batch are timed one by one, and only their steps count as lean_steps
                 launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
-                if (n_timed < TR_TIMED) cudaEventRecord(tev[2 * n_timed], s);
-                if (geo->coherent) launch_pass<R, false, false, false>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec);
-                else launch_pass<R, false, false, true>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec, SortIO{d_kctr + p + 1, d_keys, d_perm});
-                if (n_timed < TR_TIMED) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
+                const bool timed = n_timed < TR_TIMED;
+                if (timed) cudaEventRecord(tev[2 * n_timed], s);
+                launch_pass<R, false, false, FLAT>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec,
+                                                   sorted ? SortIO{d_kctr + p + 1, d_keys, d_perm} : SortIO{nullptr, nullptr, nullptr}, timed ? 1 : 0);
+                if (timed) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
                 ++launches;
             }
             if (sorted && !last) {                                           // work order of the next pass: travelling survivors by volume key
@@ -1076,8 +767,7 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
         if (refill) {                                        // one persistent launch per batch: as many blocks as fit on the chip
             unsigned* d_next = (unsigned*)((char*)d_stats + 256);
             int per_sm = 0, sms = 0;
-            auto kern = track ? (geo->coherent ? transport_refill<R, true, false> : transport_refill<R, true, true>)
-                              : (geo->coherent ? transport_refill<R, false, false> : transport_refill<R, false, true>);
+            auto kern = track ? transport_refill<R, true, FLAT> : transport_refill<R, false, FLAT>;
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TR_THREADS, 0);
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, geo->device);
             const unsigned blocks = std::min<unsigned>((n0 + TR_THREADS - 1) / TR_THREADS, (unsigned)std::max(1, per_sm * sms));
@@ -1124,211 +814,3 @@ int transport_impl(const gn_geometry* geo, const gn_source* h_src, uint64_t seed
 }
 
 }  // namespace gn
-
-using namespace gn;
-
-extern "C" int gn_nav_locate(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, int64_t n,
-                             int32_t* d_vol_out, void* cuda_stream) {
-    if (!geo || n < 0 || (n > 0 && (!d_pos || !d_vol_out))) return fail(GN_INVALID_ARGUMENT, "gn_nav_locate: bad argument");
-    if (precision == 32) return locate_impl<float>(geo, d_pos, d_dir, n, d_vol_out, (cudaStream_t)cuda_stream);
-    if (precision == 64) return locate_impl<double>(geo, d_pos, d_dir, n, d_vol_out, (cudaStream_t)cuda_stream);
-    return fail(GN_INVALID_ARGUMENT, "gn_nav_locate: precision must be 32 or 64");
-}
-
-extern "C" int gn_nav_compute_step(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir,
-                                   const int32_t* d_vol_in, const void* d_max_step, int64_t n, void* d_step_out,
-                                   int32_t* d_next_vol_out, void* cuda_stream) {
-    if (!geo || n < 0 || (n > 0 && (!d_pos || !d_dir || !d_vol_in || !d_step_out || !d_next_vol_out)))
-        return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step: bad argument");
-    if (precision == 32) return step_impl<float>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, (cudaStream_t)cuda_stream);
-    if (precision == 64) return step_impl<double>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, (cudaStream_t)cuda_stream);
-    return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step: precision must be 32 or 64");
-}
-
-extern "C" int gn_transport_run(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed, int64_t first_photon_id,
-                                int64_t n_photons, double* d_edep_out, gn_run_stats* h_stats_out, uint64_t* d_hash_out,
-                                uint32_t* d_nsteps_out, double* d_efinal_out, void* cuda_stream) {
-    if (!geo || !h_src || !d_edep_out || n_photons < 0 || first_photon_id < 0) return fail(GN_INVALID_ARGUMENT, "gn_transport_run: bad argument");
-    if (h_stats_out) std::memset(h_stats_out, 0, sizeof *h_stats_out);
-    if (precision == 32) return transport_impl<float>(geo, h_src, seed, first_photon_id, n_photons, d_edep_out, h_stats_out, d_hash_out, d_nsteps_out, d_efinal_out, (cudaStream_t)cuda_stream);
-    if (precision == 64) return transport_impl<double>(geo, h_src, seed, first_photon_id, n_photons, d_edep_out, h_stats_out, d_hash_out, d_nsteps_out, d_efinal_out, (cudaStream_t)cuda_stream);
-    return fail(GN_INVALID_ARGUMENT, "gn_transport_run: precision must be 32 or 64");
-}
-
-template <class R> int step_normal_impl(const gn_geometry* geo, const void* pos, const void* dir, const int32_t* vol, const void* ms,
-                                        int64_t n, void* step, int32_t* next, void* normal, cudaStream_t s) {
-    if (n == 0) return GN_OK;
-    if (geo->coherent) step_normal_kernel<R, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, (R*)normal);
-    else step_normal_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, (R*)normal);
-    GN_CUDA(cudaGetLastError(), "gn_nav_compute_step_normal launch");
-    return GN_OK;
-}
-
-extern "C" int gn_nav_compute_step_normal(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, const int32_t* d_vol_in,
-                                          const void* d_max_step, int64_t n, void* d_step_out, int32_t* d_next_vol_out, void* d_normal_out,
-                                          void* cuda_stream) {
-    if (!geo || n < 0 || (n > 0 && (!d_pos || !d_dir || !d_vol_in || !d_step_out || !d_next_vol_out || !d_normal_out)))
-        return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step_normal: bad argument");
-    if (precision == 32) return step_normal_impl<float>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, d_normal_out, (cudaStream_t)cuda_stream);
-    if (precision == 64) return step_normal_impl<double>(geo, d_pos, d_dir, d_vol_in, d_max_step, n, d_step_out, d_next_vol_out, d_normal_out, (cudaStream_t)cuda_stream);
-    return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_step_normal: precision must be 32 or 64");
-}
-
-extern "C" int gn_nav_compute_safety(const gn_geometry* geo, int precision, const void* d_pos, const int32_t* d_vol_in, int64_t n,
-                                     void* d_safety_out, void* cuda_stream) {
-    if (!geo || n < 0 || (n > 0 && (!d_pos || !d_vol_in || !d_safety_out))) return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_safety: bad argument");
-    if (precision != 32 && precision != 64) return fail(GN_INVALID_ARGUMENT, "gn_nav_compute_safety: precision must be 32 or 64");
-    if (n == 0) return GN_OK;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (precision == 32) safety_kernel<float><<<nav_grid(n), NAV_THREADS, 0, s>>>(geo->v32, (const float*)d_pos, d_vol_in, n, (float*)d_safety_out);
-    else safety_kernel<double><<<nav_grid(n), NAV_THREADS, 0, s>>>(geo->v64, (const double*)d_pos, d_vol_in, n, (double*)d_safety_out);
-    GN_CUDA(cudaGetLastError(), "gn_nav_compute_safety launch");
-    return GN_OK;
-}
-
-template <class R> int free_path_impl(const gn_geometry* geo, const void* pos, const void* dir, const void* Y, int64_t n, double mu_mass,
-                                      void* T, uint32_t* ns, cudaStream_t s) {
-    if (n == 0) return GN_OK;
-    const int64_t blocks = (n + NAV_THREADS - 1) / NAV_THREADS;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(blocks, 148 * 64));
-    if (geo->coherent) free_path_kernel<R, false><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
-    else free_path_kernel<R, true><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
-    GN_CUDA(cudaGetLastError(), "gn_free_path_run launch");
-    return GN_OK;
-}
-
-extern "C" int gn_free_path_run(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir, const void* d_Y, int64_t n,
-                                double mu_mass_cm2_g, void* d_T_out, uint32_t* d_nsteps_out, void* cuda_stream) {
-    if (!geo || n < 0 || !(mu_mass_cm2_g >= 0) || (n > 0 && (!d_pos || !d_dir || !d_Y || !d_T_out)))
-        return fail(GN_INVALID_ARGUMENT, "gn_free_path_run: bad argument");
-    if (precision == 32) return free_path_impl<float>(geo, d_pos, d_dir, d_Y, n, mu_mass_cm2_g, d_T_out, d_nsteps_out, (cudaStream_t)cuda_stream);
-    if (precision == 64) return free_path_impl<double>(geo, d_pos, d_dir, d_Y, n, mu_mass_cm2_g, d_T_out, d_nsteps_out, (cudaStream_t)cuda_stream);
-    return fail(GN_INVALID_ARGUMENT, "gn_free_path_run: precision must be 32 or 64");
-}
-
-extern "C" int gn_free_path_run_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, const void* h_Y, int64_t n,
-                                     double mu_mass_cm2_g, void* h_T_out, uint32_t* h_nsteps_out) {
-    if (!geo || n < 0 || (precision != 32 && precision != 64) || (n > 0 && (!h_pos || !h_dir || !h_Y || !h_T_out)))
-        return fail(GN_INVALID_ARGUMENT, "gn_free_path_run_host: bad argument");
-    if (n == 0) return GN_OK;
-    const size_t rs = precision == 32 ? 4 : 8;
-    const size_t b3 = 3 * rs * (size_t)n, b1 = rs * (size_t)n, bi = 4 * (size_t)n;
-    char* d = nullptr;
-    if (cudaMalloc((void**)&d, 2 * b3 + 2 * b1 + bi) != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, "gn_free_path_run_host: cudaMalloc"); }
-    char *dp = d, *dd = d + b3, *dY = d + 2 * b3, *dT = dY + b1, *dn = dT + b1;
-    // Algorithm 2 phases 4-6: transfer the particle states and lifetimes, compute, transfer T back
-    cudaError_t e = cudaMemcpy(dp, h_pos, b3, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(dd, h_dir, b3, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(dY, h_Y, b1, cudaMemcpyHostToDevice);
-    int rc = GN_OK;
-    if (e == cudaSuccess) rc = gn_free_path_run(geo, precision, dp, dd, dY, n, mu_mass_cm2_g, dT, h_nsteps_out ? (uint32_t*)dn : nullptr, nullptr);
-    if (rc == GN_OK && e == cudaSuccess) e = cudaMemcpy(h_T_out, dT, b1, cudaMemcpyDeviceToHost);
-    if (rc == GN_OK && e == cudaSuccess && h_nsteps_out) e = cudaMemcpy(h_nsteps_out, dn, bi, cudaMemcpyDeviceToHost);
-    cudaFree(d);
-    if (rc != GN_OK) return rc;
-    if (e != cudaSuccess) return cuda_fail(e, "gn_free_path_run_host");
-    return GN_OK;
-}
-
-extern "C" int gn_nav_query_host(const gn_geometry* geo, int precision, const void* h_pos, const void* h_dir, int64_t n,
-                                 int32_t* h_vol_out, void* h_step_out, int32_t* h_next_vol_out) {
-    if (!geo || n < 0 || (precision != 32 && precision != 64) || (n > 0 && (!h_pos || !h_dir || !h_vol_out || !h_step_out || !h_next_vol_out)))
-        return fail(GN_INVALID_ARGUMENT, "gn_nav_query_host: bad argument");
-    if (n == 0) return GN_OK;
-    const size_t rs = precision == 32 ? 4 : 8;
-    char* d = nullptr;
-    const size_t b_pos = 3 * rs * (size_t)n, b_i = 4 * (size_t)n, b_r = rs * (size_t)n;
-    cudaError_t e = cudaMalloc((void**)&d, 2 * b_pos + 2 * b_i + b_r);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, "gn_nav_query_host: cudaMalloc"); }
-    char *dp = d, *dd = d + b_pos, *dstep = d + 2 * b_pos, *dvol = dstep + b_r, *dnext = dvol + b_i;
-    int rc = GN_OK;
-    e = cudaMemcpy(dp, h_pos, b_pos, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(dd, h_dir, b_pos, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) {
-        rc = gn_nav_locate(geo, precision, dp, dd, n, (int32_t*)dvol, nullptr);
-        if (rc == GN_OK) rc = gn_nav_compute_step(geo, precision, dp, dd, (const int32_t*)dvol, nullptr, n, dstep, (int32_t*)dnext, nullptr);
-    }
-    if (rc == GN_OK && e == cudaSuccess) e = cudaMemcpy(h_vol_out, dvol, b_i, cudaMemcpyDeviceToHost);
-    if (rc == GN_OK && e == cudaSuccess) e = cudaMemcpy(h_step_out, dstep, b_r, cudaMemcpyDeviceToHost);
-    if (rc == GN_OK && e == cudaSuccess) e = cudaMemcpy(h_next_vol_out, dnext, b_i, cudaMemcpyDeviceToHost);
-    cudaFree(d);
-    if (rc != GN_OK) return rc;
-    if (e != cudaSuccess) return cuda_fail(e, "gn_nav_query_host");
-    return GN_OK;
-}
-
-extern "C" int gn_transport_run_host(const gn_geometry* geo, int precision, const gn_source* h_src, uint64_t seed,
-                                     int64_t first_photon_id, int64_t n_photons, double* h_edep_out, gn_run_stats* h_stats_out) {
-    if (!geo || !h_edep_out) return fail(GN_INVALID_ARGUMENT, "gn_transport_run_host: bad argument");
-    const size_t bytes = sizeof(double) * (size_t)geo->n_places;
-    double* d = nullptr;
-    std::lock_guard<std::mutex> host_lock(geo->host_mutex);
-    {   // the device staging buffer of the tally belongs to the handle (no allocation per call)
-        if (!geo->ws_host_edep && cudaMalloc((void**)&geo->ws_host_edep, bytes) != cudaSuccess) {
-            cudaGetLastError(); geo->ws_host_edep = nullptr;
-            return fail(GN_OUT_OF_MEMORY, "gn_transport_run_host: cudaMalloc");
-        }
-        d = geo->ws_host_edep;
-    }
-    int rc = gn_transport_run(geo, precision, h_src, seed, first_photon_id, n_photons, d, h_stats_out, nullptr, nullptr, nullptr, nullptr);
-    if (rc != GN_OK) return rc;
-    cudaError_t e = cudaMemcpy(h_edep_out, d, bytes, cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess) return cuda_fail(e, "gn_transport_run_host");
-    return GN_OK;
-}
-
-// -------------------------------------------------------------------------------------------------------
-// arithmetic self-test: the in-line correctly rounded fp32 division / square root of nav.cuh against the
-// toolchain's __fdiv_rn / __fsqrt_rn (IEEE round-to-nearest), bit for bit
-// -------------------------------------------------------------------------------------------------------
-namespace gn {
-__device__ __forceinline__ uint32_t mix32(uint64_t z) {          // splitmix64 finaliser
-    z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull; z = (z ^ (z >> 27)) * 0x94d049bb133111ebull; z ^= z >> 31;
-    return (uint32_t)(z >> 16);
-}
-__global__ void selftest_sqrt_kernel(unsigned long long* out) {
-    unsigned bad = 0;
-    for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < (1ull << 32); i += (uint64_t)gridDim.x * blockDim.x) {
-        float a = __uint_as_float((uint32_t)i);
-        float mine = rsqrt_(a), ref = __fsqrt_rn(a);
-        bool same = __float_as_uint(mine) == __float_as_uint(ref) || (mine != mine && ref != ref);
-        if (!same) { ++bad; atomicMin(&out[2], (unsigned long long)i); }
-    }
-    if (bad) atomicAdd(&out[0], (unsigned long long)bad);
-}
-__global__ void selftest_div_kernel(unsigned long long n, unsigned long long* out) {
-    unsigned bad = 0;
-    for (uint64_t i = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
-        uint32_t ua = mix32(2 * i + 1), ub = mix32(2 * i + 2) ^ 0x9e3779b9u;
-        const unsigned mode = (unsigned)(i & 3);
-        if (mode == 1) {                      // exponents of lengths and direction cosines: 2^-24 .. 2^16
-            ua = (ua & 0x807fffffu) | ((103u + (ua >> 23) % 40u) << 23); ub = (ub & 0x807fffffu) | ((103u + (ub >> 23) % 40u) << 23);
-        } else if (mode == 2) {               // quotient just below / above a power of two and a rounding boundary
-            ub = (ub & 0x807fffffu) | (127u << 23); ua = (ua & 0x80000000u) | ((ub & 0x7fffffffu) + (ua & 3u) - 1u);
-        } else if (mode == 3) {               // few mantissa bits: exact and half-way cases
-            ua &= 0xfff80000u; ub &= 0xffe00000u;
-        }
-        float a = __uint_as_float(ua), b = __uint_as_float(ub);
-        float mine = rdiv(a, b), ref = __fdiv_rn(a, b);
-        bool same = __float_as_uint(mine) == __float_as_uint(ref) || (mine != mine && ref != ref);
-        const float ar = fabsf(ref);
-        if (!same && ar < 1.17549435e-38f) same = fabsf(mine) < 1.17549435e-38f * 1.0001f;      // subnormal quotients: out of contract
-        if (!same) { ++bad; atomicMin(&out[3], (unsigned long long)i); }
-    }
-    if (bad) atomicAdd(&out[1], (unsigned long long)bad);
-}
-}  // namespace gn
-
-extern "C" int gn_selftest_arith(int64_t n_div_pairs, uint64_t h_out[4]) {
-    if (!h_out || n_div_pairs < 0) return fail(GN_INVALID_ARGUMENT, "gn_selftest_arith: bad argument");
-    unsigned long long* d = nullptr;
-    if (cudaMalloc((void**)&d, 32) != cudaSuccess) { cudaGetLastError(); return fail(GN_OUT_OF_MEMORY, "gn_selftest_arith: cudaMalloc"); }
-    unsigned long long init[4] = {0, 0, ~0ull, ~0ull};
-    cudaMemcpy(d, init, 32, cudaMemcpyHostToDevice);
-    selftest_sqrt_kernel<<<148 * 16, 256>>>(d);
-    if (n_div_pairs > 0) selftest_div_kernel<<<148 * 16, 256>>>((unsigned long long)n_div_pairs, d);
-    cudaError_t e = cudaMemcpy(h_out, d, 32, cudaMemcpyDeviceToHost);
-    cudaFree(d);
-    if (e != cudaSuccess) return cuda_fail(e, "gn_selftest_arith");
-    return GN_OK;
-}

@@ -83,3 +83,30 @@ def test_shard_ranges():
             for (a, ca), (b, _) in zip(spans[:-1], spans[1:]):
                 assert a + ca == b
             assert max(c for _, c in spans) - min(c for _, c in spans) <= 1
+
+
+def test_setup_arithmetic_agrees_with_the_oracle_bit_for_bit(lib):
+    """The library and the oracle derive the source frame and the composed transforms by their own code (hostmath.h's vector /
+    matrix helpers vs the oracle's explicit loops); the definitions fix the order of
+    the fp64 operations, so the rounded results must be equal bit for bit.  Host-only: needs no GPU."""
+    import oracle
+    from paper_1209_5235_b200 import binding as B, workloads as W
+    rng = np.random.default_rng(12)
+    axes = [(0, 0, 1.0), (1.0, 0, 0), (0, -2.0, 0), (1.0, 1.0, 1.0), (0.3, -0.3, 0.3), (1e-3, 5.0, -2.0)] + [tuple(rng.normal(size=3)) for _ in range(200)]
+    for ax in axes:
+        src = W.Source(W.SRC_CONE, (1.0, 2.0, 3.0), ax, W.E_MONO, 1.0, half_angle=0.1)
+        for precision in (64, 32):
+            a = B.host_source_frame(src, precision); b = oracle.source_frame(src, precision)
+            assert np.array_equal(a, b), (ax, precision)
+            if precision == 64:                      # and it is a right-handed orthonormal frame
+                assert np.allclose(a @ a.T, np.eye(3), atol=1e-14) and np.allclose(np.cross(a[0], a[1]), a[2], atol=1e-14)
+    for geom in (W.slab_geometry(1), W.detector_geometry(seed=4, n_phi=16, n_z=8, barrels=((200, 400), (450, 650))), W.lattice_geometry(4, seed=7),
+                 W.cms_like_geometry()):
+        M, T = B.host_compose_transforms(geom)
+        Mo, To = oracle.OracleGeometry(geom).composed_transforms(64)
+        assert np.array_equal(M, Mo) and np.array_equal(T, To), geom.name
+    # the hook validates like gn_geometry_create
+    g = W.slab_geometry(1)
+    bad = W.Geometry(g.materials, g.solid_type, g.solid_params, g.placements[::-1].copy(), g.transforms)
+    with pytest.raises(B.GammaNavError):
+        B.host_compose_transforms(bad)
