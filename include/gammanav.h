@@ -67,6 +67,10 @@ typedef struct {
                                   particles") as one persistent kernel per batch: each lane follows its photon to the end and
                                   then takes the next photon id from a device counter.  Same per-photon results as the default
                                   wavefront passes (0); cannot be combined with secondaries */
+    int32_t no_voxel_pass;     /* 1: keep the general lean step pass even when the geometry is mostly regular voxels (a voxel
+                                  phantom of unrotated boxes), for which the default (0) schedules the regular-voxel step kernel
+                                  plus a slow wavefront for every other step; same per-photon results either way */
+    int32_t reserved;
 } gn_opts;
 
 /* Photon source.  axis need not be normalised. */

@@ -28,7 +28,8 @@ class GammaNavError(RuntimeError):
 class Opts(C.Structure):
     _fields_ = [("tol64", C.c_double), ("tol32", C.c_double), ("sigma_pe0", C.c_double), ("e_cut", C.c_double),
                 ("voxel_min_daughters", C.c_int32), ("stuck_limit", C.c_int32), ("steps_per_pass", C.c_int32), ("first_pass_steps", C.c_int32),
-                ("tail_photons", C.c_int32), ("regroup_percent", C.c_int32), ("secondaries", C.c_int32), ("refill", C.c_int32)]
+                ("tail_photons", C.c_int32), ("regroup_percent", C.c_int32), ("secondaries", C.c_int32), ("refill", C.c_int32),
+                ("no_voxel_pass", C.c_int32), ("reserved", C.c_int32)]
 
 
 class CSource(C.Structure):

@@ -146,7 +146,7 @@ int parse_solid(int type, const double* q, HostSolid& out, const char** why) {
     }
 }
 
-struct HostGrid { int n[3]; double gmin[3], w[3]; int cell_base; };
+struct HostGrid { int n[3]; double gmin[3], w[3]; int cell_base; int mother; };
 
 }  // namespace
 }  // namespace gn
@@ -161,6 +161,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: NULL argument");
     if (n_mats <= 0 || n_solids <= 0 || n_places <= 0 || n_transforms <= 0)
         return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: empty table");
+    if (n_solids > NODE_SOLID_MASK + 1) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: at most 65536 solids (the node record keeps 16 bits for the solid index)");
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) {
         cudaGetLastError();
@@ -329,8 +330,12 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
                     for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
                         cand[pos[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++] = d;
         }
-        // regular voxels: an unrotated leaf box that fills exactly one cell, alone
-        for (int j = 0; j < nd; ++j) {
+        // regular voxels: an unrotated leaf box that fills exactly one cell, alone -- in a mother that is a box spanned exactly
+        // by the grid (so that cells at the rim are the only ones next to the mother's surface) and whose cells are much
+        // wider than the tolerances (the probe distance is a small fraction of a voxel)
+        bool regular_mother = ms.type == GN_BOX;
+        for (int k = 0; k < 3; ++k) regular_mother = regular_mother && G.w[k] >= 16.0 * std::max(geo->tol32, geo->tol64) + 64.0 * ext * 0x1p-23;
+        for (int j = 0; j < nd && regular_mother; ++j) {
             int d = dlist[kids[mth].x + j];
             if (kids[d].y != 0 || solids[node[d].y].type != GN_BOX) continue;
             const double* Rl = h_transforms + 12 * (size_t)h_placements[4 * (size_t)d + 3];
@@ -344,6 +349,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             if (count[cell] != 1) continue;
             regular_cell[d] = c0[3 * (size_t)j] | (c0[3 * (size_t)j + 1] << 10) | (c0[3 * (size_t)j + 2] << 20);
         }
+        G.mother = (int)mth;
         node[mth].w = (int)grids.size();
         grids.push_back(G);
         geo->n_cells += (int64_t)ncell;
@@ -366,7 +372,15 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         a.mat = b.mat = node[i].z;
         a.ndau = b.ndau = kids[i].y;
         a.link = b.link = node[i].w >= 0 ? ~node[i].w : kids[i].x;        // voxelised mother: ~grid id
-        if (regular_cell[i] >= 0) { a.info = b.info = a.info | NODE_REGULAR; a.link = b.link = regular_cell[i]; }
+        if (regular_cell[i] >= 0 && node[node[i].x].w <= NODE_GRID_MASK) {
+            const int gid = node[node[i].x].w;                              // grid of the mother
+            const HostGrid& G = grids[gid];
+            const int c[3] = {regular_cell[i] & 1023, (regular_cell[i] >> 10) & 1023, (regular_cell[i] >> 20) & 1023};
+            int walls = 0;
+            for (int k = 0; k < 3; ++k) walls |= (c[k] == 0 ? 1 << (2 * k) : 0) | (c[k] == G.n[k] - 1 ? 2 << (2 * k) : 0);
+            a.info = b.info = a.info | NODE_REGULAR | (gid << NODE_GRID_SHIFT) | (walls << NODE_WALL_SHIFT);
+            a.link = b.link = c[0] + G.n[0] * (c[1] + G.n[1] * c[2]);
+        }
         b.pad = 0;
         for (int k = 0; k < 3; ++k) { b.t[k] = Tg[3 * i + k]; a.t[k] = (float)Tg[3 * i + k]; }
     }
@@ -393,6 +407,20 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             (k == 0 ? b.eps0 : (k == 1 ? b.eps1 : b.eps2)) = e64;
         }
         a.cell_base = b.cell_base = G.cell_base;
+        a.sy = b.sy = G.n[0]; a.sz = b.sz = G.n[0] * G.n[1];
+        a.gpad = b.gpad = 0;
+        {   // dense: cell c holds exactly the regular voxel with node index base + c
+            int base = -1; bool dense = true;
+            const size_t ncell = (size_t)G.n[0] * G.n[1] * G.n[2];
+            for (size_t c = 0; c < ncell && dense; ++c) {
+                const int lo = cell_start[G.cell_base + c], cnt = cell_start[G.cell_base + c + 1] - lo;
+                if (cnt != 1) { dense = false; break; }
+                const int d = cand[lo];
+                if (c == 0) base = d;
+                dense = d == base + (int)c && regular_cell[d] >= 0 && (int)c == (regular_cell[d] & 1023) + G.n[0] * (((regular_cell[d] >> 10) & 1023) + G.n[1] * ((regular_cell[d] >> 20) & 1023));
+            }
+            a.dense = b.dense = dense ? base : -1;
+        }
         g32.push_back(a); g64.push_back(b);
     }
     std::vector<int2> cells(cell_start.size() - 1);
@@ -405,6 +433,9 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         for (size_t i = 0; i < V; ++i) coherent = coherent && solids[node[i].y].type == GN_BOX && (n32[i].info & NODE_IDENTITY);
         for (const int2& c : cells) coherent = coherent && c.y <= 1;
         geo->coherent = coherent;
+        size_t n_regular = 0;
+        for (size_t i = 0; i < V; ++i) n_regular += (n32[i].info & NODE_REGULAR) ? 1 : 0;
+        geo->voxel_sched = coherent && 2 * n_regular >= V && geo->opts.no_voxel_pass <= 0 && n_solids <= 32 && n_mats <= 32 && grids.size() <= 8 && ext < 0x1p50;      // table sizes: MAX_SMEM_* of common.cuh
         if (regroup_default) geo->opts.regroup_percent = coherent ? 50 : 75;
     }
     Uploader up{geo};

@@ -9,9 +9,13 @@
 //             v_local = w (the general fma chain gives the same values; only the sign of zeros can differ,
 //             which no comparison in the navigator can see) and `rot` is never read for this node
 //             flag NODE_REGULAR (leaf boxes only): the box coincides with exactly one cell of its mother's voxel grid,
-//             is that cell's only candidate and is not rotated against the mother; link = ix | iy << 10 | iz << 20
-//             (its cell).  A photon leaving it through a face or an edge finds the candidates in the neighbouring
-//             cells directly, without the general cell lookup (nav.cuh: settle, box-only kernels)
+//             is that cell's only candidate and is not rotated against the mother; link = index of its cell in the mother's
+//             grid (ix + nx (iy + ny iz)); bits 16..21 of info = id of that grid, bits 22..27 = "wall" bits: bit 22 + 2 k
+//             (+ 1) is set when the cell is the first (last) one of the grid along axis k, i.e. no neighbour cell there.
+//             A photon leaving it through a face or an edge finds the candidates in the neighbouring cells directly,
+//             without the general cell lookup (nav.cuh: settle, regular_step; box-only kernels).  Only mothers that are
+//             unrotated boxes whose grid spans them exactly hand out this flag, so a point within the probe distance of
+//             the voxel whose neighbour cell on that side exists is inside the mother by more than delta
 //   rot[i]    M (row-major, global->local rotation), 9 Real padded to 12 (fp32, three 16-byte loads) /
 //             10 (fp64, five 16-byte loads);  p_local = M (x - Tg)
 //   solids, mats, grids: small tables (staged to shared memory by every kernel)
@@ -24,7 +28,7 @@ namespace gn {
 
 enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2, SOLID_CONE = 3 };
 enum : int { TUBE_SECTOR = 1, TUBE_HOLE = 2 };
-enum : int { NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SOLID_MASK = (1 << 29) - 1 };
+enum : int { NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SOLID_MASK = 0xffff, NODE_GRID_SHIFT = 16, NODE_GRID_MASK = 0x3f, NODE_WALL_SHIFT = 22, NODE_WALL_MASK = 0x3f };
 
 template <class R> struct SolidRec {
     R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -      CONE: r0 = (r1 + r2)/2, slope m, hz
@@ -49,6 +53,10 @@ template <class R> struct alignas(16) GridRec {
     int n[3];
     int cell_base;        // offset of this grid's cells in `cells`
     R w[3], eps2;
+    int sy, sz;           // cell strides along y and z: n[0], n[0] n[1]
+    int dense;            // >= 0: every cell holds exactly one candidate, the regular voxel with node index dense + cell index
+                          // (the candidate of a cell needs no look-up); -1 otherwise
+    int gpad;
     __host__ __device__ R eps(int k) const { return k == 0 ? eps0 : (k == 1 ? eps1 : eps2); }
 };
 

@@ -43,6 +43,9 @@ constexpr int TR_WARPS = TR_THREADS / 32;
 #endif
 constexpr int REFILL_BATCH = 8;       // empty lanes that trigger a warp's refill (persistent refill kernel)
 constexpr int INTERACT_BATCH = 8;     // parked lanes that trigger a warp's interaction phase
+#ifndef GENERAL_BATCH
+#define GENERAL_BATCH 8            // box-only kernels: lanes waiting for the general ComputeStep that trigger it
+#endif
 enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
 enum : int { FATE_ALIVE = 0, FATE_ABSORBED = 1, FATE_ESCAPED = 2, FATE_STUCK = 3, FATE_NONE = 4 };
 enum : int { ST_STEPS = 0, ST_COMPTON, ST_PE, ST_PAIR, ST_CUT, ST_ESCAPED, ST_STUCK, ST_PHOTONS };
@@ -52,7 +55,13 @@ struct DevStats {
     unsigned long long cnt[8];       // ST_*
     unsigned long long lean_steps;   // steps taken inside the lean wavefront passes (the dominant kernel)
     double en[4];                    // EN_*
+    unsigned long long dbg[8];       // GN_DEBUG_COUNTERS builds only: fast steps, bails, general phases, general lane-steps, iterations
 };
+#ifdef GN_DEBUG_COUNTERS
+#define GN_DBG(i, v) atomicAdd(&stats->dbg[i], (unsigned long long)(v))
+#else
+#define GN_DBG(i, v) ((void)0)
+#endif
 // survivors of a pass: key-0 photons fill the output queue from the front, key-1 photons from the back
 struct PassCounters { unsigned front, back; };
 // general geometries: the travelling survivors of a pass are also counted by volume key, and a small kernel turns the
@@ -296,6 +305,32 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             if (fate != FATE_ALIVE) history_out(pp, sec, idx, h, misc >> 8, E);
         }
     };
+    // what a ComputeStep does to the photon (Algorithm 1 loop body): (vol, nd) already hold the volume
+    // after the boundary; inter = the interaction point s_int comes first (S_j >= Y inside vol_before)
+    auto apply_step = [&](bool inter, R s_int, R step, const V3<R>& xn, R mu, int vol_before) {
+        ++c_steps; misc += 0x100u;
+        const R len = inter ? s_int : step;
+        uint32_t zs = misc & 0xffu;
+        zs = (len <= g.delta) ? min(zs + 1u, 255u) : 0u;                  // saturates: stuck_limit <= 255 is enforced at create time
+        misc = (misc & ~0xffu) | zs;
+        if (inter) {
+            x = advance(x, w, s_int);
+            pending = true;
+        } else {                                                           // boundary: S_j update
+            x = xn;
+            Y = rmax(Y - step * mu, (R)0);
+            int ev = EV_BOUNDARY;
+            if (vol < 0) { ev = EV_ESCAPE; fate = FATE_ESCAPED; }
+            finish_step(ev, vol_before);
+        }
+    };
+    // Box-only kernels: photons inside regular voxels take regular_step (nav.cuh); whoever cannot (another kind of volume, an
+    // exit through an edge or out of the mother, ...) waits for the general ComputeStep, which the warp runs once
+    // GENERAL_BATCH lanes wait, when no lane could take the short step, or in the last iteration of the pass.
+    constexpr bool FASTV = !FLAT;
+    VoxLane<R> vl; vl.hx = vl.hy = vl.hz = 0; vl.r0 = vl.r1 = vl.r2 = 0; vl.solid = -1; vl.ok = false;
+    if (FASTV && fate == FATE_ALIVE) lane_direction(w, g.delta, vl);
+    bool bailed = false;                                                   // regular_step gave up on this photon's next step
     int act0 = 32;
 #pragma unroll 1
     for (int k = 0;;) {
@@ -321,7 +356,10 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
                     E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
                     atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
                     if (ev == EV_CUT) { atomicAdd(&sh_cnt[ST_CUT], 1ull); fate = FATE_ABSORBED; }
-                    else { Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above; }
+                    else {
+                        Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above;
+                        if (FASTV) lane_direction(w, g.delta, vl);
+                    }
                 } else {
                     atomicAdd(&sh_cnt[ev == EV_PE ? ST_PE : ST_PAIR], 1ull);
                     fate = FATE_ABSORBED;
@@ -340,32 +378,42 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             else if (__popc(act) * 100 < act0 * regroup_pct) break;
         }
         ++k;
-        if (fate == FATE_ALIVE && !pending) {
+        bool todo = fate == FATE_ALIVE && !pending;                            // this lane wants a step
+        R mu = 0;
+        if (todo) {
             const MatRec<R> m = mats[nd.mat];
             const R muPE = m.aPE * gPE, muC = m.aC * gKN;
             const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
             const R muP = (above && P > 0) ? m.aP * P : (R)0;
-            const R mu = (muPE + muC) + muP;
+            mu = (muPE + muC) + muP;
+        }
+        if (FASTV) {
+            bool stepped = false;
+            if (todo && !bailed && vl.ok && (nd.info & NODE_REGULAR)) {
+                if ((nd.info & NODE_SOLID_MASK) != vl.solid) lane_solid(nav.solids, nd.info, vl);
+                R step = 0; V3<R> xn{0, 0, 0};
+                const int vol_before = vol;
+                const int rc = regular_step(g, nav.grids, x, w, vl, mu, Y, vol, nd, step, xn);
+                if (rc == REG_BAIL) { bailed = true; GN_DBG(1, 1); }
+                else {
+                    GN_DBG(0, 1);
+                    apply_step(rc == REG_INTERACT, step, step, xn, mu, vol_before);
+                    stepped = true; todo = false;
+                }
+            }
+            const unsigned waiting = __ballot_sync(0xffffffffu, todo);
+            if (waiting && !(__popc(waiting) >= GENERAL_BATCH || !__any_sync(0xffffffffu, stepped) || k >= K)) todo = false;      // wait
+        }
+        if (lane == 0) GN_DBG(4, 1);
+        if (todo) { GN_DBG(3, 1); }
+        if (__any_sync(0xffffffffu, todo) && lane == 0) GN_DBG(2, 1);
+        if (todo) {
             const R s_int = mu > 0 ? rdiv(Y, mu) : rinf<R>();                  // remaining part of Eq. 7
             const int vol_before = vol;
             R step; V3<R> xn;
             nav.compute_step(vol, nd, x, w, s_int, step, xn);                  // "next intersection"
-            ++c_steps; misc += 0x100u;
-            const bool inter = step == rinf<R>();                              // S_j >= Y: the photon interacts in vol
-            const R len = inter ? s_int : step;
-            uint32_t zs = misc & 0xffu;
-            zs = (len <= g.delta) ? min(zs + 1u, 255u) : 0u;                  // saturates: stuck_limit <= 255 is enforced at create time
-            misc = (misc & ~0xffu) | zs;
-            if (inter) {
-                x = advance(x, w, s_int);
-                pending = true;
-            } else {                                                           // boundary: S_j update
-                x = xn;
-                Y = rmax(Y - step * mu, (R)0);
-                int ev = EV_BOUNDARY;
-                if (vol < 0) { ev = EV_ESCAPE; fate = FATE_ESCAPED; }
-                finish_step(ev, vol_before);
-            }
+            apply_step(step == rinf<R>(), s_int, step, xn, mu, vol_before);
+            bailed = false;
         }
     }
 
@@ -621,6 +669,10 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
 }
 
+}  // namespace gn
+#include "voxel_pass.cuh"
+namespace gn {
+
 constexpr int64_t TR_BATCH = 1ll << 24;     // photons per batch (bounds scratch at 2 x 16.8 M x 64 B = 2.1 GB in fp32)
 constexpr int TR_MAX_PASSES = 4096;         // device counters per batch; the last one always runs to completion
 constexpr int TR_LAG = 2;                   // the host looks at survivor counts that are this many passes old
@@ -732,11 +784,25 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             } else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass; the
                 // first TR_TIMED lean passes of a batch are timed one by one, and only their steps count as lean_steps
-                launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
                 const bool timed = n_timed < TR_TIMED;
-                if (timed) cudaEventRecord(tev[2 * n_timed], s);
-                launch_pass<R, false, false, FLAT>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec,
-                                                   sorted ? SortIO{d_kctr + p + 1, d_keys, d_perm} : SortIO{nullptr, nullptr, nullptr}, timed ? 1 : 0);
+                bool voxel = false;
+                if constexpr (!FLAT) voxel = geo->voxel_sched;
+                if (voxel) {
+                    // voxel phantoms: the slow wavefront (general steps of the flagged photons, interactions of the parked ones),
+                    // then the regular-voxel step pass (voxel_pass.cuh)
+                    if constexpr (!FLAT) {
+                        if (track) slow_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
+                        else slow_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
+                        if (timed) cudaEventRecord(tev[2 * n_timed], s);
+                        if (track) voxel_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
+                        else voxel_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
+                    }
+                } else {
+                    launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
+                    if (timed) cudaEventRecord(tev[2 * n_timed], s);
+                    launch_pass<R, false, false, FLAT>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K, regroup, sec,
+                                                       sorted ? SortIO{d_kctr + p + 1, d_keys, d_perm} : SortIO{nullptr, nullptr, nullptr}, timed ? 1 : 0);
+                }
                 if (timed) { cudaEventRecord(tev[2 * n_timed + 1], s); ++n_timed; }
                 ++launches;
             }
@@ -808,6 +874,9 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             h_stats->e_escaped = hs.en[EN_ESCAPED]; h_stats->e_stuck = hs.en[EN_STUCK]; h_stats->e_source = hs.en[EN_SOURCE]; h_stats->e_deposited = hs.en[EN_DEPOSITED];
             h_stats->n_passes = passes; h_stats->n_kernel_launches = launches; h_stats->kernel_ms = kernel_ms;
             h_stats->step_pass_ms = step_pass_ms; h_stats->n_steps_step_pass = hs.lean_steps;
+#ifdef GN_DEBUG_COUNTERS
+            fprintf(stderr, "[gn debug] fast steps %llu, bails %llu, general phases (warps) %llu, general lane-steps %llu, warp iterations %llu\n", hs.dbg[0], hs.dbg[1], hs.dbg[2], hs.dbg[3], hs.dbg[4]);
+#endif
         }
     }
     return rc;
