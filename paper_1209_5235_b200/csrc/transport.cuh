@@ -63,7 +63,7 @@ struct DevStats {
 #define GN_DBG(i, v) ((void)0)
 #endif
 // survivors of a pass: key-0 photons fill the output queue from the front, key-1 photons from the back
-struct PassCounters { unsigned front, back; };
+struct PassCounters { unsigned front, back, slow, pad; };      // slow: photons flagged for the general step (voxel schedule: buffer S)
 // general geometries: the travelling survivors of a pass are also counted by volume key, and a small kernel turns the
 // keys into the work order of the next pass (sort_scatter_kernel), so that its warps are mostly of one kind
 struct KeyCounters { unsigned long long tot[SORT_KEYS], cur[SORT_KEYS]; unsigned long long pad[2]; };
@@ -713,7 +713,10 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
     const size_t pb = secondaries ? cap * sizeof(PairVtx<R>) + 16 : 0;          // pair vertices of a batch + their count
     const size_t hb2 = (secondaries && track) ? cap * 8 : 0;                    // hash state of a batch of annihilation photons
     const size_t base = (2 * qb + hb + 512 + cb + kb + sb + 15) & ~(size_t)15;
-    const size_t need = base + pb + hb2;
+    bool voxel_sched = false;
+    if constexpr (!FLAT) voxel_sched = geo->voxel_sched;
+    const size_t vb = voxel_sched ? qb : 0;                    // buffer S of the voxel schedule: photons flagged for the general step
+    const size_t need = base + pb + hb2 + vb + 16;
     std::lock_guard<std::mutex> lock(geo->ws_mutex);          // one run at a time per handle: the workspace is shared
     GN_CUDA(cudaMemsetAsync(d_edep, 0, sizeof(double) * (size_t)geo->n_places, s), "gn_transport_run memset edep");
     if (geo->ws_bytes < need) {
@@ -742,6 +745,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
     unsigned* d_npairs = secondaries ? (unsigned*)(scratch + base) : nullptr;
     PairVtx<R>* d_pairs = secondaries ? (PairVtx<R>*)(scratch + base + 16) : nullptr;
     uint64_t* sec_hash = hb2 ? (uint64_t*)(scratch + base + pb) : nullptr;
+    PhotonRec<R>* d_slow = vb ? (PhotonRec<R>*)(scratch + ((base + pb + hb2 + 15) & ~(size_t)15)) : nullptr;
     int rc = GN_OK;
     uint64_t passes = 0, launches = 0;
     cudaEvent_t ev0 = geo->ws_events[0], ev1 = geo->ws_events[1];
@@ -770,7 +774,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             if (p > TR_LAG) {
                 e = cudaEventSynchronize(ring[(p - TR_LAG) % (TR_LAG + 1)]);
                 if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pass"); break; }
-                ub = h_ctr[p - TR_LAG].front + h_ctr[p - TR_LAG].back;        // input count of pass p - TR_LAG >= that of pass p
+                ub = h_ctr[p - TR_LAG].front + h_ctr[p - TR_LAG].back + h_ctr[p - TR_LAG].slow;      // input count of pass p - TR_LAG >= that of pass p
                 if (ub == 0) break;
             }
             const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
@@ -779,6 +783,11 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
                 launch_pass<R, true, false, FLAT>(track, blocks, s, g, src, seed, fid, n0, nullptr, d_ctr + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, k_first, regroup, sec,
                                                   sorted ? SortIO{d_kctr + 1, d_keys, nullptr} : SortIO{nullptr, nullptr, nullptr});
             } else if (last) {
+                if constexpr (!FLAT) if (geo->voxel_sched) {                 // the flagged photons of the last voxel_pass rejoin the queue
+                    if (track) general_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_slow, in, (uint32_t)cap, d_stats, pp, sec);
+                    else general_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_slow, in, (uint32_t)cap, d_stats, pp, sec);
+                    ++launches;
+                }
                 launch_pass<R, false, true, FLAT>(track, blocks, s, g, src, seed, fid, 0u, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_edep, d_stats, pp, K_UNLIMITED, regroup, sec,
                                                   sorted ? SortIO{nullptr, nullptr, d_perm} : SortIO{nullptr, nullptr, nullptr});
             } else {
@@ -791,11 +800,13 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
                     // voxel phantoms: the slow wavefront (general steps of the flagged photons, interactions of the parked ones),
                     // then the regular-voxel step pass (voxel_pass.cuh)
                     if constexpr (!FLAT) {
-                        if (track) slow_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
-                        else slow_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
+                        if (track) general_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_slow, in, (uint32_t)cap, d_stats, pp, sec);
+                        else general_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_slow, in, (uint32_t)cap, d_stats, pp, sec);
+                        launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
                         if (timed) cudaEventRecord(tev[2 * n_timed], s);
-                        if (track) voxel_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
-                        else voxel_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
+                        if (track) voxel_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, d_slow, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
+                        else voxel_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, d_slow, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
+                        ++launches;
                     }
                 } else {
                     launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
