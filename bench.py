@@ -26,6 +26,12 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 ALGO_BYTES = {("transport", 32): 96.0, ("transport", 64): 160.0, ("nav", 32): 64.0, ("nav", 64): 116.0}
+# Algorithmic flops per step (configs 1-4) / per query (config 5): operation count of the oracle's algorithm on the config's own
+# workload, measured with the oracle's counting Real (SURVEY 8(d) "instrumented oracle": + - * / sqrt compare = 1, fma = 2,
+# transcendental = 1).  bench.py re-measures it in the cpu_baseline leg; these are the committed values of that measurement
+# (oracle.transport_count_ops on the first 20000 photons / oracle.nav_count_ops on 20000 queries), used with --no-cpu-baseline.
+ALGO_FLOPS = {1: 366.6, 2: 467.4, 3: 606.1, 4: 584.7, 5: 841.9}
+PIPE_PEAK_FALLBACK = {32: 74.4, 64: 37.2}   # nominal TFLOP/s (148 SMs x 128 / 64 lanes x 2 x 1.965 GHz) when the self-test cannot run
 
 
 def measured_peaks():
@@ -121,6 +127,20 @@ def oracle_rate(k, precision, sample, cores=1):
     units = sum(u for u, _ in res)
     dt = max(d for _, d in res)            # excludes geometry construction, like the GPU side
     return units / dt, units, wall
+
+
+def oracle_flops_per_unit(k, n_sample):
+    """Flops per step / query of config k from the instrumented oracle (counting Real), on the first n_sample units."""
+    import oracle
+    from paper_1209_5235_b200 import workloads as W
+    wl = W.config(k)
+    og = oracle.OracleGeometry(wl.geometry)
+    if wl.source is not None:
+        c, st = og.transport_count_ops(wl.source, wl.seed, n_sample)
+        return c["flops"] / max(1, st["n_steps"]), {n: v / max(1, st["n_steps"]) for n, v in c.items()}
+    pos, dirs = W.nav_queries(wl.geometry, n_sample, seed=wl.seed)
+    c = og.nav_count_ops(pos, dirs)
+    return c["flops"] / n_sample, {n: v / n_sample for n, v in c.items()}
 
 
 def run_reference(args):
@@ -390,35 +410,18 @@ def run_ours(args):
         e2e = {"value": world * m / dt, "unit": "ComputeStep queries/s", "h2d_bytes_per_step": 6 * rs * m, "d2h_bytes_per_step": (8 + rs) * m,
                "note": f"{m} queries per call, inputs from and results to page-locked host memory, chunks of 2^22 on two streams"}
 
+    pipe = None
+    if rank == 0:
+        try:
+            pipe = B.selftest_pipe_peak(precision)            # FFMA / DFMA pipe peak at the clock of this run (after the timed region)
+        except Exception:
+            pipe = None
     if rank == 0:
         peak, peak_src = measured_peaks()
         kind = "transport" if transport else "nav"
         abytes = ALGO_BYTES[(kind, precision)]
-        # dominant kernel = transport_pass (the only kernel of the step); its launch durations are measured with CUDA
-        # events on the launching stream inside gn_transport_run (stats.kernel_ms), summed over the step's launches
-        whole = (units / world) * abytes / (kernel_ms * 1e-3) / 1e9 if kernel_ms > 0 else None
-        if transport and dom[1] > 0:
-            # the dominant kernel alone: steps taken inside the lean wavefront step passes x algorithmic bytes / the summed
-            # launch durations of those passes (one CUDA-event pair per launch on the launching stream, inside gn_transport_run)
-            achieved = dom[0] * abytes / (dom[1] * 1e-3) / 1e9
-        else:
-            achieved = whole
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get(f"{wl.name}_fp{precision}")
-            except Exception:
-                traffic = None
-        roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                    "traffic": traffic, "peak_source": peak_src,
-                    "kernel": "transport_pass<R,0,0,0> (lean wavefront step pass)" if transport else "locate_kernel + query sort + step_kernel",
-                    "algorithmic_bytes_per_unit": abytes,
-                    "kernel_steps_per_run": dom[0] / args.steps if transport else None, "kernel_ms_per_run": dom[1] / args.steps if transport else kernel_ms / args.steps,
-                    "whole_run": {"achieved": whole, "frac": (whole / peak) if whole else None, "ms_per_run": kernel_ms / args.steps,
-                                  "note": "all kernels of a run (source pass, step passes, interaction passes, tail): steps of the run x algorithmic bytes / CUDA-event time of the whole sequence"},
-                    "note": "achieved = algorithmic bytes of the dominant kernel's launches / their summed CUDA-event durations; traffic = ncu dram bytes of all launches of one run (profiles/traffic.json)"}
         cpu = None
+        flops_per_unit, flops_src, op_mix = ALGO_FLOPS[args.config], "committed measurement of the instrumented oracle (bench.py ALGO_FLOPS)", None
         if not args.no_cpu_baseline:
             sample = {1: 10000, 2: 100000, 3: 1500000, 4: 400000, 5: 20000000}[args.config]
             v1, u1, d1 = oracle_rate(args.config, precision, sample, 1)
@@ -428,6 +431,47 @@ def run_ours(args):
                 nc = os.cpu_count() or 1
                 vN, uN, dN = oracle_rate(args.config, precision, sample * min(nc, 8), nc)
                 cpu["all_cores"] = {"value": vN, "cores": nc, "wall_s": dN}
+            flops_per_unit, op_mix = oracle_flops_per_unit(args.config, 20000)
+            flops_src = "instrumented oracle (counting Real) on the first 20000 units of this workload, this run"
+        pipe_tflops = pipe["tflops"] if pipe else PIPE_PEAK_FALLBACK[precision]
+        pipe_src = f"gn_selftest_pipe_peak ({'FFMA' if precision == 32 else 'DFMA'} chains, {pipe['sm_mhz']:.0f} MHz)" if pipe else "nominal (self-test unavailable)"
+        # per-unit roofline: the slower of algorithmic bytes at HBM bandwidth and algorithmic flops at pipe peak
+        t_hbm, t_alu = abytes / (peak * 1e9), flops_per_unit / (pipe_tflops * 1e12)
+        bound = "hbm" if t_hbm >= t_alu else "alu"
+
+        def fracs(rate):                                       # units / s -> (frac_hbm, frac_alu)
+            return (rate * t_hbm, rate * t_alu) if rate else (None, None)
+        whole_rate = (units / world) / (kernel_ms * 1e-3) if kernel_ms > 0 else None
+        # dominant kernel = the lean step pass (voxel_pass for phantoms): steps taken inside its timed launches / their summed
+        # CUDA-event durations (one event pair per launch on the launching stream, inside gn_transport_run)
+        dom_rate = dom[0] / (dom[1] * 1e-3) if (transport and dom[1] > 0) else whole_rate
+        dh, da = fracs(dom_rate); wh, wa = fracs(whole_rate)
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(f"{wl.name}_fp{precision}")
+            except Exception:
+                traffic = None
+        if bound == "hbm":
+            ach, pk, un, fr = (dom_rate * abytes / 1e9 if dom_rate else None), peak, "GB/s", dh
+        else:
+            ach, pk, un, fr = (dom_rate * flops_per_unit / 1e12 if dom_rate else None), pipe_tflops, "TFLOP/s", da
+        voxel = transport and wl.name.startswith("config3")
+        roofline = {"bound": bound, "achieved": ach, "peak": pk, "unit": un, "frac": fr, "traffic": traffic,
+                    "peak_source": peak_src if bound == "hbm" else pipe_src,
+                    "kernel": ("voxel_pass (regular-voxel step pass)" if voxel else "transport_pass<R,0,0,0> (lean wavefront step pass)") if transport else "locate_kernel + query sort + step_kernel",
+                    "algorithmic_bytes_per_unit": abytes, "flops_per_unit": flops_per_unit, "flops_source": flops_src,
+                    "hbm_peak_gbs": peak, "pipe_peak_tflops": pipe_tflops, "pipe_peak_source": pipe_src,
+                    "frac_hbm": dh, "frac_alu": da,
+                    "kernel_steps_per_run": dom[0] / args.steps if transport else None, "kernel_ms_per_run": dom[1] / args.steps if transport else kernel_ms / args.steps,
+                    "whole_run": {"frac": wh if bound == "hbm" else wa, "frac_hbm": wh, "frac_alu": wa, "ms_per_run": kernel_ms / args.steps,
+                                  "note": "all kernels of a run: units of the run / CUDA-event time of the whole launch sequence"},
+                    "note": "bound = the slower of (algorithmic bytes / measured HBM bandwidth) and (algorithmic flops / measured pipe peak) per unit; "
+                            "a fraction above 1 on the HBM leg means the kernel does not move the algorithmic bytes: a pass keeps the photon in registers "
+                            "for up to K steps, so the record is read and written once per pass, not once per step (traffic = ncu dram bytes of one run)"}
+        if op_mix:
+            roofline["ops_per_unit"] = op_mix
         line = {"metric": "transported photon steps/s" if transport else "ComputeStep queries/s",
                 "value": units / (ms * 1e-3), "unit": "photon-steps/s" if transport else "ComputeStep queries/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
