@@ -15,7 +15,7 @@ def build(force: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-mfma", "-mavx2", "-fPIC", "-shared",
-           "-Wall", "-Wextra", "-o", LIB, SRC]
+           "-Wall", "-Wextra"] + os.environ.get("ORACLE_CXXFLAGS", "").split() + ["-o", LIB, SRC]      # e.g. -fsanitize=address,undefined -g
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -62,6 +62,15 @@ struct DevStats {
 #else
 #define GN_DBG(i, v) ((void)0)
 #endif
+// Checked builds (-DGN_CHECKED; compute-sanitizer is closed on the GPU pool): the invariants a memory checker would watch --
+// every queue slot, node index and buffer index in range, the queue segments never overlapping -- are tested in the kernels;
+// a violation sets bit `code` of stats->dbg[7] and gn_transport_run returns GN_CUDA_ERROR naming the bits.
+#ifdef GN_CHECKED
+#define GN_CHECK(cond, code) do { if (!(cond)) atomicOr(&stats->dbg[7], 1ull << (code)); } while (0)
+#else
+#define GN_CHECK(cond, code) ((void)0)
+#endif
+enum : int { CHK_LOAD_SLOT = 0, CHK_STORE_SLOT = 1, CHK_VOLUME = 2, CHK_SEGMENTS = 3, CHK_SLOW_SLOT = 4, CHK_PHOTON_INDEX = 5, CHK_PAIR_SLOT = 6, CHK_MATERIAL = 7 };
 // survivors of a pass: key-0 photons fill the output queue from the front, key-1 photons from the back
 struct PassCounters { unsigned front, back, slow, pad; };      // slow: photons flagged for the general step (voxel schedule: buffer S)
 // general geometries: the travelling survivors of a pass are also counted by volume key, and a small kernel turns the
@@ -285,7 +294,10 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         c_phot = warp_sum(c_phot); e_src = warp_sum(e_src);
         if (lane == 0) { atomicAdd(&sh_cnt[ST_PHOTONS], (unsigned long long)c_phot); atomicAdd(&sh_en[EN_SOURCE], e_src); }
     } else if (fate == FATE_ALIVE) {
-        PhotonRec<R> r; load_rec(qin, i < n_front ? ((FLAT && sio.perm_in) ? sio.perm_in[i] : i) : cap - 1u - (i - n_front), r);
+        const unsigned slot_in = i < n_front ? ((FLAT && sio.perm_in) ? sio.perm_in[i] : i) : cap - 1u - (i - n_front);
+        GN_CHECK(slot_in < cap && n_in <= cap, CHK_LOAD_SLOT);
+        PhotonRec<R> r; load_rec(qin, slot_in, r);
+        GN_CHECK(r.vol < g.n_nodes && (r.vol < 0 || g.node[r.vol].mat < g.n_mats), CHK_VOLUME);
         if (r.vol < 0) fate = FATE_NONE;                 // absorbed by interact_pass
         x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
         gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = (int)(r.tail[0] & 1u); pending = (r.tail[0] & 2u) != 0;
@@ -439,6 +451,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 #pragma unroll
         for (int q = 0; q < (int)(sizeof(r.tail) / 4); ++q) r.tail[q] = 0;
         r.tail[0] = (uint32_t)above | (pending ? 2u : 0u);
+        GN_CHECK(o < cap && vol >= 0 && vol < g.n_nodes, CHK_STORE_SLOT);
         store_rec(qout, o, r);
         if (TRACK) pp.hash[idx] = h;
         if (FLAT && sio.keys_out && !key1) {                                 // volume key of a travelling survivor
@@ -462,6 +475,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         }
     }
     __syncthreads();
+    GN_CHECK(cout->front + cout->back <= cap, CHK_SEGMENTS);
     if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
     if (!FROM_SOURCE && !PHYS && timed && threadIdx.x == 12 && sh_cnt[ST_STEPS]) atomicAdd(&stats->lean_steps, sh_cnt[ST_STEPS]);
@@ -486,8 +500,10 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
     const bool active = i < n;
     double dep_d = 0.0; int vol = 0;
     if (active) {
+        GN_CHECK(n <= cap, CHK_LOAD_SLOT);
         PhotonRec<R> r; load_rec(q, cap - 1u - i, r);
         vol = r.vol;
+        GN_CHECK(vol >= 0 && vol < g.n_nodes && g.node[vol].mat < g.n_mats, CHK_VOLUME);
         const int above = (int)(r.tail[0] & 1u);
         const MatRec<R> m = g.mats[__ldg(&g.node[vol].mat)];
         const R muPE = m.aPE * r.gPE, muC = m.aC * r.gKN;
@@ -498,7 +514,7 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         io.E = r.E; io.wx = r.wx; io.wy = r.wy; io.wz = r.wz; io.Y = r.Y; io.gPE = r.gPE; io.gKN = r.gKN; io.L2k = r.L2k; io.j = r.ctr; io.above = above;
         interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + (sec.in ? sec.in[r.idx >> 1].idx : r.idx), sec.in ? 1u + (r.idx & 1u) : 0u, sec.out != nullptr);
         int ev = io.ev;
-        if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = r.x; pv.y = r.y; pv.z = r.z; pv.idx = r.idx; sec.out[atomicAdd(sec.n_out, 1u)] = pv; }
+        if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = r.x; pv.y = r.y; pv.z = r.z; pv.idx = r.idx; const unsigned ps = atomicAdd(sec.n_out, 1u); GN_CHECK(ps < cap, CHK_PAIR_SLOT); sec.out[ps] = pv; }
         dep_d = (double)io.dep;
         bool alive = false;
         if (ev == EV_COMPTON || ev == EV_CUT) {
@@ -879,6 +895,9 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
         e = cudaMemcpyAsync(&hs, d_stats, sizeof hs, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) rc = cuda_fail(e, "gn_transport_run stats");
+#ifdef GN_CHECKED
+        else if (hs.dbg[7]) { char msg[96]; snprintf(msg, sizeof msg, "gn_transport_run (checked build): invariant bits 0x%llx violated", hs.dbg[7]); rc = fail(GN_CUDA_ERROR, msg); }
+#endif
         else if (h_stats) {
             h_stats->n_steps = hs.cnt[ST_STEPS]; h_stats->n_compton = hs.cnt[ST_COMPTON]; h_stats->n_pe = hs.cnt[ST_PE]; h_stats->n_pair = hs.cnt[ST_PAIR];
             h_stats->n_cut = hs.cnt[ST_CUT]; h_stats->n_escaped = hs.cnt[ST_ESCAPED]; h_stats->n_stuck = hs.cnt[ST_STUCK]; h_stats->n_photons = hs.cnt[ST_PHOTONS];

@@ -59,8 +59,10 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
     VoxLane<R> vl; vl.hx = vl.hy = vl.hz = 0; vl.r0 = vl.r1 = vl.r2 = 0; vl.solid = -1; vl.ok = false;
     unsigned c_steps = 0;
     if (alive) {
+        GN_CHECK(n_in <= cap, CHK_LOAD_SLOT);
         PhotonRec<R> r; load_rec(qin, i < n_front ? i : cap - 1u - (i - n_front), r);
-        if (r.vol < 0) alive = false;                        // ended in slow_pass
+        GN_CHECK(r.vol < g.n_nodes, CHK_VOLUME);
+        if (r.vol < 0) alive = false;                        // absorbed by interact_pass
         x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
         gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = r.tail[0] & REC_ABOVE;
         pending = (r.tail[0] & REC_PENDING) != 0;
@@ -131,6 +133,9 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
 #pragma unroll
         for (int q = 0; q < (int)(sizeof(r.tail) / 4); ++q) r.tail[q] = 0;
         r.tail[0] = above | (pending ? REC_PENDING : 0u);
+        GN_CHECK(vol >= 0 && vol < g.n_nodes && nd.mat < g.n_mats, CHK_VOLUME);
+        GN_CHECK(!key2 || sh_base[2] + sh_wcount[2][warp] + __popc(bal2 & below) < cap, CHK_SLOW_SLOT);
+        GN_CHECK(key2 || (key1 ? sh_base[1] + sh_wcount[1][warp] + __popc(bal1 & below) : sh_base[0] + sh_wcount[0][warp] + __popc(bal0 & below)) < cap, CHK_STORE_SLOT);
         if (key2) store_rec(S, sh_base[2] + sh_wcount[2][warp] + __popc(bal2 & below), r);
         else store_rec(qout, key1 ? cap - 1u - (sh_base[1] + sh_wcount[1][warp] + __popc(bal1 & below)) : sh_base[0] + sh_wcount[0][warp] + __popc(bal0 & below), r);
         if (TRACK && c_steps) pp.hash[idx] = h;
@@ -145,6 +150,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
         }
     }
     __syncthreads();
+    GN_CHECK(cout->front + cout->back + cout->slow <= cap, CHK_SEGMENTS);
     if (threadIdx.x == 0) {
         if (sh_steps) { atomicAdd(&stats->cnt[ST_STEPS], sh_steps); if (timed) atomicAdd(&stats->lean_steps, sh_steps); }
         if (sh_stuck) { atomicAdd(&stats->cnt[ST_STUCK], sh_stuck); atomicAdd(&stats->en[EN_STUCK], sh_estuck); }
@@ -179,7 +185,9 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
     PhotonRec<R> r;
     unsigned c_steps = 0, c_esc = 0, c_stuck = 0; double e_esc = 0.0, e_stuck = 0.0;
     if (alive) {
+        GN_CHECK(n <= cap, CHK_SLOW_SLOT);
         load_rec(S, i, r);
+        GN_CHECK(r.vol >= 0 && r.vol < g.n_nodes, CHK_VOLUME);
         V3<R> x{r.x, r.y, r.z};
         const V3<R> w{r.wx, r.wy, r.wz};
         R Y = r.Y;
@@ -226,6 +234,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
         if (lane == 0) { if (b0) base0 = atomicAdd(&ctr->front, (unsigned)__popc(b0)); if (b1) base1 = atomicAdd(&ctr->back, (unsigned)__popc(b1)); }
         base0 = __shfl_sync(0xffffffffu, base0, 0); base1 = __shfl_sync(0xffffffffu, base1, 0);
         const unsigned below = (1u << lane) - 1u;
+        GN_CHECK(!alive || (pending ? base1 + __popc(b1 & below) : base0 + __popc(b0 & below)) < cap, CHK_STORE_SLOT);
         if (alive) store_rec(q, pending ? cap - 1u - (base1 + __popc(b1 & below)) : base0 + __popc(b0 & below), r);
     }
     {
@@ -235,6 +244,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
         if (ns) { const double es = warp_sum(e_stuck); if (lane == 0) { atomicAdd(&sh_cnt[ST_STUCK], (unsigned long long)ns); atomicAdd(&sh_en[EN_STUCK], es); } }
     }
     __syncthreads();
+    GN_CHECK(ctr->front + ctr->back <= cap, CHK_SEGMENTS);
     if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
 }
