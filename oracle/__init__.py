@@ -18,7 +18,8 @@ _lib = None
 
 class Opts(C.Structure):
     _fields_ = [("tol64", C.c_double), ("tol32", C.c_double), ("sigma_pe0", C.c_double), ("e_cut", C.c_double),
-                ("grid_min_daughters", C.c_int32), ("stuck_limit", C.c_int32), ("secondaries", C.c_int32), ("reserved", C.c_int32)]
+                ("grid_min_daughters", C.c_int32), ("stuck_limit", C.c_int32), ("secondaries", C.c_int32), ("rayleigh", C.c_int32),
+                ("sigma_r0", C.c_double), ("pe_table_per_decade", C.c_int32), ("pe_k_edge", C.c_int32)]
 
 
 class CSource(C.Structure):
@@ -28,7 +29,7 @@ class CSource(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons")] + \
-               [(n, C.c_double) for n in ("e_escaped", "e_stuck", "e_source", "e_deposited")]
+               [(n, C.c_double) for n in ("e_escaped", "e_stuck", "e_source", "e_deposited")] + [("n_rayleigh", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -45,6 +46,7 @@ def lib():
         L.oracle_sigma_pe.restype = C.c_double; L.oracle_sigma_pe.argtypes = [C.c_double, C.c_double, C.c_double]
         L.oracle_uniform_from_lane.restype = C.c_double; L.oracle_uniform_from_lane.argtypes = [C.c_uint64, C.c_int]
         L.oracle_draw.restype = C.c_double; L.oracle_draw.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_int]
+        L.oracle_mu_rayleigh.restype = C.c_double; L.oracle_mu_rayleigh.argtypes = [C.c_void_p, C.c_int, C.c_int32, C.c_double]
         L.oracle_fnv1a_bytes.restype = C.c_uint64; L.oracle_fnv1a_bytes.argtypes = [C.c_void_p, C.c_int64]
         L.oracle_history_hash.restype = C.c_uint64; L.oracle_history_hash.argtypes = [C.c_void_p, C.c_int64]
         _lib = L
@@ -182,6 +184,9 @@ class OracleGeometry:
                                           C.c_int(int(use_grid))), "free_path_run")
         return T, ns
 
+    def mu_rayleigh(self, material, E, precision=64):
+        return lib().oracle_mu_rayleigh(self._h, precision, int(material), float(E))
+
     def mu(self, material, E, precision=64):
         m = np.empty(3, np.float64)
         _check(lib().oracle_mu(self._h, C.c_int(precision), C.c_int32(material), C.c_double(E), _p(m)), "mu")
@@ -257,6 +262,13 @@ def kn_sample(E, seed, n, precision=64, first_id=0):
     eps = np.empty(n); cost = np.empty(n); nt = np.empty(n, np.int32)
     _check(lib().oracle_kn_sample(C.c_int(precision), C.c_double(E), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n), _p(eps), _p(cost), _p(nt)), "kn_sample")
     return eps, cost, nt
+
+
+def rayleigh_sample(seed, n, precision=64, first_id=0):
+    """n cosines of the Rayleigh scattering angle (rejection from 1 + c^2) and the trials each took."""
+    c = np.empty(n); nt = np.empty(n, np.int32)
+    _check(lib().oracle_rayleigh_sample(C.c_int(precision), C.c_uint64(seed), C.c_int64(first_id), C.c_int64(n), _p(c), _p(nt)), "rayleigh_sample")
+    return c, nt
 
 
 def rotate(w, cost, phi, precision=64):

@@ -131,6 +131,9 @@ struct Geo {
     std::vector<int> grid_of;                /* node -> index in grids or -1 */
     std::vector<Grid> grids;
     double tol64, tol32, sigma_pe0, e_cut; int stuck_limit, grid_min, secondaries;
+    int rayleigh = 0, pe_per_decade = 0, pe_k_edge = 0; double sigma_r0 = 0;
+    std::vector<double> aR;                       /* Rayleigh material factor n sigma_R0 (Z/13)^2 / 10 [1/mm at 1 MeV], fp64 */
+    std::vector<std::vector<double>> pe_tab;      /* per material: mu_PE [1/mm] on the grid E_k = 0.01 MeV 10^(k / P), k = 0 .. 5 P, fp64 */
 };
 
 template <class R> struct Sel;
@@ -668,6 +671,46 @@ template <class R> void mu_partials(const MaterialR<R>& m, const EnergyFactors<R
     mu[2] = (f.above_pair && P > 0) ? m.aP * P : (R)0;
 }
 
+/* D:reading 19, tabulated photoelectric coefficient.  Grid E_k = E_min 10^(k / P), E_min = 0.01 MeV, k = 0 .. 5 P (1 GeV).
+ * Table (fp64, at create time): T_k = n sigma_PE(E_k) / 10 with sigma_PE = sigma_PE0 (Z/82)^5 (0.1/E)^3.5, divided by the K jump
+ * ratio 5 below E_K = 13.6e-6 MeV (Z - 1)^2 when the edge model is on; rounded once to Real.
+ * Look-up: u = clamp((ln E - ln E_min) P / ln 10, 0, 5 P (1 - 2^-24)) in fp64, rounded once to Real, evaluated when the energy
+ * changes; per step i = floor(u), f = u - i, mu_PE = T_i + f (T_{i+1} - T_i) in Real, left to right. */
+const double kPeEmin = 0.01, kPeDecades = 5.0, kKJump = 5.0;
+double pe_sigma_tab(double E, double Z, double s0_barn, int k_edge) {
+    double s = s0_barn * kBarn * std::pow(Z / 82.0, 5.0) * std::pow(0.1 / E, 3.5);
+    if (k_edge) { double eK = 13.6e-6 * (Z - 1.0) * (Z - 1.0); if (E < eK) s = s / kKJump; }
+    return s;
+}
+template <class R> R pe_table_coordinate(R E, int per_decade) {
+    typedef typename Wide<R>::type W;
+    W u = (r_log<W>(W((double)E)) - W(std::log(kPeEmin))) * W((double)per_decade / std::log(10.0));
+    const W top(kPeDecades * per_decade * (1.0 - 0x1p-24));
+    if (u < W(0.0)) u = W(0.0);
+    if (u > top) u = top;
+    return (R)(double)u;
+}
+template <class R> R pe_table_mu(const std::vector<double>& T, R u) {
+    int i = (int)std::floor((double)u);
+    R f = u - (R)(double)i;
+    R t0 = (R)T[i], t1 = (R)T[i + 1];
+    return t0 + f * (t1 - t0);
+}
+/* D:reading 18, Rayleigh: mu_R = aR gR, aR = n sigma_R0 (Z/13)^2 / 10 (fp64 at create time, rounded once), gR = 1 / (E E)
+ * evaluated in Real (one product, one division) */
+template <class R> R mu_rayleigh(const Geo& g, int material, R E) {
+    if (!g.rayleigh) return (R)0;
+    return (R)g.aR[material] * ((R)1 / (E * E));
+}
+/* the four partial coefficients of material `mat` for a photon of energy E (factors f, table coordinate u) */
+template <class R> void mu_all(const Geo& g, int mat, R E, const EnergyFactors<R>& f, R u_pe, R mu4[4]) {
+    R m3[3]; mu_partials(Sel<R>::m(g)[mat], f, m3);
+    mu4[0] = g.pe_per_decade > 0 ? pe_table_mu<R>(g.pe_tab[mat], u_pe) : m3[0];
+    mu4[1] = m3[1];
+    mu4[2] = mu_rayleigh<R>(g, mat, E);
+    mu4[3] = m3[2];
+}
+
 /* ---- RNG (S:C7) ------------------------------------------------------------------------ */
 void philox4x32_10(uint32_t c[4], uint32_t k0, uint32_t k1) {
     for (int r = 0; r < 10; ++r) {
@@ -736,6 +779,18 @@ template <class R> void rotate_dir(R w[3], R cost, R sint, R phi) {
     w[0] = n[0] / nn; w[1] = n[1] / nn; w[2] = n[2] / nn;
 }
 
+/* Rayleigh angle (D:reading 18): cos(theta) from p(c) ~ 1 + c^2 on [-1, 1] by rejection, two draws per trial:
+ * c = 2 U1 - 1, accepted when 2 U2 <= 1 + c c.  Only + - * and a comparison: the same bits everywhere. */
+template <class R> int rayleigh_sample(Stream& rng, R& cost) {
+    int trials = 0;
+    for (;;) {
+        ++trials;
+        R u1 = rng.u<R>(), u2 = rng.u<R>();
+        R c = (R)2 * u1 - (R)1;
+        if ((R)2 * u2 <= (R)1 + c * c) { cost = c; return trials; }
+    }
+}
+
 /* ---- source (S:C8, D:"source frame") ---------------------------------------------------- */
 template <class R> struct SourceR {
     int kind, energy_kind;
@@ -797,7 +852,7 @@ inline void fnv_byte(uint64_t& h, uint8_t b) { h ^= b; h *= kFnvPrime; }
 inline void fnv_word(uint64_t& h, uint32_t w) {
     for (int i = 0; i < 4; ++i) fnv_byte(h, (uint8_t)((w >> (8 * i)) & 0xffu));
 }
-enum { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
+enum { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6, EV_RAYLEIGH = 7 };
 
 /* One history from (x, w, E) with stream rng: locate, first optical depth, then the loop of Algorithm 1.
  * Returns the history hash and the step count; E holds the energy at the end.  With g.secondaries (S:8(f) NEXT-3,
@@ -831,19 +886,19 @@ void pair_directions(uint64_t seed, uint64_t id, R w1[3], R w2[3], Stream& s1) {
 template <class R>
 History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t id, Stream& rng, R x[3], R w[3], R& E,
                  const Tally& edep, oracle_stats_t& st) {
-    const std::vector<MaterialR<R>>& mats = Sel<R>::m(g);
     const R twopi = (R)6.283185307179586;
     uint64_t h = kFnvOffset; uint32_t ns = 0;
     int vol = nav.locate(x, w);
     bool alive = true;
     if (vol < 0) { st.n_escaped++; st.e_escaped += (double)E; alive = false; }
-    R Y = 0; EnergyFactors<R> ef{};
-    if (alive) { Y = -r_log(rng.u<R>()); ef = energy_factors(E); }           /* Alg.1 steps 1-2 */
+    R Y = 0; EnergyFactors<R> ef{}; R u_pe = 0;
+    const bool pe_tab = g.pe_per_decade > 0;
+    if (alive) { Y = -r_log(rng.u<R>()); ef = energy_factors(E); if (pe_tab) u_pe = pe_table_coordinate<R>(E, g.pe_per_decade); }           /* Alg.1 steps 1-2 */
     int zero_steps = 0;
     bool annihilate = false;
     while (alive) {
-        R mu3[3]; mu_partials(mats[g.material[vol]], ef, mu3);
-        R mu = (mu3[0] + mu3[1]) + mu3[2];
+        R mu4[4]; mu_all<R>(g, g.material[vol], E, ef, u_pe, mu4);             /* PE, Compton, Rayleigh, pair */
+        R mu = ((mu4[0] + mu4[1]) + mu4[2]) + mu4[3];
         R s_int = mu > 0 ? Y / mu : r_inf<R>();                                 /* Eq.7 remaining part */
         R step; int next;
         nav.compute_step(vol, x, w, s_int, step, next);                         /* "next intersection" P:L67 */
@@ -853,9 +908,11 @@ History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t 
             len = s_int;
             for (int i = 0; i < 3; ++i) x[i] = r_fma(s_int, w[i], x[i]);
             R t = rng.u<R>() * mu;
-            if (t < mu3[0]) {                                                   /* photoelectric */
+            /* process choice (D:reading 2): cumulative thresholds; U = 1 falls to the last process with a non-zero coefficient */
+            const bool last_is_pair = mu4[3] > 0, last_is_rayleigh = !last_is_pair && mu4[2] > 0;
+            if (t < mu4[0]) {                                                   /* photoelectric */
                 edep.add(vol, (double)E); st.e_deposited += (double)E; st.n_pe++; ev = EV_PE; alive = false;
-            } else if (t < mu3[0] + mu3[1] || !(mu3[2] > 0)) {                  /* Compton */
+            } else if (t < mu4[0] + mu4[1] || (!last_is_pair && !last_is_rayleigh)) {       /* Compton */
                 R eps, cost, s2; kn_sample(E, rng, eps, cost, s2);
                 R Ep = eps * E;
                 R phi = twopi * rng.u<R>();
@@ -865,7 +922,14 @@ History<R> track(const Geo& g, const Navigator<R>& nav, uint64_t seed, uint64_t 
                 E = Ep;
                 if (Ep < (R)g.e_cut) { dep = dep + Ep; st.n_cut++; ev = EV_CUT; alive = false; }
                 edep.add(vol, (double)dep); st.e_deposited += (double)dep;
-                if (alive) { ef = energy_factors(E); Y = -r_log(rng.u<R>()); }
+                if (alive) { ef = energy_factors(E); if (pe_tab) u_pe = pe_table_coordinate<R>(E, g.pe_per_decade); Y = -r_log(rng.u<R>()); }
+            } else if (t < (mu4[0] + mu4[1]) + mu4[2] || last_is_rayleigh) {    /* Rayleigh: direction changes, energy does not */
+                R cost; rayleigh_sample<R>(rng, cost);
+                R sint = r_sqrt(r_max(((R)1 - cost) * ((R)1 + cost), (R)0));
+                R phi = twopi * rng.u<R>();
+                rotate_dir(w, cost, sint, phi);
+                st.n_rayleigh++; ev = EV_RAYLEIGH;
+                Y = -r_log(rng.u<R>());
             } else {                                                            /* pair */
                 R dep = g.secondaries ? E - (R)(2.0 * kMeC2) : E;               /* local deposit: all of E, or the pair's kinetic energy */
                 edep.add(vol, (double)dep); st.e_deposited += (double)dep; st.n_pair++; ev = EV_PAIR; alive = false;
@@ -1194,6 +1258,24 @@ int oracle_geometry_create(const double* materials, int32_t n_mats, const int32_
     g->grid_min = (opts && opts->grid_min_daughters > 0) ? opts->grid_min_daughters : 8;
     g->stuck_limit = (opts && opts->stuck_limit > 0) ? opts->stuck_limit : 8;
     g->secondaries = (opts && opts->secondaries > 0) ? 1 : 0;
+    g->rayleigh = (opts && opts->rayleigh > 0) ? 1 : 0;
+    g->sigma_r0 = (opts && opts->sigma_r0 > 0) ? opts->sigma_r0 : 7.886e-3;
+    g->pe_per_decade = (opts && opts->pe_table_per_decade > 0) ? opts->pe_table_per_decade : 0;
+    g->pe_k_edge = (opts && opts->pe_k_edge > 0) ? 1 : 0;
+    if (g->pe_per_decade > 4096) { delete g; return ORACLE_INVALID_ARGUMENT; }
+    for (const MaterialD& m : g->mats) {
+        double n = m.rho * kNA / m.A;
+        g->aR.push_back(n * (g->sigma_r0 * kBarn * (m.Z / 13.0) * (m.Z / 13.0)) / 10.0);
+        std::vector<double> T;
+        if (g->pe_per_decade > 0) {
+            int np = (int)(kPeDecades * g->pe_per_decade) + 1;
+            for (int k = 0; k < np; ++k) {
+                double Ek = kPeEmin * std::pow(10.0, (double)k / g->pe_per_decade);
+                T.push_back(n * pe_sigma_tab(Ek, m.Z, g->sigma_pe0, g->pe_k_edge) / 10.0);
+            }
+        }
+        g->pe_tab.push_back(T);
+    }
     for (const SolidD& s : g->solids) { g->s64.push_back(round_solid<double>(s)); g->s32.push_back(round_solid<float>(s)); }
     for (const MaterialD& m : g->mats) { g->m64.push_back(round_material<double>(m, g->sigma_pe0)); g->m32.push_back(round_material<float>(m, g->sigma_pe0)); }
     /* operation counter: the fp64 tables again, element by element, in the counting type */
@@ -1381,8 +1463,21 @@ double oracle_sigma_pe(double E, double Z, double s0) { return sigma_pe(E, Z, s0
 int oracle_mu(const void* geo, int precision, int32_t material, double E, double* mu3) {
     const Geo& g = *(const Geo*)geo;
     if (material < 0 || material >= (int)g.mats.size()) return ORACLE_INVALID_ARGUMENT;
-    if (precision == 64) { double m[3]; mu_partials(g.m64[material], energy_factors<double>(E), m); mu3[0] = m[0]; mu3[1] = m[1]; mu3[2] = m[2]; }
-    else { float m[3]; mu_partials(g.m32[material], energy_factors<float>((float)E), m); mu3[0] = m[0]; mu3[1] = m[1]; mu3[2] = m[2]; }
+    if (precision == 64) { double m[4]; mu_all<double>(g, material, E, energy_factors<double>(E), g.pe_per_decade > 0 ? pe_table_coordinate<double>(E, g.pe_per_decade) : 0.0, m); mu3[0] = m[0]; mu3[1] = m[1]; mu3[2] = m[3]; }
+    else { float e = (float)E, m[4]; mu_all<float>(g, material, e, energy_factors<float>(e), g.pe_per_decade > 0 ? pe_table_coordinate<float>(e, g.pe_per_decade) : 0.0f, m); mu3[0] = m[0]; mu3[1] = m[1]; mu3[2] = m[3]; }
+    return ORACLE_OK;
+}
+double oracle_mu_rayleigh(const void* geo, int precision, int32_t material, double E) {
+    const Geo& g = *(const Geo*)geo;
+    if (material < 0 || material >= (int)g.mats.size()) return -1.0;
+    return precision == 64 ? mu_rayleigh<double>(g, material, E) : (double)mu_rayleigh<float>(g, material, (float)E);
+}
+int oracle_rayleigh_sample(int precision, uint64_t seed, int64_t first_id, int64_t n, double* cost_out, int32_t* ntrials_out) {
+    for (int64_t i = 0; i < n; ++i) {
+        Stream s{seed, (uint64_t)(first_id + i), 0};
+        if (precision == 64) { double c; int t = rayleigh_sample<double>(s, c); cost_out[i] = c; if (ntrials_out) ntrials_out[i] = t; }
+        else { float c; int t = rayleigh_sample<float>(s, c); cost_out[i] = c; if (ntrials_out) ntrials_out[i] = t; }
+    }
     return ORACLE_OK;
 }
 

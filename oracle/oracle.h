@@ -35,7 +35,11 @@ typedef struct {
     int32_t grid_min_daughters; /* mothers with >= this many daughters get a locate grid; <=0 -> 8 */
     int32_t stuck_limit; /* consecutive steps of length <= delta before a photon is killed; <=0 -> 8 (C9) */
     int32_t secondaries; /* 1: a pair event deposits E - 2 me c^2 and two annihilation photons are followed (S:8(f) NEXT-3); 0: deposits E */
-    int32_t reserved;
+    int32_t rayleigh;    /* 1: coherent (Rayleigh) scattering is a fourth process (S:8(f) NEXT-3, D:reading 18); 0: off */
+    double sigma_r0;     /* Rayleigh cross-section of Z = 13 at 1 MeV [barn/atom]; <=0 -> 7.886e-3 (D:reading 18) */
+    int32_t pe_table_per_decade; /* > 0: the photoelectric coefficient comes from a per-material table with this many points per
+                                    decade of energy, 10 keV .. 1 GeV (S:8(f) NEXT-3, D:reading 19); 0: the closed form of C6 */
+    int32_t pe_k_edge;   /* with the table: 1 = the tabulated cross-section drops by the K jump ratio 5 below E_K = 13.6 eV (Z-1)^2 */
 } oracle_opts_t;
 
 typedef struct {
@@ -51,6 +55,7 @@ typedef struct {
 typedef struct {
     uint64_t n_steps, n_compton, n_pe, n_pair, n_cut, n_escaped, n_stuck, n_photons;
     double e_escaped, e_stuck, e_source, e_deposited;
+    uint64_t n_rayleigh; /* Rayleigh scatters (only with opts.rayleigh) */
 } oracle_stats_t;
 
 /* geometry ------------------------------------------------------------------------------ */
@@ -127,8 +132,12 @@ int oracle_solid_eval(int32_t type, const double* params5, double tol, int preci
 double oracle_sigma_kn(double k);                       /* Klein-Nishina total, cm^2 per electron */
 double oracle_sigma_pair(double k, double Z);           /* cm^2 per atom */
 double oracle_sigma_pe(double E, double Z, double sigma_pe0_barn); /* cm^2 per atom */
-/* mu[3] = (mu_PE, mu_C, mu_pair) in 1/mm for material m at energy E, in the given precision */
+/* mu[3] = (mu_PE, mu_C, mu_pair) in 1/mm for material m at energy E, in the given precision (mu_PE from the table when the
+ * geometry was created with pe_table_per_decade > 0); oracle_mu_rayleigh: mu_R (0 unless created with rayleigh = 1) */
 int oracle_mu(const void* geo, int precision, int32_t material, double E, double* mu3);
+double oracle_mu_rayleigh(const void* geo, int precision, int32_t material, double E);
+/* n cosines of the Rayleigh scattering angle, photon ids first_id.. (draws start at 0): rejection from p(c) ~ 1 + c^2 */
+int oracle_rayleigh_sample(int precision, uint64_t seed, int64_t first_id, int64_t n, double* cost_out, int32_t* ntrials_out);
 /* directions of the two annihilation photons of photon id's pair event (S:8(f) NEXT-3): n x 3 doubles each */
 int oracle_pair_directions(int precision, uint64_t seed, int64_t first_id, int64_t n, double* w1_out, double* w2_out);
 void oracle_philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t* out4);
