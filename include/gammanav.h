@@ -70,7 +70,17 @@ typedef struct {
     int32_t no_voxel_pass;     /* 1: keep the general lean step pass even when the geometry is mostly regular voxels (a voxel
                                   phantom of unrotated boxes), for which the default (0) schedules the regular-voxel step kernel
                                   plus a slow wavefront for every other step; same per-photon results either way */
-    int32_t reserved;
+    int32_t rayleigh;          /* 1: coherent (Rayleigh) scattering is a fourth process (reading 18):
+                                  mu_R = n sigma_R0 (Z/13)^2 / E^2, angle from 1 + cos^2(theta) by rejection, energy unchanged, nothing
+                                  deposited, event word 7; 0 (default): off (BASELINE.json config 1's physics) */
+    double sigma_r0;           /* Rayleigh cross-section of Z = 13 at 1 MeV [barn/atom]; default 7.886e-3 (the model's mu / rho of
+                                  aluminium at 1 MeV then equals PAPER.md L150's 0.06146 cm^2/g) */
+    int32_t pe_table_per_decade; /* > 0: the photoelectric coefficient comes from a per-material table with this many points per
+                                  decade over 10 keV .. 1 GeV, interpolated linearly in ln E (reading 19); 0 (default): the closed
+                                  form; at most 4096 */
+    int32_t pe_k_edge;         /* with the table: 1 = the tabulated cross-section drops by the K jump ratio 5 below
+                                  E_K = 13.6 eV (Z - 1)^2; 0 = the table is the Z^5 / E^3.5 law itself.
+                                  Either option switches the regular-voxel schedule off (the general passes handle them) */
 } gn_opts;
 
 /* Photon source.  axis need not be normalised. */
@@ -95,6 +105,7 @@ typedef struct {
     double step_pass_ms;       /* sum of the launch durations of the lean wavefront step passes (the dominant kernel), one
                                   CUDA-event pair per launch; only the first 64 such passes of each batch are timed */
     uint64_t n_steps_step_pass;/* steps taken inside exactly those timed passes (later lean passes count in n_steps only) */
+    uint64_t n_rayleigh;       /* Rayleigh scatters (gn_opts.rayleigh) */
 } gn_run_stats;
 
 /*

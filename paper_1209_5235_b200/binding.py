@@ -29,7 +29,7 @@ class Opts(C.Structure):
     _fields_ = [("tol64", C.c_double), ("tol32", C.c_double), ("sigma_pe0", C.c_double), ("e_cut", C.c_double),
                 ("voxel_min_daughters", C.c_int32), ("stuck_limit", C.c_int32), ("steps_per_pass", C.c_int32), ("first_pass_steps", C.c_int32),
                 ("tail_photons", C.c_int32), ("regroup_percent", C.c_int32), ("secondaries", C.c_int32), ("refill", C.c_int32),
-                ("no_voxel_pass", C.c_int32), ("reserved", C.c_int32)]
+                ("no_voxel_pass", C.c_int32), ("rayleigh", C.c_int32), ("sigma_r0", C.c_double), ("pe_table_per_decade", C.c_int32), ("pe_k_edge", C.c_int32)]
 
 
 class CSource(C.Structure):
@@ -41,7 +41,7 @@ class RunStats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons")] + \
                [(n, C.c_double) for n in ("e_escaped", "e_stuck", "e_source", "e_deposited")] + \
                [("n_passes", C.c_uint64), ("n_kernel_launches", C.c_uint64), ("kernel_ms", C.c_double), ("step_pass_ms", C.c_double),
-                ("n_steps_step_pass", C.c_uint64)]
+                ("n_steps_step_pass", C.c_uint64), ("n_rayleigh", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

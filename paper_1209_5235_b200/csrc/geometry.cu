@@ -226,6 +226,9 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     if (!(o.e_cut > 0)) o.e_cut = 0.010;
     if (o.voxel_min_daughters <= 0) o.voxel_min_daughters = 8;
     if (o.stuck_limit <= 0) o.stuck_limit = 8;
+    if (!(o.sigma_r0 > 0)) o.sigma_r0 = 7.886e-3;
+    if (o.pe_table_per_decade < 0) o.pe_table_per_decade = 0;
+    if (o.pe_table_per_decade > 4096) { gn_geometry_destroy(geo); return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: pe_table_per_decade must be <= 4096"); }
     if (o.stuck_limit > 255) { gn_geometry_destroy(geo); return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: stuck_limit must be <= 255 (the per-photon counter of consecutive short steps has 8 bits)"); }
     if (o.steps_per_pass <= 0) o.steps_per_pass = 16;
     if (o.first_pass_steps <= 0) o.first_pass_steps = 1;
@@ -435,7 +438,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         geo->coherent = coherent;
         size_t n_regular = 0;
         for (size_t i = 0; i < V; ++i) n_regular += (n32[i].info & NODE_REGULAR) ? 1 : 0;
-        geo->voxel_sched = coherent && 2 * n_regular >= V && geo->opts.no_voxel_pass <= 0 && n_solids <= 32 && n_mats <= 32 && grids.size() <= 8 && ext < 0x1p50;      // table sizes: MAX_SMEM_* of common.cuh
+        geo->voxel_sched = coherent && 2 * n_regular >= V && geo->opts.no_voxel_pass <= 0 && geo->opts.rayleigh <= 0 && geo->opts.pe_table_per_decade <= 0 && n_solids <= 32 && n_mats <= 32 && grids.size() <= 8 && ext < 0x1p50;      // table sizes: MAX_SMEM_* of common.cuh
         if (regroup_default) geo->opts.regroup_percent = coherent ? 50 : 75;
     }
     Uploader up{geo};
@@ -454,6 +457,28 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         std::vector<double> rho(n_mats);
         for (int i = 0; i < n_mats; ++i) rho[i] = h_materials[3 * i + 2];
         a.rho = b.rho = up.put(rho);
+    }
+    {   // optional physics: Rayleigh factors (reading 18) and the photoelectric table (reading 19), built in
+        // fp64 and rounded once per precision
+        const int P = o.pe_table_per_decade, points = P > 0 ? 5 * P + 1 : 0;
+        std::vector<float> r32(n_mats); std::vector<double> r64(n_mats);
+        std::vector<float> t32((size_t)points * n_mats); std::vector<double> t64((size_t)points * n_mats);
+        for (int i = 0; i < n_mats; ++i) {
+            const double Z = h_materials[3 * i], A = h_materials[3 * i + 1], rho = h_materials[3 * i + 2];
+            const double atoms = rho * kNA / A;                            // per cm^3
+            r64[i] = atoms * (o.sigma_r0 * kBarn * (Z / 13.0) * (Z / 13.0)) / 10.0; r32[i] = (float)r64[i];
+            const double k_edge = 13.6e-6 * (Z - 1.0) * (Z - 1.0);          // MeV
+            for (int k = 0; k < points; ++k) {
+                const double Ek = 0.01 * std::pow(10.0, (double)k / P);
+                double sigma = o.sigma_pe0 * kBarn * std::pow(Z / 82.0, 5.0) * std::pow(0.1 / Ek, 3.5);
+                if (o.pe_k_edge > 0 && Ek < k_edge) sigma = sigma / 5.0;  // below the K edge the K shell does not absorb
+                t64[(size_t)i * points + k] = atoms * sigma / 10.0; t32[(size_t)i * points + k] = (float)t64[(size_t)i * points + k];
+            }
+        }
+        a.mat_r = up.put(r32); b.mat_r = up.put(r64);
+        a.pe_tab = up.put(t32); b.pe_tab = up.put(t64);
+        a.rayleigh = b.rayleigh = o.rayleigh > 0 ? 1 : 0;
+        a.pe_per_decade = b.pe_per_decade = P; a.pe_points = b.pe_points = points;
     }
     a.tol = (float)geo->tol32; a.delta = a.tol / 2; a.probe = (float)(1.25 * 0.5 * geo->tol32 + 4.0 * ext * 0x1p-23); a.e_cut = (float)o.e_cut;
     b.tol = geo->tol64; b.delta = b.tol / 2; b.probe = 1.25 * 0.5 * geo->tol64 + 4.0 * ext * 0x1p-52; b.e_cut = o.e_cut;

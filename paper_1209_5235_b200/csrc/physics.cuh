@@ -62,7 +62,16 @@ __device__ __forceinline__ void rsincos(double a, double* s, double* c) { *s = s
 #define GN_PI 3.14159265358979323846
 template <class R> struct EnergyFactors { R gPE, gKN, L2k; int above_pair; };
 
-template <class R> __device__ EnergyFactors<R> energy_factors(R E) {
+// photoelectric table coordinate (reading 19): u = clamp((ln E - ln 0.01) P / ln 10, 0, 5 P (1 - 2^-24)), fp64, rounded once
+template <class R> __device__ __forceinline__ R pe_coordinate(R E, int per_decade) {
+    double u = (log((double)E) - log(0.01)) * ((double)per_decade / log(10.0));
+    const double top = 5.0 * per_decade * (1.0 - 0x1p-24);
+    if (u < 0.0) u = 0.0;
+    if (u > top) u = top;
+    return (R)u;
+}
+// gPE is the closed-form factor (0.1 / E)^3.5, or -- pe_per_decade > 0 -- the table coordinate of E
+template <class R> __device__ EnergyFactors<R> energy_factors(R E, int pe_per_decade) {
     // Klein-Nishina total cross-section per electron in units of 2 pi r_e^2 (C6):
     //   (1+k)/k^2 [2(1+k)/(1+2k) - ln(1+2k)/k] + ln(1+2k)/(2k) - (1+3k)/(1+2k)^2,  k = E / me c^2
     // DESIGN.md reading 1 writes g_KN as sigma_KN / (2 pi r_e^2): the prefactor is multiplied in and divided out again
@@ -73,16 +82,29 @@ template <class R> __device__ EnergyFactors<R> energy_factors(R E) {
     const double two_pi_re2 = 2.0 * GN_PI * 2.8179403262e-13 * 2.8179403262e-13;
     EnergyFactors<R> f;
     f.gKN = (R)((two_pi_re2 * (first + second - third)) / two_pi_re2);
-    f.gPE = (R)pow(0.1 / (double)E, 3.5);
+    f.gPE = pe_per_decade > 0 ? pe_coordinate<R>(E, pe_per_decade) : (R)pow(0.1 / (double)E, 3.5);
     f.L2k = (R)log(2.0 * k);
     f.above_pair = k > 2.0;
     return f;
 }
-template <class R> __device__ __forceinline__ void mu_partials(const MatRec<R>& m, const EnergyFactors<R>& f, R& muPE, R& muC, R& muP) {
-    muPE = m.aPE * f.gPE;
-    muC = m.aC * f.gKN;
-    R P = rmin((R)(28.0 / 9.0) * f.L2k - (R)(218.0 / 27.0), m.capZ);
-    muP = (f.above_pair && P > 0) ? m.aP * P : (R)0;
+// The four partial attenuation coefficients of a photon (energy E, factors gPE / gKN / L2k) in material `mat` (C6; readings
+// 1, 18, 19).  With the options off the Rayleigh term is an exact zero and the sum is (mu_PE + mu_C) + mu_pair as before.
+template <class R> struct MuParts { R pe, c, r, p, tot; };
+template <class R> __device__ __forceinline__ MuParts<R> photon_mu(const GeoView<R>& g, const MatRec<R>& m, int mat, R E, R gPE, R gKN, R L2k, int above) {
+    MuParts<R> o;
+    if (g.pe_per_decade > 0) {                                   // table: T_i + f (T_{i+1} - T_i), i = floor(u), f = u - i
+        const int i = (int)rfloor(gPE);
+        const R f = gPE - (R)i;
+        const R* T = g.pe_tab + (size_t)mat * g.pe_points + i;
+        const R t0 = __ldg(T), t1 = __ldg(T + 1);
+        o.pe = t0 + f * (t1 - t0);
+    } else o.pe = m.aPE * gPE;
+    o.c = m.aC * gKN;
+    const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
+    o.p = (above && P > 0) ? m.aP * P : (R)0;
+    o.r = g.rayleigh ? __ldg(&g.mat_r[mat]) * rdiv((R)1, E * E) : (R)0;
+    o.tot = ((o.pe + o.c) + o.r) + o.p;
+    return o;
 }
 
 // ---- Klein-Nishina composition-rejection (C7) ------------------------------------------------------------
@@ -101,6 +123,16 @@ template <class R> __device__ void kn_sample(R E, PhiloxStream& rng, R& eps, R& 
         R t = ((R)1 - e) / (k * e);
         R s2 = t * ((R)2 - t);
         if ((R)1 - e * s2 / ((R)1 + e2) >= u3) { eps = e; cost = (R)1 - t; sint2 = s2; return; }
+    }
+}
+
+// Rayleigh angle (reading 18): cos(theta) from p(c) ~ 1 + c^2 by rejection, two draws per trial: c = 2 U1 - 1, accepted when
+// 2 U2 <= 1 + c c
+template <class R> __device__ R rayleigh_sample(PhiloxStream& rng) {
+    for (;;) {
+        const R u1 = draw<R>(rng), u2 = draw<R>(rng);
+        const R c = (R)2 * u1 - (R)1;
+        if ((R)2 * u2 <= (R)1 + c * c) return c;
     }
 }
 

@@ -68,12 +68,15 @@ template <class R> struct GeoView {
     const SolidRec<R>* solids;
     const MatRec<R>* mats;
     const double* rho;    // density per material [g/cm3] (attenuation-only mode: mu = rho * mu_mass)
+    const R* mat_r;       // Rayleigh factor per material, n sigma_R0 (Z/13)^2 / 10 (gn_opts.rayleigh; reading 18)
+    const R* pe_tab;      // tabulated photoelectric coefficient, n_mats x pe_points (gn_opts.pe_table_per_decade; reading 19)
     const GridRec<R>* grids;
     const int2* cells;
     const int* cand;
     R tol, delta, probe;  // surface tolerance, tol/2, voxel probe half-width
     R e_cut;
     int n_nodes, n_solids, n_mats, n_grids, stuck_limit;
+    int rayleigh, pe_per_decade, pe_points;       // optional physics; 0 = off
 };
 
 }  // namespace gn

@@ -46,13 +46,13 @@ constexpr int INTERACT_BATCH = 8;     // parked lanes that trigger a warp's inte
 #ifndef GENERAL_BATCH
 #define GENERAL_BATCH 8            // box-only kernels: lanes waiting for the general ComputeStep that trigger it
 #endif
-enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6 };
+enum : int { EV_BOUNDARY = 0, EV_PE = 1, EV_COMPTON = 2, EV_PAIR = 3, EV_CUT = 4, EV_ESCAPE = 5, EV_STUCK = 6, EV_RAYLEIGH = 7 };
 enum : int { FATE_ALIVE = 0, FATE_ABSORBED = 1, FATE_ESCAPED = 2, FATE_STUCK = 3, FATE_NONE = 4 };
-enum : int { ST_STEPS = 0, ST_COMPTON, ST_PE, ST_PAIR, ST_CUT, ST_ESCAPED, ST_STUCK, ST_PHOTONS };
+enum : int { ST_STEPS = 0, ST_COMPTON, ST_PE, ST_PAIR, ST_CUT, ST_ESCAPED, ST_STUCK, ST_PHOTONS, ST_RAYLEIGH, ST_COUNT };
 enum : int { EN_ESCAPED = 0, EN_STUCK, EN_SOURCE, EN_DEPOSITED };
 
 struct DevStats {
-    unsigned long long cnt[8];       // ST_*
+    unsigned long long cnt[16];      // ST_*
     unsigned long long lean_steps;   // steps taken inside the lean wavefront passes (the dominant kernel)
     double en[4];                    // EN_*
     unsigned long long dbg[8];       // GN_DEBUG_COUNTERS builds only: fast steps, bails, general phases, general lane-steps, iterations
@@ -172,12 +172,14 @@ template <class R> struct InteractIO {
     uint32_t j; int above, ev;
 };
 template <class R>
-__device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R mu, R e_cut, uint64_t seed, uint64_t id, uint32_t tag, bool annihilate) {
+__device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muR, R muP, R mu, R e_cut, int pe_pd, uint64_t seed, uint64_t id, uint32_t tag, bool annihilate) {
     PhiloxStream rng; rng.init(seed, id, io->j, tag);
     R E = io->E;
     R t = draw<R>(rng) * mu;
+    // cumulative thresholds PE | Compton | Rayleigh | pair; U = 1 falls to the last process with a non-zero coefficient (reading 2)
+    const bool last_pair = muP > 0, last_rayleigh = !last_pair && muR > 0;
     if (t < muPE) { io->dep = E; io->ev = EV_PE; }
-    else if (t < muPE + muC || !(muP > 0)) {
+    else if (t < muPE + muC || (!last_pair && !last_rayleigh)) {
         R eps, cost, s2;
         kn_sample(E, rng, eps, cost, s2);
         R Ep = eps * E;
@@ -189,11 +191,20 @@ __device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R
         io->E = Ep; io->ev = EV_COMPTON;
         if (Ep < e_cut) { dep = dep + Ep; io->ev = EV_CUT; }
         else {
-            EnergyFactors<R> ef = energy_factors(Ep);
+            EnergyFactors<R> ef = energy_factors(Ep, pe_pd);
             io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
             io->Y = -rlog(draw<R>(rng));
         }
         io->dep = dep;
+    } else if (t < (muPE + muC) + muR || last_rayleigh) {          // Rayleigh (reading 18): new direction, same energy, no deposit
+        const R cost = rayleigh_sample<R>(rng);
+        const R sint = rsqrt_(rmax(((R)1 - cost) * ((R)1 + cost), (R)0));
+        R phi = (R)6.283185307179586 * draw<R>(rng);
+        V3<R> w{io->wx, io->wy, io->wz};
+        rotate_direction(w, cost, sint, phi);
+        io->wx = w.x; io->wy = w.y; io->wz = w.z;
+        io->Y = -rlog(draw<R>(rng));
+        io->dep = 0; io->ev = EV_RAYLEIGH;
     } else { io->dep = annihilate ? E - (R)(2.0 * GN_ME_C2) : E; io->ev = EV_PAIR; }   // pair: all of E, or the pair's kinetic energy
     io->j = rng.j;
 }
@@ -201,14 +212,14 @@ __device__ __noinline__ void interact(InteractIO<R>* io, R muPE, R muC, R muP, R
 // photon birth (C8, Algorithm 1 steps 1-2), out of line: source sampling, energy factors, first optical depth
 template <class R> struct BirthIO { R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k; uint32_t j; int above; };
 template <class R>
-__device__ __forceinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, const EnergyFactors<R>* mono, uint64_t seed, uint64_t id) {
+__device__ __forceinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, const EnergyFactors<R>* mono, int pe_pd, uint64_t seed, uint64_t id) {
     PhiloxStream rng; rng.init(seed, id, 0);
     V3<R> x, w; R E;
     sample_source(*src, rng, x, w, E);
     io->x = x.x; io->y = x.y; io->z = x.z; io->wx = w.x; io->wy = w.y; io->wz = w.z; io->E = E;
     io->Y = -rlog(draw<R>(rng));                       // Algorithm 1 steps 1-2
     // mono-energetic source: the factors of E0 were evaluated once per block (same function, same value)
-    EnergyFactors<R> ef = mono ? *mono : energy_factors(E);
+    EnergyFactors<R> ef = mono ? *mono : energy_factors(E, pe_pd);
     io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
     io->j = rng.j;
 }
@@ -216,7 +227,7 @@ __device__ __forceinline__ void birth(BirthIO<R>* io, const SourceDev<R>* src, c
 // birth of annihilation photon k (NEXT-3): isotropic direction from draws 0, 1 of stream tag 1 of the parent (cos theta =
 // 1 - 2 u0, phi = 2 pi u1); photon 2 flies exactly the other way on stream tag 2; both have E = me c^2
 template <class R>
-__device__ __noinline__ void birth_secondary(BirthIO<R>* io, const PairVtx<R>* vtx, uint32_t k, uint64_t seed, uint64_t first_id) {
+__device__ __noinline__ void birth_secondary(BirthIO<R>* io, const PairVtx<R>* vtx, uint32_t k, int pe_pd, uint64_t seed, uint64_t first_id) {
     const PairVtx<R> pv = vtx[k >> 1];
     PhiloxStream rng; rng.init(seed, first_id + pv.idx, 0, 1);
     R u0 = draw<R>(rng), u1 = draw<R>(rng);
@@ -227,7 +238,7 @@ __device__ __noinline__ void birth_secondary(BirthIO<R>* io, const PairVtx<R>* v
     if (k & 1u) { wx = -wx; wy = -wy; wz = -wz; rng.init(seed, first_id + pv.idx, 0, 2); }
     io->x = pv.x; io->y = pv.y; io->z = pv.z; io->wx = wx; io->wy = wy; io->wz = wz; io->E = (R)GN_ME_C2;
     io->Y = -rlog(draw<R>(rng));
-    EnergyFactors<R> ef = energy_factors(io->E);
+    EnergyFactors<R> ef = energy_factors(io->E, pe_pd);
     io->gPE = ef.gPE; io->gKN = ef.gKN; io->L2k = ef.L2k; io->above = ef.above_pair;
     io->j = rng.j;
 }
@@ -252,15 +263,15 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     __shared__ EnergyFactors<R> sh_mono;
     __shared__ unsigned sh_wcount[2][TR_WARPS];
     __shared__ unsigned sh_base[2];
-    __shared__ unsigned long long sh_cnt[8];
+    __shared__ unsigned long long sh_cnt[ST_COUNT];
     __shared__ double sh_en[4];
     __shared__ unsigned sh_key[SORT_KEYS];
     if (threadIdx.x < SORT_KEYS) sh_key[threadIdx.x] = 0;
     stage_tables(g, tab);
     const MatRec<R>* mats = g.mats;
     if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
-    if (FROM_SOURCE && threadIdx.x == 0) { sh_src = src; if (src.energy_kind == 0) sh_mono = energy_factors(src.e0); }
-    if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
+    if (FROM_SOURCE && threadIdx.x == 0) { sh_src = src; if (src.energy_kind == 0) sh_mono = energy_factors(src.e0, g.pe_per_decade); }
+    if (threadIdx.x < ST_COUNT) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
     Navigator<R, true, FLAT> nav(g, &tab.ctx);
@@ -280,8 +291,8 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         if (fate == FATE_ALIVE) {
             idx = i;
             BirthIO<R> b;
-            if (sec.in) birth_secondary(&b, sec.in, i, seed, first_id);
-            else birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, seed, first_id + i);
+            if (sec.in) birth_secondary(&b, sec.in, i, g.pe_per_decade, seed, first_id);
+            else birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, g.pe_per_decade, seed, first_id + i);
             x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
             gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
             if (!sec.in) { c_phot = 1; e_src = (double)E; }               // annihilation photons are not source photons
@@ -353,18 +364,18 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             // ---- interaction phase (A6-A9) ----------------------------------------------------------------------
             double dep_d = 0.0;
             if (pending) {
-                const MatRec<R> m = mats[nd.mat];
-                const R muPE = m.aPE * gPE, muC = m.aC * gKN;
-                const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
-                const R muP = (above && P > 0) ? m.aP * P : (R)0;
-                const R mu = (muPE + muC) + muP;
+                const MuParts<R> mp = photon_mu(g, mats[nd.mat], nd.mat, E, gPE, gKN, L2k, above);
                 InteractIO<R> io;
                 io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
-                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + (sec.in ? sec.in[idx >> 1].idx : idx), sec.in ? 1u + (idx & 1u) : 0u, sec.out != nullptr);
+                interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, first_id + (sec.in ? sec.in[idx >> 1].idx : idx), sec.in ? 1u + (idx & 1u) : 0u, sec.out != nullptr);
                 const int ev = io.ev; ctr = io.j;
                 if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = x.x; pv.y = x.y; pv.z = x.z; pv.idx = idx; sec.out[atomicAdd(sec.n_out, 1u)] = pv; }
                 dep_d = (double)io.dep;
-                if (ev == EV_COMPTON || ev == EV_CUT) {
+                if (ev == EV_RAYLEIGH) {
+                    w.x = io.wx; w.y = io.wy; w.z = io.wz; Y = io.Y;
+                    atomicAdd(&sh_cnt[ST_RAYLEIGH], 1ull);
+                    if (FASTV) lane_direction(w, g.delta, vl);
+                } else if (ev == EV_COMPTON || ev == EV_CUT) {
                     E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
                     atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
                     if (ev == EV_CUT) { atomicAdd(&sh_cnt[ST_CUT], 1ull); fate = FATE_ABSORBED; }
@@ -392,13 +403,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         ++k;
         bool todo = fate == FATE_ALIVE && !pending;                            // this lane wants a step
         R mu = 0;
-        if (todo) {
-            const MatRec<R> m = mats[nd.mat];
-            const R muPE = m.aPE * gPE, muC = m.aC * gKN;
-            const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
-            const R muP = (above && P > 0) ? m.aP * P : (R)0;
-            mu = (muPE + muC) + muP;
-        }
+        if (todo) mu = photon_mu(g, mats[nd.mat], nd.mat, E, gPE, gKN, L2k, above).tot;
         if (FASTV) {
             bool stepped = false;
             if (todo && !bailed && vl.ok && (nd.info & NODE_REGULAR)) {
@@ -476,8 +481,8 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     }
     __syncthreads();
     GN_CHECK(cout->front + cout->back <= cap, CHK_SEGMENTS);
-    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
-    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+    if (threadIdx.x < ST_COUNT && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 16 && threadIdx.x < 20 && sh_en[threadIdx.x - 16] != 0.0) atomicAdd(&stats->en[threadIdx.x - 16], sh_en[threadIdx.x - 16]);
     if (!FROM_SOURCE && !PHYS && timed && threadIdx.x == 12 && sh_cnt[ST_STEPS]) atomicAdd(&stats->lean_steps, sh_cnt[ST_STEPS]);
     if (FLAT && sio.kout && threadIdx.x >= 32 && threadIdx.x < 32 + SORT_KEYS && sh_key[threadIdx.x - 32]) atomicAdd(&sio.kout->tot[threadIdx.x - 32], (unsigned long long)sh_key[threadIdx.x - 32]);
 }
@@ -491,9 +496,9 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = cin->back;
     if (blockIdx.x * TR_THREADS >= n) return;
-    __shared__ unsigned long long sh_cnt[8];
+    __shared__ unsigned long long sh_cnt[ST_COUNT];
     __shared__ double sh_en[4];
-    if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
+    if (threadIdx.x < ST_COUNT) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
     const unsigned i = blockIdx.x * TR_THREADS + threadIdx.x;
@@ -505,19 +510,19 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         vol = r.vol;
         GN_CHECK(vol >= 0 && vol < g.n_nodes && g.node[vol].mat < g.n_mats, CHK_VOLUME);
         const int above = (int)(r.tail[0] & 1u);
-        const MatRec<R> m = g.mats[__ldg(&g.node[vol].mat)];
-        const R muPE = m.aPE * r.gPE, muC = m.aC * r.gKN;
-        const R P = rmin((R)(28.0 / 9.0) * r.L2k - (R)(218.0 / 27.0), m.capZ);
-        const R muP = (above && P > 0) ? m.aP * P : (R)0;
-        const R mu = (muPE + muC) + muP;
+        const int mat = __ldg(&g.node[vol].mat);
+        const MuParts<R> mp = photon_mu(g, g.mats[mat], mat, r.E, r.gPE, r.gKN, r.L2k, above);
         InteractIO<R> io;
         io.E = r.E; io.wx = r.wx; io.wy = r.wy; io.wz = r.wz; io.Y = r.Y; io.gPE = r.gPE; io.gKN = r.gKN; io.L2k = r.L2k; io.j = r.ctr; io.above = above;
-        interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + (sec.in ? sec.in[r.idx >> 1].idx : r.idx), sec.in ? 1u + (r.idx & 1u) : 0u, sec.out != nullptr);
+        interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, first_id + (sec.in ? sec.in[r.idx >> 1].idx : r.idx), sec.in ? 1u + (r.idx & 1u) : 0u, sec.out != nullptr);
         int ev = io.ev;
         if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = r.x; pv.y = r.y; pv.z = r.z; pv.idx = r.idx; const unsigned ps = atomicAdd(sec.n_out, 1u); GN_CHECK(ps < cap, CHK_PAIR_SLOT); sec.out[ps] = pv; }
         dep_d = (double)io.dep;
         bool alive = false;
-        if (ev == EV_COMPTON || ev == EV_CUT) {
+        if (ev == EV_RAYLEIGH) {
+            r.wx = io.wx; r.wy = io.wy; r.wz = io.wz; r.Y = io.Y; alive = true;
+            atomicAdd(&sh_cnt[ST_RAYLEIGH], 1ull);
+        } else if (ev == EV_COMPTON || ev == EV_CUT) {
             r.E = io.E; r.wx = io.wx; r.wy = io.wy; r.wz = io.wz;
             atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
             if (ev == EV_CUT) atomicAdd(&sh_cnt[ST_CUT], 1ull);
@@ -539,8 +544,8 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
     }
     warp_tally(edep, &sh_en[EN_DEPOSITED], vol, dep_d, active);
     __syncthreads();
-    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
-    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+    if (threadIdx.x < ST_COUNT && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 16 && threadIdx.x < 20 && sh_en[threadIdx.x - 16] != 0.0) atomicAdd(&stats->en[threadIdx.x - 16], sh_en[threadIdx.x - 16]);
 }
 
 // The paper's own remedy for threads whose particle has finished (stream compaction "and filling the empty places
@@ -556,13 +561,13 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     __shared__ MatRec<R> sh_mats[MAX_SMEM_MATS];
     __shared__ SourceDev<R> sh_src;
     __shared__ EnergyFactors<R> sh_mono;
-    __shared__ unsigned long long sh_cnt[8];
+    __shared__ unsigned long long sh_cnt[ST_COUNT];
     __shared__ double sh_en[4];
     stage_tables(g, tab);
     const MatRec<R>* mats = g.mats;
     if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
-    if (threadIdx.x == 0) { sh_src = src; if (src.energy_kind == 0) sh_mono = energy_factors(src.e0); }
-    if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
+    if (threadIdx.x == 0) { sh_src = src; if (src.energy_kind == 0) sh_mono = energy_factors(src.e0, g.pe_per_decade); }
+    if (threadIdx.x < ST_COUNT) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
     Navigator<R, true, FLAT> nav(g, &tab.ctx);
@@ -574,7 +579,7 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     uint32_t idx = 0, misc = 0, ctr = 0; int above = 0;
     uint64_t h = 0;
     int vol = -1; NodeRec<R> nd = {};
-    unsigned c_steps = 0, c_phot = 0, c_esc = 0, c_stuck = 0, c_compton = 0, c_pe = 0, c_pair = 0, c_cut = 0;
+    unsigned c_steps = 0, c_phot = 0, c_esc = 0, c_stuck = 0, c_compton = 0, c_pe = 0, c_pair = 0, c_cut = 0, c_ray = 0;
     double e_src = 0.0, e_esc = 0.0, e_stuck = 0.0;
 #pragma unroll 1
     for (;;) {
@@ -592,7 +597,7 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
                 else {
                     idx = i; misc = 0; h = 0xcbf29ce484222325ull;
                     BirthIO<R> b;
-                    birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, seed, first_id + i);
+                    birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, g.pe_per_decade, seed, first_id + i);
                     x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
                     gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
                     ++c_phot; e_src += (double)E;
@@ -610,17 +615,14 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
             double dep_d = 0.0;
             const bool was = alive && pending;
             if (was) {
-                const MatRec<R> m = mats[nd.mat];
-                const R muPE = m.aPE * gPE, muC = m.aC * gKN;
-                const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
-                const R muP = (above && P > 0) ? m.aP * P : (R)0;
-                const R mu = (muPE + muC) + muP;
+                const MuParts<R> mp = photon_mu(g, mats[nd.mat], nd.mat, E, gPE, gKN, L2k, above);
                 InteractIO<R> io;
                 io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
-                interact(&io, muPE, muC, muP, mu, g.e_cut, seed, first_id + idx, 0u, false);
+                interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, first_id + idx, 0u, false);
                 int ev = io.ev; ctr = io.j;
                 dep_d = (double)io.dep;
-                if (ev == EV_COMPTON || ev == EV_CUT) {
+                if (ev == EV_RAYLEIGH) { w.x = io.wx; w.y = io.wy; w.z = io.wz; Y = io.Y; ++c_ray; }
+                else if (ev == EV_COMPTON || ev == EV_CUT) {
                     E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
                     ++c_compton;
                     if (ev == EV_CUT) { ++c_cut; alive = false; }
@@ -641,11 +643,7 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
         }
         // ---- one navigation step (A1-A5) for every travelling lane ----------------------------------------------------
         if (alive && !pending) {
-            const MatRec<R> m = mats[nd.mat];
-            const R muPE = m.aPE * gPE, muC = m.aC * gKN;
-            const R P = rmin((R)(28.0 / 9.0) * L2k - (R)(218.0 / 27.0), m.capZ);
-            const R muP = (above && P > 0) ? m.aP * P : (R)0;
-            const R mu = (muPE + muC) + muP;
+            const R mu = photon_mu(g, mats[nd.mat], nd.mat, E, gPE, gKN, L2k, above).tot;
             const R s_int = mu > 0 ? rdiv(Y, mu) : rinf<R>();
             const int vol_before = vol;
             R step; V3<R> xn;
@@ -674,15 +672,15 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     }
     // ---- statistics -----------------------------------------------------------------------------------------------
     {
-        const unsigned v[8] = {c_steps, c_compton, c_pe, c_pair, c_cut, c_esc, c_stuck, c_phot};      // ST_* order
+        const unsigned v[ST_COUNT] = {c_steps, c_compton, c_pe, c_pair, c_cut, c_esc, c_stuck, c_phot, c_ray};      // ST_* order
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { unsigned t = warp_sum(v[q]); if (lane == 0 && t) atomicAdd(&sh_cnt[q], (unsigned long long)t); }
+        for (int q = 0; q < ST_COUNT; ++q) { unsigned t = warp_sum(v[q]); if (lane == 0 && t) atomicAdd(&sh_cnt[q], (unsigned long long)t); }
         double a = warp_sum(e_esc), b2 = warp_sum(e_stuck), c2 = warp_sum(e_src);
         if (lane == 0) { if (a != 0.0) atomicAdd(&sh_en[EN_ESCAPED], a); if (b2 != 0.0) atomicAdd(&sh_en[EN_STUCK], b2); if (c2 != 0.0) atomicAdd(&sh_en[EN_SOURCE], c2); }
     }
     __syncthreads();
-    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
-    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+    if (threadIdx.x < ST_COUNT && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 16 && threadIdx.x < 20 && sh_en[threadIdx.x - 16] != 0.0) atomicAdd(&stats->en[threadIdx.x - 16], sh_en[threadIdx.x - 16]);
 }
 
 }  // namespace gn
@@ -903,7 +901,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             h_stats->n_cut = hs.cnt[ST_CUT]; h_stats->n_escaped = hs.cnt[ST_ESCAPED]; h_stats->n_stuck = hs.cnt[ST_STUCK]; h_stats->n_photons = hs.cnt[ST_PHOTONS];
             h_stats->e_escaped = hs.en[EN_ESCAPED]; h_stats->e_stuck = hs.en[EN_STUCK]; h_stats->e_source = hs.en[EN_SOURCE]; h_stats->e_deposited = hs.en[EN_DEPOSITED];
             h_stats->n_passes = passes; h_stats->n_kernel_launches = launches; h_stats->kernel_ms = kernel_ms;
-            h_stats->step_pass_ms = step_pass_ms; h_stats->n_steps_step_pass = hs.lean_steps;
+            h_stats->step_pass_ms = step_pass_ms; h_stats->n_steps_step_pass = hs.lean_steps; h_stats->n_rayleigh = hs.cnt[ST_RAYLEIGH];
 #ifdef GN_DEBUG_COUNTERS
             fprintf(stderr, "[gn debug] fast steps %llu, bails %llu, general phases (warps) %llu, general lane-steps %llu, warp iterations %llu\n", hs.dbg[0], hs.dbg[1], hs.dbg[2], hs.dbg[3], hs.dbg[4]);
 #endif

@@ -170,12 +170,12 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
     if (blockIdx.x * TR_THREADS >= n) return;
     __shared__ BlockTables<R> tab;
     __shared__ MatRec<R> sh_mats[MAX_SMEM_MATS];
-    __shared__ unsigned long long sh_cnt[8];
+    __shared__ unsigned long long sh_cnt[ST_COUNT];
     __shared__ double sh_en[4];
     stage_tables(g, tab);
     const MatRec<R>* mats = g.mats;
     if (g.n_mats <= MAX_SMEM_MATS) { for (int i = threadIdx.x; i < g.n_mats; i += blockDim.x) sh_mats[i] = g.mats[i]; mats = sh_mats; }
-    if (threadIdx.x < 8) sh_cnt[threadIdx.x] = 0;
+    if (threadIdx.x < ST_COUNT) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
     Navigator<R, true, false> nav(g, &tab.ctx);
@@ -199,11 +199,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
         NodeRec<R> nd = nav.node(vol);
         const bool cacheable = direction_cacheable(w, g.delta);
         for (int it = 0; it < SLOW_STEPS; ++it) {
-            const MatRec<R> m = mats[nd.mat];
-            const R muPE = m.aPE * r.gPE, muC = m.aC * r.gKN;
-            const R P = rmin((R)(28.0 / 9.0) * r.L2k - (R)(218.0 / 27.0), m.capZ);
-            const R muP = (above && P > 0) ? m.aP * P : (R)0;
-            const R mu = (muPE + muC) + muP;
+            const R mu = photon_mu(g, mats[nd.mat], nd.mat, r.E, r.gPE, r.gKN, r.L2k, above).tot;
             const R s_int = mu > 0 ? rdiv(Y, mu) : rinf<R>();              // remaining part of Eq. 7
             const int vol_before = vol;
             R step; V3<R> xn;
@@ -245,8 +241,8 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
     }
     __syncthreads();
     GN_CHECK(ctr->front + ctr->back <= cap, CHK_SEGMENTS);
-    if (threadIdx.x < 8 && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
-    if (threadIdx.x >= 8 && threadIdx.x < 12 && sh_en[threadIdx.x - 8] != 0.0) atomicAdd(&stats->en[threadIdx.x - 8], sh_en[threadIdx.x - 8]);
+    if (threadIdx.x < ST_COUNT && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x >= 16 && threadIdx.x < 20 && sh_en[threadIdx.x - 16] != 0.0) atomicAdd(&stats->en[threadIdx.x - 16], sh_en[threadIdx.x - 16]);
 }
 
 }  // namespace gn

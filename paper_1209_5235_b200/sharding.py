@@ -15,7 +15,7 @@ def shard_range(n_total: int, rank: int, world: int):
     return first, base + (1 if rank < rem else 0)
 
 
-STAT_KEYS = ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons",
+STAT_KEYS = ("n_steps", "n_compton", "n_pe", "n_pair", "n_cut", "n_escaped", "n_stuck", "n_photons", "n_rayleigh",
              "e_escaped", "e_stuck", "e_source", "e_deposited")
 
 
@@ -26,7 +26,7 @@ def allreduce_tally(edep, stats: dict, group=None):
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
         return edep, dict(stats)
     dist.all_reduce(edep, op=dist.ReduceOp.SUM, group=group)
-    vec = torch.tensor([float(stats[k]) for k in STAT_KEYS], dtype=torch.float64, device=edep.device)
+    vec = torch.tensor([float(stats.get(k, 0)) for k in STAT_KEYS], dtype=torch.float64, device=edep.device)
     dist.all_reduce(vec, op=dist.ReduceOp.SUM, group=group)
     out = dict(stats)
     for k, v in zip(STAT_KEYS, vec.tolist()):

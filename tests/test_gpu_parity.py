@@ -354,6 +354,60 @@ def test_stuck_limit_above_the_counter_width_is_refused(B):
     assert g.n_places == 6
 
 
+# ---- SURVEY 8(f) NEXT-3, the rest: Rayleigh scattering and the tabulated photoelectric coefficient -----------------------------
+OPTIONAL_PHYSICS = {
+    "rayleigh": dict(rayleigh=1),
+    "rayleigh_strong": dict(rayleigh=1, sigma_r0=0.5),                    # coherent scattering as frequent as Compton in the light materials
+    "pe_table": dict(pe_table_per_decade=256),
+    "pe_table_k_edge": dict(pe_table_per_decade=64, pe_k_edge=1),
+    "all": dict(rayleigh=1, pe_table_per_decade=128, pe_k_edge=1, secondaries=1),
+}
+PHYSICS_GEOMS = {
+    "config1_300keV": lambda: (W.slab_geometry(1), W.Source(W.SRC_PENCIL, (0.0, 0.0, -500.0), (0.0, 0.0, 1.0), W.E_MONO, 0.3), 20000, 1),
+    "phantom16": lambda: TRANSPORT_CASES["phantom16"](),
+    "detector": lambda: TRANSPORT_CASES["detector"](),
+}
+
+
+@pytest.mark.parametrize("schedule", ["tail", "wavefront"])
+@pytest.mark.parametrize("geo_name", list(PHYSICS_GEOMS))
+@pytest.mark.parametrize("physics", list(OPTIONAL_PHYSICS))
+def test_optional_physics_fp64_histories_identical(B, physics, geo_name, schedule):
+    """gn_opts.rayleigh / pe_table_per_decade / pe_k_edge (readings 18, 19): same Philox draws, same process choice, same
+    rejection loops as the oracle -> identical fp64 histories, event word 7 for a Rayleigh scatter, n_rayleigh equal."""
+    geom, src, n, seed = PHYSICS_GEOMS[geo_name]()
+    opts = OPTIONAL_PHYSICS[physics]
+    got, ref, frac = compare_transport(B, geom, src, n, seed, 64, 0.999, opts=dict(opts, **SCHEDULES[schedule]), oracle_opts=opts)
+    s, r = got["stats"], ref["stats"]
+    assert s["n_rayleigh"] == r["n_rayleigh"]
+    if not opts.get("rayleigh"):
+        assert s["n_rayleigh"] == 0
+    elif physics == "rayleigh_strong" or geo_name == "config1_300keV":       # (at 6 MeV the default cross-section is negligible)
+        assert s["n_rayleigh"] > 20
+    ends = s["n_pe"] + s["n_pair"] + s["n_cut"] + s["n_escaped"] + s["n_stuck"]
+    assert ends == n + (2 * s["n_pair"] if opts.get("secondaries") else 0)
+
+
+@pytest.mark.parametrize("physics", ["rayleigh_strong", "all"])
+def test_optional_physics_fp32_and_refill(B, physics):
+    geom, src, n, seed = PHYSICS_GEOMS["detector"]()
+    opts = dict(OPTIONAL_PHYSICS[physics]); opts.pop("secondaries", None)
+    got, ref, frac = compare_transport(B, geom, src, n, seed, 32, 0.97, opts=opts, oracle_opts=opts)
+    assert abs(got["stats"]["n_rayleigh"] - ref["stats"]["n_rayleigh"]) <= 0.02 * ref["stats"]["n_rayleigh"] + 5
+    got2, _, _ = compare_transport(B, geom, src, n, seed, 64, 0.999, opts=dict(opts, refill=1), oracle_opts=opts)
+    assert got2["stats"]["n_rayleigh"] > 20
+
+
+def test_optional_physics_leaves_the_default_untouched(B):
+    """Options off: the new terms are exact zeros -- same hashes as a library that never heard of them (the oracle's default run)."""
+    geom, src, n, seed = TRANSPORT_CASES["phantom16"]()
+    a = B.transport_run(B.Geometry(geom), src, seed, n, 64, per_photon=True)
+    b = B.transport_run(B.Geometry(geom, rayleigh=0, pe_table_per_decade=0, no_voxel_pass=1), src, seed, n, 64, per_photon=True)
+    assert np.array_equal(a["hash"].cpu().numpy(), b["hash"].cpu().numpy()) and a["stats"]["n_rayleigh"] == 0
+    with pytest.raises(B.GammaNavError):
+        B.Geometry(geom, pe_table_per_decade=5000)
+
+
 def _four_walls():
     from paper_1209_5235_b200.workloads import _Builder
     b = _Builder("four_walls")

@@ -33,9 +33,9 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_struct_layouts_match_header():
     from paper_1209_5235_b200 import binding as B
-    assert C.sizeof(B.Opts) == 4 * 8 + 10 * 4
+    assert C.sizeof(B.Opts) == 4 * 8 + 10 * 4 + 8 + 2 * 4
     assert C.sizeof(B.CSource) == 8 + 6 * 8 + 4 * 8
-    assert C.sizeof(B.RunStats) == 8 * 8 + 4 * 8 + 2 * 8 + 8 + 2 * 8
+    assert C.sizeof(B.RunStats) == 8 * 8 + 4 * 8 + 2 * 8 + 8 + 2 * 8 + 8
 
 
 def test_no_cpu_fallback(lib):
