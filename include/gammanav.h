@@ -54,7 +54,8 @@ typedef struct {
     int32_t stuck_limit;       /* consecutive steps of length <= tol/2 before a photon is killed; default 8, at most 255
                                   (gn_geometry_create returns GN_INVALID_ARGUMENT above that: the per-photon counter has 8 bits;
                                   the per-photon step count has 24 bits and wraps at 2^24 steps of one photon) */
-    int32_t steps_per_pass;    /* K: steps a photon takes per wavefront pass before it is re-queued; default 16 */
+    int32_t steps_per_pass;    /* K: steps a photon takes per wavefront pass before it is re-queued; default 16 (24 with the
+                                  regular-voxel schedule) */
     int32_t first_pass_steps;  /* K0: steps in the pass that also generates the photons (sheds photons that miss early); default 1 */
     int32_t tail_photons;      /* once at most this many photons are left, one last pass runs them to completion; default 148 * 512 */
     int32_t regroup_percent;   /* a warp ends its pass early once fewer than this % of the lanes it started with still travel

@@ -18,6 +18,12 @@ constexpr int NAV_THREADS = 256;
 #ifndef NAV_STEP_MIN_BLOCKS
 #define NAV_STEP_MIN_BLOCKS 8      // ComputeStep kernels are latency-bound at ~10 of 32 lanes: full occupancy (32 registers, spills) wins
 #endif
+#ifndef NAV_LOCATE_MIN_BLOCKS_F64
+#define NAV_LOCATE_MIN_BLOCKS_F64 4
+#endif
+#ifndef NAV_STEP_MIN_BLOCKS_F64
+#define NAV_STEP_MIN_BLOCKS_F64 4      // 64 registers: +14 % on config 5 fp64 over 3 blocks
+#endif
 constexpr int MAX_SMEM_SOLIDS = 32;
 constexpr int MAX_SMEM_GRIDS = 8;
 constexpr int MAX_SMEM_MATS = 32;

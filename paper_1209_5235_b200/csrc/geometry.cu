@@ -230,7 +230,8 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     if (o.pe_table_per_decade < 0) o.pe_table_per_decade = 0;
     if (o.pe_table_per_decade > 4096) { gn_geometry_destroy(geo); return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: pe_table_per_decade must be <= 4096"); }
     if (o.stuck_limit > 255) { gn_geometry_destroy(geo); return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: stuck_limit must be <= 255 (the per-photon counter of consecutive short steps has 8 bits)"); }
-    if (o.steps_per_pass <= 0) o.steps_per_pass = 16;
+    const bool steps_default = o.steps_per_pass <= 0;
+    if (steps_default) o.steps_per_pass = 16;
     if (o.first_pass_steps <= 0) o.first_pass_steps = 1;
     if (o.tail_photons <= 0) o.tail_photons = 148 * 512;
     const bool regroup_default = o.regroup_percent <= 0;
@@ -440,6 +441,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         for (size_t i = 0; i < V; ++i) n_regular += (n32[i].info & NODE_REGULAR) ? 1 : 0;
         geo->voxel_sched = coherent && 2 * n_regular >= V && geo->opts.no_voxel_pass <= 0 && geo->opts.rayleigh <= 0 && geo->opts.pe_table_per_decade <= 0 && n_solids <= 32 && n_mats <= 32 && grids.size() <= 8 && ext < 0x1p50;      // table sizes: MAX_SMEM_* of common.cuh
         if (regroup_default) geo->opts.regroup_percent = coherent ? 50 : 75;
+        if (steps_default && geo->voxel_sched) geo->opts.steps_per_pass = 24;      // the regular-voxel pass is cheap per step: fewer, longer passes (measured)
     }
     Uploader up{geo};
     const int* d_dlist = up.put(dlist);

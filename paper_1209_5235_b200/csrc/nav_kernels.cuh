@@ -10,7 +10,7 @@ namespace gn {
 // navigation kernels: pure maps over queries
 // -------------------------------------------------------------------------------------------------------
 template <class R, bool HAS_DIR, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : 3) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : NAV_LOCATE_MIN_BLOCKS_F64) locate_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                              int64_t n, int32_t* __restrict__ vol_out) {
     __shared__ BlockTables<R> tab;
     stage_tables(g, tab);
@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_B
 }
 
 template <class R, bool FLAT>
-__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLOCKS : 3) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLOCKS : NAV_STEP_MIN_BLOCKS_F64) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                            const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
                                                            int64_t n, R* __restrict__ step_out, int32_t* __restrict__ next_out,
                                                            const uint32_t* __restrict__ perm) {
