@@ -161,6 +161,23 @@ int gn_nav_compute_step(const gn_geometry* geo, int precision, const void* d_pos
                         void* d_step_out, int32_t* d_next_vol_out, void* cuda_stream);
 
 /*
+ * gn_nav_compute_step_noalloc -- gn_nav_compute_step for callers that must not allocate:
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same arguments, same results bit
+ * for bit.  gn_nav_compute_step takes the scratch of its query sort (general geometries: queries grouped by the kind of
+ * their current volume before ComputeStep) from the handle's stream-ordered memory pool; this entry point takes it from one
+ * fixed array in device memory that belongs to the library, and calls no cudaMalloc, cudaFree or pool routine.
+ *   Limit: n <= GN_NOALLOC_MAX_QUERIES (2^20); larger n returns GN_INVALID_ARGUMENT with outputs untouched -- split the
+ *   batch.  Cost: every GPU that loads the library holds GN_NOALLOC_SCRATCH_BYTES (5.3 MB) until the process exits.
+ *   All calls share the array, on every handle: two calls that overlap on the GPU (different streams) race on it --
+ *   serialise them (same stream, or an event between them).  Asynchronous on cuda_stream like gn_nav_compute_step.
+ */
+#define GN_NOALLOC_MAX_QUERIES (1 << 20)
+#define GN_NOALLOC_SCRATCH_BYTES (256 + 5 * (1 << 20))
+int gn_nav_compute_step_noalloc(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir,
+                                const int32_t* d_vol_in, const void* d_max_step, int64_t n,
+                                void* d_step_out, int32_t* d_next_vol_out, void* cuda_stream);
+
+/*
  * gn_nav_compute_step_normal -- PAPER.md L125 in full: "... If so, where, and what is the normal of the boundary surface at
  * that point?"  As gn_nav_compute_step, plus d_normal_out n x 3 Real: the outward unit normal, in the global frame, of the
  * solid whose surface ends the step -- the current volume's own solid (the step leaves it), or the daughter entered (ties:

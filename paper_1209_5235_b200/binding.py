@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "libgammanav.so")
 _lib = None
 
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",
-           "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_nav_compute_step_normal", "gn_nav_compute_safety", "gn_transport_run", "gn_nav_query_host",
+           "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_nav_compute_step_noalloc", "gn_nav_compute_step_normal", "gn_nav_compute_safety", "gn_transport_run", "gn_nav_query_host",
            "gn_transport_run_host", "gn_free_path_run", "gn_free_path_run_host", "gn_selftest_arith", "gn_selftest_pipe_peak",
            "gn_host_source_frame", "gn_host_compose_transforms", "gn_last_error", "gn_version")
 
@@ -68,6 +68,7 @@ def lib():
         L.gn_geometry_voxel_info.argtypes = [C.c_void_p, C.c_void_p]
         L.gn_nav_locate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.gn_nav_compute_step.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.gn_nav_compute_step_noalloc.argtypes = L.gn_nav_compute_step.argtypes
         L.gn_nav_compute_safety.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.gn_nav_compute_step_normal.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_transport_run.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
@@ -189,6 +190,29 @@ def nav_compute_step(geo: Geometry, pos, dirs, vol, max_step=None, precision=Non
                                      C.c_void_p(max_step.data_ptr()) if max_step is not None else None, C.c_int64(n),
                                      C.c_void_p(out[0].data_ptr()), C.c_void_p(out[1].data_ptr()), _stream_ptr(torch)), "gn_nav_compute_step")
     return out
+
+
+def nav_compute_step_noalloc(geo: Geometry, pos, dirs, vol, out, max_step=None, precision=None):
+    """gn_nav_compute_step_noalloc: gn_nav_compute_step without any allocation inside the library (scratch in a fixed device
+    array; n <= NOALLOC_MAX_QUERIES).  The caller passes every buffer, outputs included: out = (step (n,) Real, next_vol (n,)
+    int32), contiguous CUDA tensors; nothing is converted or copied here."""
+    torch = _torch()
+    precision = precision or (32 if pos.dtype == torch.float32 else 64)
+    dt = _real_dtype(torch, precision)
+    tensors = [pos, dirs, vol, out[0], out[1]] + ([max_step] if max_step is not None else [])
+    if pos.dtype != dt or dirs.dtype != dt or vol.dtype != torch.int32 or out[0].dtype != dt or out[1].dtype != torch.int32 or \
+            (max_step is not None and max_step.dtype != dt) or not all(t.is_cuda and t.is_contiguous() for t in tensors):
+        raise GammaNavError("nav_compute_step_noalloc: tensors must be contiguous CUDA tensors, Real / int32")
+    n = pos.shape[0]
+    if out[0].numel() < n or out[1].numel() < n or vol.numel() < n or dirs.shape[0] < n:
+        raise GammaNavError("nav_compute_step_noalloc: buffers shorter than n")
+    _check(lib().gn_nav_compute_step_noalloc(geo._h, precision, C.c_void_p(pos.data_ptr()), C.c_void_p(dirs.data_ptr()), C.c_void_p(vol.data_ptr()),
+                                             C.c_void_p(max_step.data_ptr()) if max_step is not None else None, C.c_int64(n),
+                                             C.c_void_p(out[0].data_ptr()), C.c_void_p(out[1].data_ptr()), _stream_ptr(torch)), "gn_nav_compute_step_noalloc")
+    return out
+
+
+NOALLOC_MAX_QUERIES = 1 << 20      # GN_NOALLOC_MAX_QUERIES of include/gammanav.h
 
 
 def nav_compute_step_normal(geo: Geometry, pos, dirs, vol, max_step=None, precision=None):
