@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libgammanav.so")
+_LIB_PATH = os.environ.get("GN_LIBRARY") or os.path.join(_HERE, "libgammanav.so")      # GN_LIBRARY: load another build of the same library (diagnostics)
 _lib = None
 
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",

@@ -86,6 +86,45 @@ void daughter_bounds(const HostSolid& s, const double* R, const double* T, doubl
     }
 }
 
+// Can the placed daughter (R, T: local -> mother) come anywhere near the cell [clo, chi] of its mother's voxel grid?  Returns
+// true only when that is PROVABLY not so: some bounding set of the solid (slab, cylinder, hole, half-plane,
+// ball, cone -- the solid is their intersection and the outsideness D is the largest signed distance s_k to one of them) stays
+// farther than `margin` from every point of the cell, so D > margin on the whole cell.  Planar sets are tested at the eight
+// corners (s_k is linear: its minimum over a box is at a corner), curved ones through the centre and the half diagonal rho
+// (every s_k is 1-Lipschitz: s_k >= s_k(centre) - rho), the hole through the corners (the distance from the axis is convex:
+// its maximum over a box is at a corner).  An axis-aligned bounding box is a poor fit for a tube sector or a rotated box;
+// this test keeps such a daughter out of the cells its box covers but the solid does not.
+static bool cell_excluded(const HostSolid& s, const double* R, const double* T, const double clo[3], const double chi[3], double margin) {
+    double q[8][3], ctr[3] = {0, 0, 0};
+    for (int c = 0; c < 8; ++c) {
+        const double y[3] = {((c & 1) ? chi[0] : clo[0]) - T[0], ((c & 2) ? chi[1] : clo[1]) - T[1], ((c & 4) ? chi[2] : clo[2]) - T[2]};
+        for (int k = 0; k < 3; ++k) { q[c][k] = R[k] * y[0] + R[3 + k] * y[1] + R[6 + k] * y[2]; ctr[k] += q[c][k] / 8; }      // q = R^T y
+    }
+    const double rho = 0.5 * std::sqrt((chi[0] - clo[0]) * (chi[0] - clo[0]) + (chi[1] - clo[1]) * (chi[1] - clo[1]) + (chi[2] - clo[2]) * (chi[2] - clo[2]));
+    auto beyond_plane = [&](double nx, double ny, double nz, double h) {           // n . q - h > margin at every corner
+        for (int c = 0; c < 8; ++c) if (!(nx * q[c][0] + ny * q[c][1] + nz * q[c][2] - h > margin)) return false;
+        return true;
+    };
+    if (s.type == GN_ORB) return std::sqrt(ctr[0] * ctr[0] + ctr[1] * ctr[1] + ctr[2] * ctr[2]) - rho - s.a > margin;
+    if (s.type == GN_BOX)
+        return beyond_plane(1, 0, 0, s.a) || beyond_plane(-1, 0, 0, s.a) || beyond_plane(0, 1, 0, s.b) || beyond_plane(0, -1, 0, s.b) ||
+               beyond_plane(0, 0, 1, s.c) || beyond_plane(0, 0, -1, s.c);
+    if (beyond_plane(0, 0, 1, s.c) || beyond_plane(0, 0, -1, s.c)) return true;
+    const double rc = std::sqrt(ctr[0] * ctr[0] + ctr[1] * ctr[1]);
+    if (s.type == GN_CONE) {                                                        // (r - u(z)) cs, u = r0 + m z (a, b of the record)
+        const double m = s.b, cs = 1.0 / std::sqrt(1.0 + m * m);
+        return (rc - (s.a + m * ctr[2])) * cs - rho > margin;
+    }
+    if (rc - rho - s.b > margin) return true;                                       // outside the outer cylinder
+    if (s.a > 0) {                                                                  // inside the hole
+        double rmax = 0;
+        for (int c = 0; c < 8; ++c) rmax = std::max(rmax, std::sqrt(q[c][0] * q[c][0] + q[c][1] * q[c][1]));
+        if (s.a - rmax > margin) return true;
+    }
+    if (s.sector && (beyond_plane(s.sS, -s.cS, 0, 0) || beyond_plane(-s.sE, s.cE, 0, 0))) return true;
+    return false;
+}
+
 template <class R> SolidRec<R> make_solid_rec(const HostSolid& s) {
     SolidRec<R> o;
     o.a = (R)s.a; o.b = (R)s.b; o.c = (R)s.c; o.cS = (R)s.cS; o.sS = (R)s.sS; o.cE = (R)s.cE; o.sE = (R)s.sE;
@@ -282,6 +321,22 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             if (fb < fa) fb = fa;
             a = (int)fa; b = (int)fb;
         };
+        // daughter j is listed in cell (ix, iy, iz) of a grid of n cells unless the solid itself provably stays clear of it
+        // (cell_excluded; margin = 16 delta + rounding, far beyond the 1.25 delta of the probes -- DESIGN.md reading 5)
+        const double excl_margin = 8.0 * std::max(geo->tol32, geo->tol64) + 256.0 * ext * 0x1p-23;
+        std::vector<char> tight(nd, 1);
+        auto in_cell = [&](int j, const int n[3], int ix, int iy, int iz) -> bool {
+            if (!tight[j]) return true;
+#ifdef GN_AABB_LISTS
+            return true;                          // diagnostics: candidate lists by bounding box only
+#endif
+            const int d = dlist[kids[mth].x + j];
+            const double* Rl = h_transforms + 12 * (size_t)h_placements[4 * (size_t)d + 3];
+            const int ii[3] = {ix, iy, iz};
+            double clo[3], chi[3];
+            for (int k = 0; k < 3; ++k) { const double w = (mhi[k] - mlo[k]) / n[k]; clo[k] = mlo[k] + ii[k] * w; chi[k] = mlo[k] + (ii[k] + 1) * w; }
+            return !cell_excluded(solids[node[d].y], Rl, Rl + 9, clo, chi, excl_margin);
+        };
         // refinement (the smart-voxel idea of choosing the cut that minimises candidate references): while cells hold
         // more than ~1 candidate on average, double the axis whose doubling shortens the lists most, within a budget of
         // 64 cells per daughter.  Short, equally long lists keep the lanes of a warp in step during relocation.
@@ -291,7 +346,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
                 int a[3], b[3];
                 for (int k = 0; k < 3; ++k) cell_range(j, k, n[k], a[k], b[k]);
                 for (int iz = a[2]; iz <= b[2]; ++iz) for (int iy = a[1]; iy <= b[1]; ++iy) for (int ix = a[0]; ix <= b[0]; ++ix)
-                    cnt[ix + (size_t)n[0] * (iy + (size_t)n[1] * iz)]++;
+                    if (in_cell(j, n, ix, iy, iz)) cnt[ix + (size_t)n[0] * (iy + (size_t)n[1] * iz)]++;
             }
             refs = 0; nonempty = 0;
             for (int c : cnt) if (c) { refs += c; nonempty += 1; }
@@ -319,10 +374,16 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         std::vector<int> c0(3 * (size_t)nd), c1(3 * (size_t)nd);
         for (int j = 0; j < nd; ++j) {
             for (int k = 0; k < 3; ++k) cell_range(j, k, G.n[k], c0[3 * (size_t)j + k], c1[3 * (size_t)j + k]);
+            int kept = 0;
             for (int iz = c0[3 * (size_t)j + 2]; iz <= c1[3 * (size_t)j + 2]; ++iz)
                 for (int iy = c0[3 * (size_t)j + 1]; iy <= c1[3 * (size_t)j + 1]; ++iy)
                     for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
-                        count[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++;
+                        kept += in_cell(j, G.n, ix, iy, iz) ? 1 : 0;
+            if (kept == 0) tight[j] = 0;          // a daughter outside its mother's grid: listed by its bounding box, as before
+            for (int iz = c0[3 * (size_t)j + 2]; iz <= c1[3 * (size_t)j + 2]; ++iz)
+                for (int iy = c0[3 * (size_t)j + 1]; iy <= c1[3 * (size_t)j + 1]; ++iy)
+                    for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
+                        if (in_cell(j, G.n, ix, iy, iz)) count[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++;
         }
         size_t base = cand.size();
         std::vector<size_t> pos(ncell);
@@ -332,7 +393,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             for (int iz = c0[3 * (size_t)j + 2]; iz <= c1[3 * (size_t)j + 2]; ++iz)
                 for (int iy = c0[3 * (size_t)j + 1]; iy <= c1[3 * (size_t)j + 1]; ++iy)
                     for (int ix = c0[3 * (size_t)j]; ix <= c1[3 * (size_t)j]; ++ix)
-                        cand[pos[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++] = d;
+                        if (in_cell(j, G.n, ix, iy, iz)) cand[pos[ix + (size_t)G.n[0] * (iy + (size_t)G.n[1] * iz)]++] = d;
         }
         // regular voxels: an unrotated leaf box that fills exactly one cell, alone -- in a mother that is a box spanned exactly
         // by the grid (so that cells at the rim are the only ones next to the mother's surface) and whose cells are much

@@ -30,8 +30,12 @@ namespace gn {
 // -------------------------------------------------------------------------------------------------------
 // transport
 // -------------------------------------------------------------------------------------------------------
-constexpr int TR_THREADS = 128;
+#ifndef TR_THREADS_N
+#define TR_THREADS_N 128          // threads per block of the transport kernels
+#endif
+constexpr int TR_THREADS = TR_THREADS_N;
 constexpr int TR_WARPS = TR_THREADS / 32;
+constexpr int TR_PER_128 = 128 / TR_THREADS;      // the min-blocks figures below are per 128 threads
 #ifndef TR_MIN_BLOCKS
 #define TR_MIN_BLOCKS 8          // general fp32 step pass: 64 registers, 32 warps / SM
 #endif
@@ -250,7 +254,7 @@ __device__ __noinline__ void birth_secondary(BirthIO<R>* io, const PairVtx<R>* v
 // back of the output queue; interact_pass handles them before the next pass.  PHYS = true: interactions happen inside
 // the pass (batched per warp); used for the last pass, which runs the few remaining photons to completion.
 template <class R, bool FROM_SOURCE, bool TRACK, bool PHYS, bool FLAT>
-__global__ void __launch_bounds__(TR_THREADS, PHYS ? 1 : (sizeof(R) == 4 ? (FROM_SOURCE ? TR_MIN_BLOCKS_SRC : (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX)) : TR_MIN_BLOCKS_F64))
+__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (PHYS ? 1 : (sizeof(R) == 4 ? (FROM_SOURCE ? TR_MIN_BLOCKS_SRC : (FLAT ? TR_MIN_BLOCKS : TR_MIN_BLOCKS_BOX)) : TR_MIN_BLOCKS_F64)))
 transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id, uint32_t n_src, const PassCounters* __restrict__ cin,
                PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin, PhotonRec<R>* __restrict__ qout, uint32_t cap,
                double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, int K, int regroup_pct, SortIO sio, SecIO<R> sec, int timed) {

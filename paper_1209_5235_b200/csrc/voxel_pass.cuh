@@ -28,7 +28,7 @@ template <class R> __device__ __forceinline__ bool direction_cacheable(const V3<
 }
 
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS, sizeof(R) == 4 ? VOX_MIN_BLOCKS : 4)
+__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? VOX_MIN_BLOCKS : 4))
 voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin,
            PhotonRec<R>* __restrict__ qout, PhotonRec<R>* __restrict__ S, uint32_t cap, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec,
            int K, int regroup_pct, int timed) {
@@ -163,7 +163,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
 // coming voxel_pass -- travelling ones behind its front segment, those that reached their interaction point to its back
 // segment, where interact_pass finds them; there is room, because front + back + flagged never exceeds the photons alive.
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS, sizeof(R) == 4 ? 6 : 2)
+__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? 6 : 2))
 general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* __restrict__ S, PhotonRec<R>* __restrict__ q, uint32_t cap,
              DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = ctr->slow;
