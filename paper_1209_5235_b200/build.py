@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("GN_LIB_OUT") or os.path.join(HERE, "libgammanav.so")      # GN_LIB_OUT: build a variant beside the product (diagnostics)
 SOURCES = ["transport_f32_box.cu", "transport_f32_gen.cu", "transport_f64_box.cu", "transport_f64_gen.cu", "nav_f32.cu", "nav_f64.cu", "noalloc.cu", "api.cu", "geometry.cu"]
-HEADERS = ["store.h", "geometry.h", "hostmath.h", "impl.h", "common.cuh", "nav.cuh", "physics.cuh", "nav_kernels.cuh", "transport.cuh", "voxel_pass.cuh",
+HEADERS = ["store.h", "geometry.h", "hostmath.h", "impl.h", "common.cuh", "nav.cuh", "physics.cuh", "nav_kernels.cuh", "transport.cuh", "voxel_pass.cuh", "coherent.cuh",
            os.path.join("..", "..", "include", "gammanav.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "--fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-Xptxas", "-v"]

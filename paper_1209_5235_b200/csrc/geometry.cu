@@ -259,6 +259,11 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     gn_opts o{}; if (h_opts) o = *h_opts;
     const HostSolid& ws = solids[node[0].y];
     double ext = ws.type == GN_BOX ? std::max(ws.a, std::max(ws.b, ws.c)) : (ws.type == GN_ORB ? ws.a : (ws.type == GN_CONE ? std::max(ws.rbound, ws.c) : std::max(ws.b, ws.c)));
+    {   // bounding box of the world solid (schedule only: the cells of the ray-coherent work order)
+        const double hxy = ws.type == GN_BOX ? ws.a : (ws.type == GN_ORB ? ws.a : (ws.type == GN_CONE ? ws.rbound : ws.b));
+        const double hb[3] = {hxy, ws.type == GN_BOX ? ws.b : hxy, ws.type == GN_ORB ? ws.a : ws.c};
+        for (int k = 0; k < 3; ++k) { geo->world_h[k] = (float)hb[k]; geo->world_c[k] = 0.0f; }
+    }
     geo->tol64 = o.tol64 > 0 ? o.tol64 : 1e-9;
     geo->tol32 = o.tol32 > 0 ? o.tol32 : (double)(float)(ext * 0x1p-18);
     if (!(o.sigma_pe0 > 0)) o.sigma_pe0 = 1750.0;

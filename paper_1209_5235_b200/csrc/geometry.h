@@ -17,6 +17,7 @@ struct gn_geometry {
     gn_opts opts{};
     int64_t n_grids = 0, n_cells = 0, n_cand = 0, device_bytes = 0;
     int device = 0;
+    float world_c[3] = {0, 0, 0}, world_h[3] = {1, 1, 1};      // bounding box of the world solid (centre, half extents): cells of the ray-coherent work order (coherent.cuh)
     bool voxel_sched = false;            // coherent and mostly regular voxels: lean passes are voxel_pass + slow_pass (voxel_pass.cuh)
     bool coherent = false;               // boxes only, no rotations, at most one candidate per voxel cell: lanes of a warp do the same thing per node visit
     // transport workspace (photon queues, counters, pinned read-back, events): grown on demand, reused by every

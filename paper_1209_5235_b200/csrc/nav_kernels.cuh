@@ -2,6 +2,7 @@
 // their launchers, templated on the precision; instantiated in nav_f32.cu / nav_f64.cu.
 #pragma once
 #include "common.cuh"
+#include "coherent.cuh"
 #include "impl.h"
 
 namespace gn {
@@ -128,7 +129,7 @@ __global__ void __launch_bounds__(NAV_THREADS) step_normal_kernel(GeoView<R> g, 
 template <class R, bool FLAT>
 __global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                                 const R* __restrict__ Yin, int64_t n, double mu_mass,
-                                                                R* __restrict__ T_out, uint32_t* __restrict__ nsteps_out) {
+                                                                R* __restrict__ T_out, uint32_t* __restrict__ nsteps_out, const uint32_t* __restrict__ perm) {
     __shared__ BlockTables<R> tab;
     __shared__ R sh_mu[MAX_SMEM_MATS];
     stage_tables(g, tab);
@@ -136,7 +137,8 @@ __global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, co
     for (int i = threadIdx.x; i < g.n_mats && i < MAX_SMEM_MATS; i += blockDim.x) sh_mu[i] = (R)(g.rho[i] * mu_mass / 10.0);
     __syncthreads();
     Navigator<R, true, FLAT> nav(g, &tab.ctx);
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    for (int64_t t_ = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t_ < n; t_ += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = perm ? (int64_t)perm[t_] : t_;                   // ray-coherent work order (coherent.cuh)
         V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
         const V3<R> w{dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
         NodeRec<R> nd;
@@ -159,6 +161,38 @@ __global__ void __launch_bounds__(NAV_THREADS) free_path_kernel(GeoView<R> g, co
         T_out[i] = T;
         if (nsteps_out) nsteps_out[i] = ns;
     }
+}
+
+// (key, rank) of every ray of a batch for the ray-coherent work order: cell of the position, bin of the direction
+template <class R>
+__global__ void __launch_bounds__(NAV_THREADS) coh_ray_keys_kernel(CohGrid cg, const R* __restrict__ pos, const R* __restrict__ dir, int64_t n,
+                                                                   unsigned* __restrict__ hist, uint2* __restrict__ kr) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint32_t key = coh_key(cg, (float)pos[3 * i], (float)pos[3 * i + 1], (float)pos[3 * i + 2],
+                                     (float)dir[3 * i], (float)dir[3 * i + 1], (float)dir[3 * i + 2], 0);
+        kr[i] = make_uint2(key, atomicAdd(&hist[key], 1u));
+    }
+}
+// Work order of a batch of rays (stream-ordered scratch from the handle's pool).  nullptr = arrival order: small batches, or
+// no scratch to be had.  The caller frees *scratch_out with cudaFreeAsync once its kernel is enqueued.
+constexpr int64_t COH_MIN_RAYS = 1 << 12;
+template <class R>
+static const uint32_t* ray_order(const gn_geometry* geo, const void* pos, const void* dir, int64_t n, cudaStream_t s, char** scratch_out) {
+    *scratch_out = nullptr;
+    if (n < COH_MIN_RAYS || n >= (1ll << 32) || !geo->pool) return nullptr;
+    const CohGrid cg = coh_grid(geo->world_c, geo->world_h, 4, 16, 1);            // 64 cells x 4096 direction bins
+    const unsigned nb = cg.buckets();
+    const size_t b_hist = ((size_t)nb * 4 + 255) & ~(size_t)255, b_tiles = (coh_tiles(nb) * 4 + 255) & ~(size_t)255, b_kr = ((size_t)n * 8 + 255) & ~(size_t)255;
+    char* scratch = nullptr;
+    if (cudaMallocFromPoolAsync((void**)&scratch, b_hist + b_tiles + b_kr + (size_t)n * 4, geo->pool, s) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    unsigned* hist = (unsigned*)scratch; unsigned* tiles = (unsigned*)(scratch + b_hist);
+    uint2* kr = (uint2*)(scratch + b_hist + b_tiles);
+    uint32_t* perm = (uint32_t*)(scratch + b_hist + b_tiles + b_kr);
+    cudaMemsetAsync(hist, 0, (size_t)nb * 4, s);
+    coh_ray_keys_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(cg, (const R*)pos, (const R*)dir, n, hist, kr);
+    coh_build_order(hist, nb, tiles, kr, n, nullptr, perm, s);
+    *scratch_out = scratch;
+    return perm;
 }
 
 template <class R> int locate_impl(const gn_geometry* geo, const void* pos, const void* dir, int64_t n, int32_t* out, cudaStream_t s) {
@@ -225,9 +259,15 @@ template <class R> int free_path_impl(const gn_geometry* geo, const void* pos, c
     if (n == 0) return GN_OK;
     const int64_t blocks = (n + NAV_THREADS - 1) / NAV_THREADS;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(blocks, 148 * 64));
-    if (geo->coherent) free_path_kernel<R, false><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
-    else free_path_kernel<R, true><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns);
-    GN_CUDA(cudaGetLastError(), "gn_free_path_run launch");
+    // one thread walks one particle to the end: lanes that start close together and look the same way visit the same
+    // cells and daughters, so the particles are walked in ray-coherent order (Random set, N = 1e5: 1.4x; 1e6: 2.4x)
+    char* scratch = nullptr;
+    const uint32_t* perm = ray_order<R>(geo, pos, dir, n, s, &scratch);
+    if (geo->coherent) free_path_kernel<R, false><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns, perm);
+    else free_path_kernel<R, true><<<grid, NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, (const R*)Y, n, mu_mass, (R*)T, ns, perm);
+    const cudaError_t e = cudaGetLastError();
+    if (scratch) cudaFreeAsync(scratch, s);
+    GN_CUDA(e, "gn_free_path_run launch");
     return GN_OK;
 }
 
