@@ -453,6 +453,9 @@ def run_ours(args):
                 traffic = json.load(open(tpath)).get(f"{wl.name}_fp{precision}")
             except Exception:
                 traffic = None
+        traffic_note = None
+        if isinstance(traffic, dict):                          # per launch of the dominant kernel, from the committed ncu capture
+            traffic, traffic_note = traffic.get("dram_bytes_per_launch"), traffic.get("note")
         if bound == "hbm":
             ach, pk, un, fr = (dom_rate * abytes / 1e9 if dom_rate else None), peak, "GB/s", dh
         else:
@@ -469,7 +472,9 @@ def run_ours(args):
                                   "note": "all kernels of a run: units of the run / CUDA-event time of the whole launch sequence"},
                     "note": "bound = the slower of (algorithmic bytes / measured HBM bandwidth) and (algorithmic flops / measured pipe peak) per unit; "
                             "a fraction above 1 on the HBM leg means the kernel does not move the algorithmic bytes: a pass keeps the photon in registers "
-                            "for up to K steps, so the record is read and written once per pass, not once per step (traffic = ncu dram bytes of one run)"}
+                            "for up to K steps, so the record is read and written once per pass, not once per step (traffic = ncu dram bytes of one launch of the dominant kernel, profiles/traffic.json)"}
+        if traffic_note:
+            roofline["traffic_note"] = traffic_note
         if op_mix:
             roofline["ops_per_unit"] = op_mix
         line = {"metric": "transported photon steps/s" if transport else "ComputeStep queries/s",
