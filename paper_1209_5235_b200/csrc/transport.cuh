@@ -291,6 +291,10 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     uint64_t h = 0xcbf29ce484222325ull;
     int vol = -1; NodeRec<R> nd = {};
     unsigned c_steps = 0;
+    // events of this lane's photon inside the pass (tail pass only; a lane follows one photon): Compton scatters in bits 0-15,
+    // Rayleigh scatters in 16-28, energy cut / photoelectric / pair (at most one each) in bits 29 / 30 / 31; summed per warp
+    // at the end (a 64-bit shared-memory atomic per lane and event is a compare-and-swap loop under contention)
+    unsigned c_ev = 0;
     bool pending = false;       // the photon sits at its interaction point, waiting for an interaction phase
 
     if (FROM_SOURCE) {
@@ -380,18 +384,20 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
                 dep_d = (double)io.dep;
                 if (ev == EV_RAYLEIGH) {
                     w.x = io.wx; w.y = io.wy; w.z = io.wz; Y = io.Y;
-                    atomicAdd(&sh_cnt[ST_RAYLEIGH], 1ull);
+                    c_ev += 1u << 16;
+                    if (((c_ev >> 16) & 0x1fffu) == 0x1fffu) { atomicAdd(&sh_cnt[ST_RAYLEIGH], 0x1fffull); c_ev &= ~(0x1fffu << 16); }      // field full: flush
                     if (FASTV) lane_direction(w, g.delta, vl);
                 } else if (ev == EV_COMPTON || ev == EV_CUT) {
                     E = io.E; w.x = io.wx; w.y = io.wy; w.z = io.wz;
-                    atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
-                    if (ev == EV_CUT) { atomicAdd(&sh_cnt[ST_CUT], 1ull); fate = FATE_ABSORBED; }
+                    c_ev += 1u;
+                    if ((c_ev & 0xffffu) == 0xffffu) { atomicAdd(&sh_cnt[ST_COMPTON], 0xffffull); c_ev &= ~0xffffu; }                        // field full: flush
+                    if (ev == EV_CUT) { c_ev |= 1u << 29; fate = FATE_ABSORBED; }
                     else {
                         Y = io.Y; gPE = io.gPE; gKN = io.gKN; L2k = io.L2k; above = io.above;
                         if (FASTV) lane_direction(w, g.delta, vl);
                     }
                 } else {
-                    atomicAdd(&sh_cnt[ev == EV_PE ? ST_PE : ST_PAIR], 1ull);
+                    c_ev |= ev == EV_PE ? 1u << 30 : 1u << 31;
                     fate = FATE_ABSORBED;
                 }
                 finish_step(ev, vol);
@@ -485,6 +491,17 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
             double es = warp_sum(fate == FATE_STUCK ? (double)E : 0.0);
             if (lane == 0) { atomicAdd(&sh_cnt[ST_STUCK], (unsigned long long)ns); atomicAdd(&sh_en[EN_STUCK], es); }
         }
+        if (PHYS) {
+            const unsigned nc = warp_sum(c_ev & 0xffffu), nr = warp_sum((c_ev >> 16) & 0x1fffu), nx = warp_sum((c_ev >> 29) & 1u),
+                           ne = warp_sum((c_ev >> 30) & 1u), np = warp_sum(c_ev >> 31);
+            if (lane == 0) {
+                if (nc) atomicAdd(&sh_cnt[ST_COMPTON], (unsigned long long)nc);
+                if (nr) atomicAdd(&sh_cnt[ST_RAYLEIGH], (unsigned long long)nr);
+                if (nx) atomicAdd(&sh_cnt[ST_CUT], (unsigned long long)nx);
+                if (ne) atomicAdd(&sh_cnt[ST_PE], (unsigned long long)ne);
+                if (np) atomicAdd(&sh_cnt[ST_PAIR], (unsigned long long)np);
+            }
+        }
     }
     __syncthreads();
     GN_CHECK(cout->front + cout->back <= cap, CHK_SEGMENTS);
@@ -497,8 +514,11 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 // The interaction wavefront (A6-A9): every photon parked at an interaction point by the previous pass sits in the
 // back segment of the queue (slots cap-1, cap-2, ...); one thread per photon samples the process, updates the record
 // in place (absorbed photons are marked vol = -1) and the warp tallies the deposits.
+#ifndef INTERACT_MIN_BLOCKS
+#define INTERACT_MIN_BLOCKS 6      // 80 registers, 24 warps / SM (1 block: 82 registers -- the same code, but the occupancy is then promised)
+#endif
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS)
+__global__ void __launch_bounds__(TR_THREADS, sizeof(R) == 4 ? INTERACT_MIN_BLOCKS : (INTERACT_MIN_BLOCKS + 1) / 2)
 interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters* __restrict__ cin, PhotonRec<R>* __restrict__ q, uint32_t cap,
               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = cin->back;
@@ -510,7 +530,7 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
     __syncthreads();
     const unsigned i = blockIdx.x * TR_THREADS + threadIdx.x;
     const bool active = i < n;
-    double dep_d = 0.0; int vol = 0;
+    double dep_d = 0.0; int vol = 0, ev_done = -1;
     if (active) {
         GN_CHECK(n <= cap, CHK_LOAD_SLOT);
         PhotonRec<R> r; load_rec(q, cap - 1u - i, r);
@@ -526,15 +546,13 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = r.x; pv.y = r.y; pv.z = r.z; pv.idx = r.idx; const unsigned ps = atomicAdd(sec.n_out, 1u); GN_CHECK(ps < cap, CHK_PAIR_SLOT); sec.out[ps] = pv; }
         dep_d = (double)io.dep;
         bool alive = false;
+        ev_done = ev;                                                          // counted per warp below
         if (ev == EV_RAYLEIGH) {
             r.wx = io.wx; r.wy = io.wy; r.wz = io.wz; r.Y = io.Y; alive = true;
-            atomicAdd(&sh_cnt[ST_RAYLEIGH], 1ull);
         } else if (ev == EV_COMPTON || ev == EV_CUT) {
             r.E = io.E; r.wx = io.wx; r.wy = io.wy; r.wz = io.wz;
-            atomicAdd(&sh_cnt[ST_COMPTON], 1ull);
-            if (ev == EV_CUT) atomicAdd(&sh_cnt[ST_CUT], 1ull);
-            else { r.Y = io.Y; r.gPE = io.gPE; r.gKN = io.gKN; r.L2k = io.L2k; r.tail[0] = (uint32_t)io.above; alive = true; }
-        } else atomicAdd(&sh_cnt[ev == EV_PE ? ST_PE : ST_PAIR], 1ull);
+            if (ev != EV_CUT) { r.Y = io.Y; r.gPE = io.gPE; r.gKN = io.gKN; r.L2k = io.L2k; r.tail[0] = (uint32_t)io.above; alive = true; }
+        }
         r.ctr = io.j;
         if (alive && (r.misc & 0xffu) >= (uint32_t)g.stuck_limit) {           // stuck guard (C9), after the step's event
             ev = EV_STUCK; alive = false;
@@ -548,6 +566,18 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         }
         if (alive) r.tail[0] &= 1u; else r.vol = -1;
         store_rec(q, cap - 1u - i, r);
+    }
+    {   // event counters: one ballot per kind of event, one shared atomic per warp and counter that is not zero
+        const unsigned nC = __popc(__ballot_sync(0xffffffffu, ev_done == EV_COMPTON || ev_done == EV_CUT)), nX = __popc(__ballot_sync(0xffffffffu, ev_done == EV_CUT));
+        const unsigned nE = __popc(__ballot_sync(0xffffffffu, ev_done == EV_PE)), nP = __popc(__ballot_sync(0xffffffffu, ev_done == EV_PAIR));
+        const unsigned nR = __popc(__ballot_sync(0xffffffffu, ev_done == EV_RAYLEIGH));
+        if ((threadIdx.x & 31) == 0) {
+            if (nC) atomicAdd(&sh_cnt[ST_COMPTON], (unsigned long long)nC);
+            if (nX) atomicAdd(&sh_cnt[ST_CUT], (unsigned long long)nX);
+            if (nE) atomicAdd(&sh_cnt[ST_PE], (unsigned long long)nE);
+            if (nP) atomicAdd(&sh_cnt[ST_PAIR], (unsigned long long)nP);
+            if (nR) atomicAdd(&sh_cnt[ST_RAYLEIGH], (unsigned long long)nR);
+        }
     }
     warp_tally(edep, &sh_en[EN_DEPOSITED], vol, dep_d, active);
     __syncthreads();
