@@ -20,6 +20,9 @@ enum : uint32_t { REC_ABOVE = 1u, REC_PENDING = 2u };      // PhotonRec::tail[0]
 #ifndef VOX_MIN_BLOCKS
 #define VOX_MIN_BLOCKS 8            // 64 registers: 32 warps / SM (10 blocks = 48 registers spill)
 #endif
+#ifndef GENERAL_MIN_BLOCKS
+#define GENERAL_MIN_BLOCKS 6        // general_pass, fp32: 80 registers, 24 warps / SM
+#endif
 constexpr int SLOW_STEPS = 8;       // general steps a flagged photon may take in one slow_pass
 
 template <class R> __device__ __forceinline__ bool direction_cacheable(const V3<R>& w, R delta) {
@@ -163,7 +166,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
 // coming voxel_pass -- travelling ones behind its front segment, those that reached their interaction point to its back
 // segment, where interact_pass finds them; there is room, because front + back + flagged never exceeds the photons alive.
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? 6 : 2))
+__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? GENERAL_MIN_BLOCKS : 2))
 general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* __restrict__ S, PhotonRec<R>* __restrict__ q, uint32_t cap,
              DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = ctr->slow;
