@@ -285,6 +285,10 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     // ---- voxel grids (C5): one uniform 3-D grid per mother = three nested levels of uniform slices, flattened
     std::vector<HostGrid> grids;
     std::vector<int> regular_cell(V, -1);      // leaf box that coincides with one voxel cell of its mother: ix | iy << 10 | iz << 20
+    // regular slab: an unrotated leaf box that coincides with a row of cells along ONE axis, alone in each of them (a layer of a
+    // sampling calorimeter in a grid whose pitch divides every layer thickness): lowest cell, axis, number of cells, walls
+    struct SlabInfo { int cell = -1, axis = 0, span = 0, walls = 0; };
+    std::vector<SlabInfo> slab(V);
     std::vector<int> cell_start(1, 0), cand;
     const double shrink = geo->tol64 / 8;
     for (size_t mth = 0; mth < V; ++mth) {
@@ -419,12 +423,49 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             if (count[cell] != 1) continue;
             regular_cell[d] = c0[3 * (size_t)j] | (c0[3 * (size_t)j + 1] << 10) | (c0[3 * (size_t)j + 2] << 20);
         }
+        for (int j = 0; j < nd && regular_mother; ++j) {                   // regular slabs
+            int d = dlist[kids[mth].x + j];
+            if (regular_cell[d] >= 0 || kids[d].y != 0 || solids[node[d].y].type != GN_BOX) continue;
+            const double* Rl = h_transforms + 12 * (size_t)h_placements[4 * (size_t)d + 3];
+            bool ok = Rl[0] == 1.0 && Rl[4] == 1.0 && Rl[8] == 1.0 && Rl[1] == 0.0 && Rl[2] == 0.0 && Rl[3] == 0.0 && Rl[5] == 0.0 && Rl[6] == 0.0 && Rl[7] == 0.0;
+            int axis = -1, span = 1;
+            for (int k = 0; k < 3 && ok; ++k) {
+                const int a = c0[3 * (size_t)j + k], b = c1[3 * (size_t)j + k];
+                ok = std::fabs(blo[3 * (size_t)j + k] - (G.gmin[k] + a * G.w[k])) <= geo->tol64 && std::fabs(bhi[3 * (size_t)j + k] - (G.gmin[k] + (b + 1) * G.w[k])) <= geo->tol64;
+                if (b > a) { ok = ok && axis < 0 && b - a + 1 <= 4096; axis = k; span = b - a + 1; }
+            }
+            if (!ok || axis < 0) continue;
+            int walls = 0;
+            for (int k = 0; k < 3; ++k) walls |= (c0[3 * (size_t)j + k] == 0 ? 1 << (2 * k) : 0) | (c1[3 * (size_t)j + k] == G.n[k] - 1 ? 2 << (2 * k) : 0);
+            size_t cell0 = c0[3 * (size_t)j] + (size_t)G.n[0] * (c0[3 * (size_t)j + 1] + (size_t)G.n[1] * c0[3 * (size_t)j + 2]);
+            const size_t stride = axis == 0 ? 1 : (axis == 1 ? (size_t)G.n[0] : (size_t)G.n[0] * G.n[1]);
+            for (int q = 0; q < span && ok; ++q) ok = count[cell0 + q * stride] == 1;
+            if (!ok || cell0 + (size_t)span * stride >= (1u << 30)) continue;
+            slab[d].cell = (int)cell0; slab[d].axis = axis; slab[d].span = span; slab[d].walls = walls;
+        }
         G.mother = (int)mth;
         node[mth].w = (int)grids.size();
         grids.push_back(G);
         geo->n_cells += (int64_t)ncell;
     }
     geo->n_grids = (int64_t)grids.size(); geo->n_cand = (int64_t)cand.size();
+
+    // a solid carries the axis and the number of cells of its regular slabs (SolidRec: cS, sS of a box): every slab placement
+    // of one solid must agree, and the mother's grid id must fit the node record; the others stay ordinary boxes
+    {
+        std::vector<int> s_axis(solids.size(), -1), s_span(solids.size(), 0);
+        std::vector<char> s_bad(solids.size(), 0);
+        for (size_t i = 0; i < V; ++i) {
+            if (slab[i].cell < 0) continue;
+            const int si = node[i].y;
+            if (node[node[i].x].w > NODE_GRID_MASK) { slab[i].cell = -1; continue; }
+            if (s_axis[si] < 0) { s_axis[si] = slab[i].axis; s_span[si] = slab[i].span; }
+            else if (s_axis[si] != slab[i].axis || s_span[si] != slab[i].span) s_bad[si] = 1;
+        }
+        for (size_t i = 0; i < V; ++i) if (slab[i].cell >= 0 && s_bad[node[i].y]) slab[i].cell = -1;
+        for (size_t si = 0; si < solids.size(); ++si)
+            if (solids[si].type == GN_BOX) { const bool on = s_axis[si] >= 0 && !s_bad[si]; solids[si].cS = on ? s_axis[si] : -1; solids[si].sS = on ? s_span[si] : 1; }
+    }
 
     // ---- per-precision tables (store.h): node records with Tg inline, padded rotations
     std::vector<NodeRec<float>> n32(V); std::vector<NodeRec<double>> n64(V);
@@ -450,6 +491,10 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             for (int k = 0; k < 3; ++k) walls |= (c[k] == 0 ? 1 << (2 * k) : 0) | (c[k] == G.n[k] - 1 ? 2 << (2 * k) : 0);
             a.info = b.info = a.info | NODE_REGULAR | (gid << NODE_GRID_SHIFT) | (walls << NODE_WALL_SHIFT);
             a.link = b.link = c[0] + G.n[0] * (c[1] + G.n[1] * c[2]);
+        } else if (slab[i].cell >= 0) {
+            const int gid = node[node[i].x].w;
+            a.info = b.info = a.info | NODE_SLAB | (gid << NODE_GRID_SHIFT) | (slab[i].walls << NODE_WALL_SHIFT);
+            a.link = b.link = slab[i].cell;
         }
         b.pad = 0;
         for (int k = 0; k < 3; ++k) { b.t[k] = Tg[3 * i + k]; a.t[k] = (float)Tg[3 * i + k]; }
@@ -504,7 +549,9 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         for (const int2& c : cells) coherent = coherent && c.y <= 1;
         geo->coherent = coherent;
         size_t n_regular = 0;
-        for (size_t i = 0; i < V; ++i) n_regular += (n32[i].info & NODE_REGULAR) ? 1 : 0;
+        bool has_slabs = false;
+        for (size_t i = 0; i < V; ++i) { n_regular += (n32[i].info & (NODE_REGULAR | NODE_SLAB)) ? 1 : 0; has_slabs = has_slabs || (n32[i].info & NODE_SLAB); }
+        geo->has_slabs = has_slabs;
         geo->voxel_sched = coherent && 2 * n_regular >= V && geo->opts.no_voxel_pass <= 0 && geo->opts.rayleigh <= 0 && geo->opts.pe_table_per_decade <= 0 && n_solids <= 32 && n_mats <= 32 && grids.size() <= 8 && ext < 0x1p50;      // table sizes: MAX_SMEM_* of common.cuh
         if (regroup_default) geo->opts.regroup_percent = coherent ? 50 : 75;
         if (steps_default && geo->voxel_sched) geo->opts.steps_per_pass = 24;      // the regular-voxel pass is cheap per step: fewer, longer passes (measured)

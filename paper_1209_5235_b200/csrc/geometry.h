@@ -19,6 +19,7 @@ struct gn_geometry {
     int device = 0;
     float world_c[3] = {0, 0, 0}, world_h[3] = {1, 1, 1};      // bounding box of the world solid (centre, half extents): cells of the ray-coherent work order (coherent.cuh)
     bool voxel_sched = false;            // coherent and mostly regular voxels: lean passes are voxel_pass + slow_pass (voxel_pass.cuh)
+    bool has_slabs = false;              // some leaf boxes are regular slabs (NODE_SLAB): the regular-voxel step kernel is built with the slab rule
     bool coherent = false;               // boxes only, no rotations, at most one candidate per voxel cell: lanes of a warp do the same thing per node visit
     // transport workspace (photon queues, counters, pinned read-back, events): grown on demand, reused by every
     // gn_transport_run on this handle, released by gn_geometry_destroy; runs on one handle are serialised

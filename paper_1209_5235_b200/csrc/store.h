@@ -16,6 +16,11 @@
 //             without the general cell lookup (nav.cuh: settle, regular_step; box-only kernels).  Only mothers that are
 //             unrotated boxes whose grid spans them exactly hand out this flag, so a point within the probe distance of
 //             the voxel whose neighbour cell on that side exists is inside the mother by more than delta
+//             flag NODE_SLAB (leaf boxes only): the same for a box that coincides with a ROW of cells along one axis, alone in
+//             each (a calorimeter layer in a grid whose pitch divides every layer thickness); link = index of its lowest
+//             cell; the axis and the number of cells of the row are in its solid record (cS, sS of a box); wall bits for the
+//             two ends of the row and the sides.  A photon leaving it through one of the two end faces finds its candidate in
+//             the cell beyond that end (nav.cuh: regular_step<.., SLABS>)
 //   rot[i]    M (row-major, global->local rotation), 9 Real padded to 12 (fp32, three 16-byte loads) /
 //             10 (fp64, five 16-byte loads);  p_local = M (x - Tg)
 //   solids, mats, grids: small tables (staged to shared memory by every kernel)
@@ -28,11 +33,12 @@ namespace gn {
 
 enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2, SOLID_CONE = 3 };
 enum : int { TUBE_SECTOR = 1, TUBE_HOLE = 2 };
-enum : int { NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SOLID_MASK = 0xffff, NODE_GRID_SHIFT = 16, NODE_GRID_MASK = 0x3f, NODE_WALL_SHIFT = 22, NODE_WALL_MASK = 0x3f };
+enum : int { NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SLAB = 1 << 28, NODE_SOLID_MASK = 0xffff, NODE_GRID_SHIFT = 16, NODE_GRID_MASK = 0x3f, NODE_WALL_SHIFT = 22, NODE_WALL_MASK = 0x3f };
 
 template <class R> struct SolidRec {
     R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -      CONE: r0 = (r1 + r2)/2, slope m, hz
-    R cS, sS, cE, sE;     // trig of sphi and sphi + dphi (host libm, fp64, rounded once);  CONE: cS = 1/sqrt(1 + m^2)
+    R cS, sS, cE, sE;     // trig of sphi and sphi + dphi (host libm, fp64, rounded once);  CONE: cS = 1/sqrt(1 + m^2);
+                          // BOX: cS = axis of its regular slabs (-1: none), sS = cells per slab (NODE_SLAB)
     int type, flags;
 };
 

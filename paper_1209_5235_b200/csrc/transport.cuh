@@ -419,11 +419,11 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         if (todo) mu = photon_mu(g, mats[nd.mat], nd.mat, E, gPE, gKN, L2k, above).tot;
         if (FASTV) {
             bool stepped = false;
-            if (todo && !bailed && vl.ok && (nd.info & NODE_REGULAR)) {
+            if (todo && !bailed && vl.ok && (nd.info & (NODE_REGULAR | NODE_SLAB))) {
                 if ((nd.info & NODE_SOLID_MASK) != vl.solid) lane_solid(nav.solids, nd.info, vl);
                 R step = 0; V3<R> xn{0, 0, 0};
                 const int vol_before = vol;
-                const int rc = regular_step(g, nav.grids, x, w, vl, mu, Y, vol, nd, step, xn);
+                const int rc = regular_step<R, true>(g, nav.grids, nav.solids, x, w, vl, mu, Y, vol, nd, step, xn);
                 if (rc == REG_BAIL) { bailed = true; GN_DBG(1, 1); }
                 else {
                     GN_DBG(0, 1);
@@ -855,8 +855,8 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
                         else general_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_slow, in, (uint32_t)cap, d_stats, pp, sec);
                         launch_interact<R>(track, blocks, s, g, seed, fid, d_ctr + p, in, (uint32_t)cap, d_edep, d_stats, pp, sec);
                         if (timed) cudaEventRecord(tev[2 * n_timed], s);
-                        if (track) voxel_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, d_slow, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
-                        else voxel_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, d_slow, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
+                        auto vp = geo->has_slabs ? (track ? voxel_pass<R, true, true> : voxel_pass<R, false, true>) : (track ? voxel_pass<R, true, false> : voxel_pass<R, false, false>);
+                        vp<<<blocks, TR_THREADS, 0, s>>>(g, d_ctr + p, d_ctr + p + 1, in, out, d_slow, (uint32_t)cap, d_stats, pp, sec, K, regroup, timed ? 1 : 0);
                         ++launches;
                     }
                 } else {

@@ -30,7 +30,7 @@ template <class R> __device__ __forceinline__ bool direction_cacheable(const V3<
     return c.ok;
 }
 
-template <class R, bool TRACK>
+template <class R, bool TRACK, bool SLABS>
 __global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? VOX_MIN_BLOCKS : 4))
 voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin,
            PhotonRec<R>* __restrict__ qout, PhotonRec<R>* __restrict__ S, uint32_t cap, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec,
@@ -74,7 +74,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
             nd = load_node(g.node, vol);
             lane_direction(w, g.delta, vl);
             lane_solid(solids, nd.info, vl);
-            if (!(nd.info & NODE_REGULAR) || !vl.ok) needgen = true;
+            if (!(nd.info & (NODE_REGULAR | (SLABS ? NODE_SLAB : 0))) || !vl.ok) needgen = true;
             if (TRACK && !pending && !needgen) h = pp.hash[idx];
         }
     }
@@ -94,7 +94,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
             const R mu = (muPE + muC) + muP;
             R step = 0; V3<R> xn{0, 0, 0};
             const int vol_before = vol;
-            const int rc = regular_step(g, grids, x, w, vl, mu, Y, vol, nd, step, xn);
+            const int rc = regular_step<R, SLABS>(g, grids, solids, x, w, vl, mu, Y, vol, nd, step, xn);
             if (rc == REG_BAIL) needgen = true;
             else {
                 ++c_steps; misc += 0x100u;
@@ -220,7 +220,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
             if (vol < 0) { ev = EV_ESCAPE; alive = false; ++c_esc; e_esc += (double)r.E; }
             else if (zs >= (uint32_t)g.stuck_limit) { ev = EV_STUCK; alive = false; ++c_stuck; e_stuck += (double)r.E; }      // stuck guard (C9)
             if (TRACK) { fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev); if (!alive) history_out(pp, sec, r.idx, h, misc >> 8, r.E); }
-            if (!alive || ((nd.info & NODE_REGULAR) && cacheable)) break;  // gone, or voxel_pass takes over
+            if (!alive || ((nd.info & (NODE_REGULAR | NODE_SLAB)) && cacheable)) break;  // gone, or voxel_pass takes over
         }
         if (TRACK && alive) pp.hash[r.idx] = h;
         r.x = x.x; r.y = x.y; r.z = x.z; r.Y = Y; r.misc = misc; r.vol = vol;

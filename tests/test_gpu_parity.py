@@ -301,6 +301,42 @@ def test_transport_fp32_aggregate(B, name):
     print(f"{name} fp32 identical histories: {frac:.5f}")
 
 
+def _layer_stack(axis, thicknesses=(2.0, 4.0, 6.0, 2.0), periods=6, half=150.0):
+    """Layers of several thicknesses (multiples of the thinnest) stacked along `axis` in a mother box: the voxel grid's pitch is
+    the thinnest layer, so the thin layers are regular voxels and the others regular slabs of 2 and 3 cells (store.h NODE_SLAB)."""
+    from paper_1209_5235_b200.workloads import _Builder
+    b = _Builder(f"layer_stack_axis{axis}")
+    L = periods * sum(thicknesses)
+    def dims(t):
+        h = [half, half, half]; h[axis] = t / 2
+        return h
+    world = b.place(-1, b.box(400.0, 400.0, 400.0), "air")
+    mh = [half, half, half]; mh[axis] = L / 2
+    mother = b.place(world, b.box(*mh), "air")
+    solids = [b.box(*dims(t)) for t in thicknesses]
+    mats = ["lead", "scint", "iron", "water"]
+    u = -L / 2
+    for _ in range(periods):
+        for k, t in enumerate(thicknesses):
+            T = [0.0, 0.0, 0.0]; T[axis] = u + t / 2
+            b.place(mother, solids[k], mats[k % len(mats)], T=tuple(T)); u += t
+    return b.finish()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_regular_slabs_along_every_axis(B, axis, precision):
+    """The slab rule of the regular-voxel step kernel (nav.cuh regular_step<.., SLABS>): stacks along x, y and z whose layers
+    are 1, 2 and 3 grid cells thick, entered obliquely so that photons cross layers both ways, leave through the sides (the
+    general step) and change solid at every boundary.  Histories against the oracle as for every other geometry."""
+    geom = _layer_stack(axis)
+    d = [0.25, 0.15, 0.15]; d[axis] = 1.0
+    o = [3.0, -2.0, 1.0]; o[axis] = -300.0
+    src = W.Source(W.SRC_GAUSS_PENCIL, tuple(o), tuple(d), W.E_MONO, 3.0, 0.0, 8.0)
+    got, ref, frac = compare_transport(B, geom, src, 20000, 11 + axis, precision, 0.999 if precision == 64 else 0.97)
+    assert got["stats"]["n_steps"] > 20000 * 10 and got["stats"]["n_escaped"] > 0 and (got["edep"].cpu().numpy()[2:] > 0).sum() >= 20
+
+
 # ---- stuck guard (SURVEY 8(c) C9, DESIGN.md reading 7): the EV_STUCK branch on every schedule ----------------------------
 def _big_water():
     from paper_1209_5235_b200.workloads import _Builder
