@@ -460,7 +460,7 @@ def run_ours(args):
             ach, pk, un, fr = (dom_rate * abytes / 1e9 if dom_rate else None), peak, "GB/s", dh
         else:
             ach, pk, un, fr = (dom_rate * flops_per_unit / 1e12 if dom_rate else None), pipe_tflops, "TFLOP/s", da
-        voxel = transport and wl.name.startswith("config3")
+        voxel = transport and wl.name.startswith(("config3", "config2"))      # geometries of regular voxels / slabs run the voxel schedule (gn_geometry::voxel_sched)
         roofline = {"bound": bound, "achieved": ach, "peak": pk, "unit": un, "frac": fr, "traffic": traffic,
                     "peak_source": peak_src if bound == "hbm" else pipe_src,
                     "kernel": ("voxel_pass (regular-voxel step pass)" if voxel else "transport_pass<R,0,0,0> (lean wavefront step pass)") if transport else "locate_kernel + query sort + step_kernel",
