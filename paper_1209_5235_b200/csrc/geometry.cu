@@ -467,6 +467,59 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
             if (solids[si].type == GN_BOX) { const bool on = s_axis[si] >= 0 && !s_bad[si]; solids[si].cS = on ? s_axis[si] : -1; solids[si].sS = on ? s_span[si] : 1; }
     }
 
+    // ---- sibling hints (store.h NODE_HINT): a full tube whose daughters are one tube-sector solid on a cylindrical lattice --
+    // N_phi sectors around, N_z along z, same radii as the mother (a segmented barrel).  A photon that leaves such a sector
+    // through ONE of its z or phi faces, farther than 2 probe distances from every other face, can only be in the sibling
+    // across that face or in the mother: every other sibling lies behind a second face of the sector left, i.e. farther than
+    // delta from the point.  hint[4 d + {0,1,2,3}] = sibling across the lower / upper z face, the start / end phi plane (-1: none)
+    std::vector<int> hint(4 * V, -1);
+    std::vector<char> hinted(V, 0);
+    for (size_t mth = 0; mth < V; ++mth) {
+        const int nd = kids[mth].y;
+        const HostSolid& ms = solids[node[mth].y];
+        if (nd < 8 || ms.type != GN_TUBE || ms.sector || !(ms.a > 0)) continue;
+        const int S = node[dlist[kids[mth].x]].y;
+        const HostSolid& ss = solids[S];
+        const double margin = 2.0 * (1.25 * 0.5 * std::max(geo->tol32, geo->tol64) + 4.0 * ext * 0x1p-23);      // 2 x the fp32 probe distance
+        if (ss.type != GN_TUBE || !ss.sector || std::fabs(ss.a - ms.a) > geo->tol64 || std::fabs(ss.b - ms.b) > geo->tol64) continue;
+        const double two_pi = 6.283185307179586476925;
+        const int n_phi = (int)std::lround(two_pi / ss.dphi), n_z = (int)std::lround(ms.c / ss.c);
+        if (n_phi < 3 || n_z < 1 || std::fabs(n_phi * ss.dphi - two_pi) > 1e-9 || std::fabs(n_z * ss.c - ms.c) > geo->tol64) continue;
+        if ((size_t)n_phi * n_z > (1u << 24)) continue;
+        if (!(2 * ss.c > 16 * margin && ss.b - ss.a > 16 * margin && ss.a * std::sin(ss.dphi) > 16 * margin && ss.dphi < 1.6)) continue;
+        std::vector<int> slot((size_t)n_phi * n_z, -1);
+        bool ok = true;
+        for (int j = 0; j < nd && ok; ++j) {
+            const int d = dlist[kids[mth].x + j];
+            const double* Rl = h_transforms + 12 * (size_t)h_placements[4 * (size_t)d + 3];
+            const double* T = Rl + 9;
+            ok = node[d].y == S && std::fabs(Rl[8] - 1.0) < 1e-12 && std::fabs(Rl[2]) < 1e-12 && std::fabs(Rl[5]) < 1e-12 && std::fabs(Rl[6]) < 1e-12 &&
+                 std::fabs(Rl[7]) < 1e-12 && std::fabs(Rl[0] - Rl[4]) < 1e-12 && std::fabs(Rl[1] + Rl[3]) < 1e-12 && std::fabs(T[0]) <= geo->tol64 && std::fabs(T[1]) <= geo->tol64;
+            if (!ok) break;
+            double th = std::atan2(Rl[3], Rl[0]); if (th < 0) th += two_pi;
+            const long jj = std::lround(th / ss.dphi);
+            const long iz = std::lround((T[2] + ms.c - ss.c) / (2 * ss.c));
+            double dth = std::fabs(th - jj * ss.dphi);
+            ok = dth < 1e-9 && iz >= 0 && iz < n_z && std::fabs(T[2] - (-ms.c + ss.c * (2 * iz + 1))) <= geo->tol64;
+            if (!ok) break;
+            int& sl = slot[(size_t)iz * n_phi + (size_t)(jj % n_phi)];
+            ok = sl < 0; sl = d;
+        }
+        if (!ok) continue;
+        for (int iz = 0; iz < n_z; ++iz) for (int jp = 0; jp < n_phi; ++jp) {
+            const int d = slot[(size_t)iz * n_phi + jp];
+            if (d < 0) continue;
+            hinted[d] = 1;
+            hint[4 * (size_t)d + 0] = iz > 0 ? slot[(size_t)(iz - 1) * n_phi + jp] : -1;
+            hint[4 * (size_t)d + 1] = iz + 1 < n_z ? slot[(size_t)(iz + 1) * n_phi + jp] : -1;
+            hint[4 * (size_t)d + 2] = slot[(size_t)iz * n_phi + (jp + n_phi - 1) % n_phi];        // across the start plane
+            hint[4 * (size_t)d + 3] = slot[(size_t)iz * n_phi + (jp + 1) % n_phi];                // across the end plane
+        }
+    }
+#ifdef GN_NO_HINTS
+    std::fill(hinted.begin(), hinted.end(), 0);
+#endif
+
     // ---- per-precision tables (store.h): node records with Tg inline, padded rotations
     std::vector<NodeRec<float>> n32(V); std::vector<NodeRec<double>> n64(V);
     std::vector<float> rot32((size_t)RotStride<float>::value * V, 0.f); std::vector<double> rot64((size_t)RotStride<double>::value * V, 0.0);
@@ -479,7 +532,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         }
         NodeRec<float>& a = n32[i]; NodeRec<double>& b = n64[i];
         a.parent = b.parent = node[i].x;
-        a.info = b.info = node[i].y | (ident ? NODE_IDENTITY : 0);
+        a.info = b.info = node[i].y | (ident ? NODE_IDENTITY : 0) | (hinted[i] ? NODE_HINT : 0);
         a.mat = b.mat = node[i].z;
         a.ndau = b.ndau = kids[i].y;
         a.link = b.link = node[i].w >= 0 ? ~node[i].w : kids[i].x;        // voxelised mother: ~grid id
@@ -559,6 +612,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     Uploader up{geo};
     const int* d_dlist = up.put(dlist);
     { std::vector<int> dfirst(V); for (size_t i = 0; i < V; ++i) dfirst[i] = kids[i].x; geo->v32.dfirst = geo->v64.dfirst = up.put(dfirst); }
+    geo->v32.hint = geo->v64.hint = up.put(hint);
     const int2* d_cells = up.put(cells); const int* d_cand = up.put(cand);
     GeoView<float>& a = geo->v32; GeoView<double>& b = geo->v64;
     a.dlist = b.dlist = d_dlist; a.cells = b.cells = d_cells; a.cand = b.cand = d_cand;

@@ -21,6 +21,10 @@
 //             cell; the axis and the number of cells of the row are in its solid record (cS, sS of a box); wall bits for the
 //             two ends of the row and the sides.  A photon leaving it through one of the two end faces finds its candidate in
 //             the cell beyond that end (nav.cuh: regular_step<.., SLABS>)
+//             flag NODE_HINT (tube sectors on a cylindrical lattice inside a full tube of the same radii -- a segmented
+//             barrel): hint[4 i ..] names the sibling across each z face and phi plane.  A photon that leaves the sector
+//             through one of those faces, farther than 2 probe distances from all its other faces, is in that sibling or in
+//             the mother: relocation tests just that one (nav.cuh: settle_flat), the result is the general search's
 //   rot[i]    M (row-major, global->local rotation), 9 Real padded to 12 (fp32, three 16-byte loads) /
 //             10 (fp64, five 16-byte loads);  p_local = M (x - Tg)
 //   solids, mats, grids: small tables (staged to shared memory by every kernel)
@@ -33,7 +37,7 @@ namespace gn {
 
 enum : int { SOLID_BOX = 0, SOLID_TUBE = 1, SOLID_ORB = 2, SOLID_CONE = 3 };
 enum : int { TUBE_SECTOR = 1, TUBE_HOLE = 2 };
-enum : int { NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SLAB = 1 << 28, NODE_SOLID_MASK = 0xffff, NODE_GRID_SHIFT = 16, NODE_GRID_MASK = 0x3f, NODE_WALL_SHIFT = 22, NODE_WALL_MASK = 0x3f };
+enum : int { NODE_HINT = (int)0x80000000u, NODE_IDENTITY = 1 << 30, NODE_REGULAR = 1 << 29, NODE_SLAB = 1 << 28, NODE_SOLID_MASK = 0xffff, NODE_GRID_SHIFT = 16, NODE_GRID_MASK = 0x3f, NODE_WALL_SHIFT = 22, NODE_WALL_MASK = 0x3f };
 
 template <class R> struct SolidRec {
     R a, b, c;            // BOX: hx hy hz      TUBE: rmin rmax hz      ORB: r - -      CONE: r0 = (r1 + r2)/2, slope m, hz
@@ -71,6 +75,7 @@ template <class R> struct GeoView {
     const R* rot;
     const int* dlist;
     const int* dfirst;    // node -> offset of its daughters in dlist (every node, voxelised or not; the safety scan)
+    const int* hint;      // 4 per node: sibling across the lower / upper z face, the start / end phi plane of a NODE_HINT tube sector
     const SolidRec<R>* solids;
     const MatRec<R>* mats;
     const double* rho;    // density per material [g/cm3] (attenuation-only mode: mu = rho * mu_mass)

@@ -190,6 +190,57 @@ def test_points_in_the_tolerance_band_of_voxel_faces(B):
         assert np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(step.cpu().numpy(), rstep)
 
 
+def test_steps_that_end_near_the_edges_of_barrel_sectors(B):
+    """Sibling hints (store.h NODE_HINT): a photon that leaves a barrel sector through one z or phi face, farther than two
+    probe distances from its other faces, is relocated by testing only the sibling across that face.  Rays are aimed at points
+    on the z faces, the phi planes and the radial surfaces of sectors, at offsets of 0 .. 3 probe distances from a SECOND face
+    (on both sides of the threshold of that rule, and onto edges and corners), so the shortcut and the general search meet;
+    step lengths and volumes entered must be the oracle's bit for bit."""
+    geom = GEOMS["detector"]()                  # 2 barrels x 16 phi x 8 z sectors, r 200-400 and 450-650, hz 1600
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    rng = np.random.default_rng(91)
+    n = 60000
+    dphi, hz_s = 2 * np.pi / 16, 1600.0 / 8
+    for precision in (32, 64):
+        R = np.float64 if precision == 64 else np.float32
+        probe = 1.25 * g.tolerance(precision) / 2 + 4 * 2000.0 * (2.0 ** -23 if precision == 32 else 2.0 ** -52)
+        k = rng.choice([0.0, 0.5, 1.0, 1.9, 2.1, 3.0, 30.0], size=(n, 3)) * rng.choice([-1.0, 1.0], size=(n, 3)) * probe
+        barrel = rng.integers(0, 2, n)
+        rlo, rhi = np.where(barrel == 0, 200.0, 450.0), np.where(barrel == 0, 400.0, 650.0)
+        # target point: on a z face (kind 0), a phi plane (1) or a radial surface (2); the other two coordinates are either
+        # free or sit at an offset k from another face
+        kind = rng.integers(0, 3, n)
+        near2 = rng.random((n, 2)) < 0.6
+        r_face = np.where(rng.random(n) < 0.5, rlo, rhi)
+        z_face = -1600.0 + hz_s * 2 * rng.integers(0, 9, n)
+        phi_face = dphi * (rng.integers(0, 16, n) + 0.5)                  # sector j spans (j - 1/2, j + 1/2) dphi
+        r = np.where(kind == 2, r_face + k[:, 0], np.where(near2[:, 0], r_face + k[:, 0], rng.uniform(rlo + 1, rhi - 1)))
+        z = np.where(kind == 0, z_face + k[:, 1], np.where(near2[:, 1], z_face + k[:, 1], rng.uniform(-1590, 1590, n)))
+        phi = np.where(kind == 1, phi_face + k[:, 2] / r, np.where(np.where(kind == 0, near2[:, 1], near2[:, 0]), phi_face + k[:, 2] / r, rng.uniform(0, 2 * np.pi, n)))
+        target = np.stack([r * np.cos(phi), r * np.sin(phi), z], axis=1)
+        v = unit(rng, n)
+        origin = target - v * rng.uniform(1.0, 30.0, size=(n, 1))
+        p, v = origin.astype(R), v.astype(R)
+        v = (v / np.linalg.norm(v.astype(np.float64), axis=1, keepdims=True)).astype(R)
+        tp, tv = cuda(p), cuda(v)
+        ref = og.locate(p, v, precision)
+        assert np.array_equal(B.nav_locate(g, tp, tv).cpu().numpy(), ref)
+        step, nxt = B.nav_compute_step(g, tp, tv, cuda(ref))
+        rstep, rnxt = og.compute_step(p, v, ref, None, precision)
+        assert np.array_equal(nxt.cpu().numpy(), rnxt) and np.array_equal(step.cpu().numpy(), rstep)
+        # a second query from where the first step ended: points on (or within rounding of) the boundary just reached
+        alive = np.isfinite(rstep) & (rnxt >= 0)
+        p2 = (p[alive] + rstep[alive, None] * v[alive]).astype(R)
+        v2 = v[alive]
+        ref2 = og.locate(p2, v2, precision)
+        assert np.array_equal(B.nav_locate(g, cuda(p2), cuda(v2)).cpu().numpy(), ref2)
+        step2, nxt2 = B.nav_compute_step(g, cuda(p2), cuda(v2), cuda(ref2))
+        rstep2, rnxt2 = og.compute_step(p2, v2, ref2, None, precision)
+        assert np.array_equal(nxt2.cpu().numpy(), rnxt2) and np.array_equal(step2.cpu().numpy(), rstep2)
+        in_sector = np.isin(ref, np.arange(3, geom.n_places))            # world = 0, barrels = 1, 2
+        assert in_sector.mean() > 0.5 and (rnxt[in_sector] >= 3).mean() > 0.3
+
+
 def test_nav_edge_cases(B):
     import torch
     geom = GEOMS["slab"]()
