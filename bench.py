@@ -30,7 +30,7 @@ ALGO_BYTES = {("transport", 32): 96.0, ("transport", 64): 160.0, ("nav", 32): 64
 # workload, measured with the oracle's counting Real (SURVEY 8(d) "instrumented oracle": + - * / sqrt compare = 1, fma = 2,
 # transcendental = 1).  bench.py re-measures it in the cpu_baseline leg; these are the committed values of that measurement
 # (oracle.transport_count_ops on the first 20000 photons / oracle.nav_count_ops on 20000 queries), used with --no-cpu-baseline.
-ALGO_FLOPS = {1: 366.6, 2: 467.4, 3: 606.1, 4: 584.7, 5: 841.9}
+ALGO_FLOPS = {1: 371.4, 2: 469.6, 3: 606.5, 4: 582.4, 5: 841.9}
 PIPE_PEAK_FALLBACK = {32: 74.4, 64: 37.2}   # nominal TFLOP/s (148 SMs x 128 / 64 lanes x 2 x 1.965 GHz) when the self-test cannot run
 
 

@@ -657,7 +657,9 @@ template <class R> EnergyFactors<R> energy_factors(R E) {
     typedef typename Wide<R>::type W;
     W e = W((double)E), k = e / W(kMeC2);
     EnergyFactors<R> f;
-    f.gPE = (R)(double)r_pow<W>(W(0.1) / e, W(3.5));
+    /* (0.1 / E)^3.5 as x x x sqrt(x), x = 0.1 / E (D:reading 1): products, one division and one square root are correctly
+     * rounded by every IEEE-754 implementation, a library pow is not -- host and device libm differ in the last bit */
+    { const W xq = W(0.1) / e; f.gPE = (R)(double)(((xq * xq) * xq) * r_sqrt<W>(xq)); }
     const W two_pi_re2(2.0 * kPi * kRe * kRe);
     f.gKN = (R)(double)((two_pi_re2 * sigma_kn_over_2pire2<W>(k)) / two_pi_re2);      /* sigma_KN(k) / (2 pi r_e^2), as D:reading 1 writes it */
     f.L2k = (R)(double)r_log<W>(W(2.0) * k);

@@ -82,7 +82,8 @@ template <class R> __device__ EnergyFactors<R> energy_factors(R E, int pe_per_de
     const double two_pi_re2 = 2.0 * GN_PI * 2.8179403262e-13 * 2.8179403262e-13;
     EnergyFactors<R> f;
     f.gKN = (R)((two_pi_re2 * (first + second - third)) / two_pi_re2);
-    f.gPE = pe_per_decade > 0 ? pe_coordinate<R>(E, pe_per_decade) : (R)pow(0.1 / (double)E, 3.5);
+    if (pe_per_decade > 0) f.gPE = pe_coordinate<R>(E, pe_per_decade);
+    else { const double xq = __ddiv_rn(0.1, (double)E); f.gPE = (R)__dmul_rn(__dmul_rn(__dmul_rn(xq, xq), xq), __dsqrt_rn(xq)); }      // (0.1 / E)^3.5 = x x x sqrt(x): IEEE operations only (reading 1)
     f.L2k = (R)log(2.0 * k);
     f.above_pair = k > 2.0;
     return f;
