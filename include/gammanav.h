@@ -18,8 +18,8 @@
  * untouched on failure.  gn_last_error() gives a human-readable string for the calling thread's last failure.
  * All nav calls are asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream).  gn_transport_run is
  * host-synchronous: the stream only orders it against earlier work; the call waits for survivor counts while it
- * enqueues its passes, synchronises the stream at the end of every batch (and once more per batch of annihilation
- * photons with gn_opts.secondaries) and returns when the tally and the statistics are complete.
+ * enqueues its passes, synchronises the stream at the end of every batch (with gn_opts.secondaries also before the last pass of a batch
+ * and once per leftover batch of annihilation photons) and returns when the tally and the statistics are complete.
  * Every call runs on the device the geometry was created on; the caller's current device is restored on return.
  */
 #ifndef GAMMANAV_H

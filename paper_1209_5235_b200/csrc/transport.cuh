@@ -21,6 +21,7 @@
 //   * solids, voxel-grid headers and material factors are staged in shared memory; node records and voxel
 //     cells stay in L2.
 #pragma once
+#include <vector>
 #include "common.cuh"
 #include "impl.h"
 #include "physics.cuh"
@@ -109,19 +110,33 @@ template <class R> __device__ __forceinline__ void store_rec(PhotonRec<R>* q, un
 struct PerPhotonOut { uint64_t* hash; uint32_t* nsteps; double* efinal; };
 
 // Secondary photons (reading 16).  A pair event of a primary appends its vertex to a list
-// (out / n_out); when the batch of primaries is done, the list is the source of a batch of 2 x n_pairs annihilation
-// photons (in): photon k belongs to pair k >> 1, runs on Philox stream tag 1 + (k & 1) of its parent's id, and adds its
-// history hash and step count to the parent's (sums: the order in which they finish does not matter).
+// (out / n_out).  Annihilation photon k (k = 0, 1, ... over the whole list) belongs to pair k >> 1, runs on Philox stream
+// tag 1 + (k & 1) of its parent's id, and adds its history hash and step count to the parent's (sums: the order in which
+// they finish does not matter).  It travels through the same queues and kernels as the primaries -- a source pass with
+// birth = 1 appends photons 2 birth_first ... to the queue of the pass that comes next -- and is told apart by SEC_BIT of
+// its photon index: idx = SEC_BIT | k.
+constexpr uint32_t SEC_BIT = 0x80000000u;
 template <class R> struct alignas(16) PairVtx { R x, y, z; uint32_t idx; };
 template <class R> struct SecIO {
-    PairVtx<R>* out; unsigned* n_out;                          // primaries: where pair vertices go (nullptr = secondaries off)
-    const PairVtx<R>* in;                                      // secondaries: their parents' vertices (nullptr = a batch of primaries)
-    unsigned long long* parent_hash; uint32_t* parent_nsteps;  // secondaries, per-photon outputs wanted: the parents' slots
+    PairVtx<R>* out; unsigned* n_out;                          // where pair vertices go (nullptr = secondaries off)
+    const PairVtx<R>* in;                                      // the list again, for the photons with SEC_BIT: their parents' vertices
+    unsigned long long* parent_hash; uint32_t* parent_nsteps;  // per-photon outputs wanted: the parents' slots
+    unsigned long long* state_hash;                            // hash state of annihilation photon k between passes (tracked runs)
+    uint32_t birth_first; int birth;                           // source pass: birth = 1 -> it births photons 2 birth_first + i
 };
+template <class R> __host__ __device__ inline SecIO<R> no_secondaries() { SecIO<R> o; o.out = nullptr; o.n_out = nullptr; o.in = nullptr; o.parent_hash = nullptr; o.parent_nsteps = nullptr; o.state_hash = nullptr; o.birth_first = 0; o.birth = 0; return o; }
+// id and Philox stream tag of photon idx; its hash state between passes
+template <class R> __device__ __forceinline__ uint64_t photon_id(const SecIO<R>& sec, uint64_t first_id, uint32_t idx) {
+    return first_id + ((idx & SEC_BIT) ? sec.in[(idx & ~SEC_BIT) >> 1].idx : idx);
+}
+__device__ __forceinline__ uint32_t photon_tag(uint32_t idx) { return (idx & SEC_BIT) ? 1u + (idx & 1u) : 0u; }
+template <class R> __device__ __forceinline__ unsigned long long& hash_state(const PerPhotonOut& pp, const SecIO<R>& sec, uint32_t idx) {
+    return (idx & SEC_BIT) ? sec.state_hash[idx & ~SEC_BIT] : *reinterpret_cast<unsigned long long*>(&pp.hash[idx]);
+}
 // per-photon outputs at the end of a history
 template <class R> __device__ __forceinline__ void history_out(const PerPhotonOut& pp, const SecIO<R>& sec, uint32_t idx, uint64_t h, uint32_t ns, R E) {
-    if (sec.in) {
-        const uint32_t parent = sec.in[idx >> 1].idx;
+    if (idx & SEC_BIT) {
+        const uint32_t parent = sec.in[(idx & ~SEC_BIT) >> 1].idx;
         if (sec.parent_hash) atomicAdd(&sec.parent_hash[parent], (unsigned long long)h);
         if (sec.parent_nsteps) atomicAdd(&sec.parent_nsteps[parent], ns);
     } else {
@@ -300,13 +315,12 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
     if (FROM_SOURCE) {
         unsigned c_phot = 0; double e_src = 0.0;
         if (fate == FATE_ALIVE) {
-            idx = i;
             BirthIO<R> b;
-            if (sec.in) birth_secondary(&b, sec.in, i, g.pe_per_decade, seed, first_id);
-            else birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, g.pe_per_decade, seed, first_id + i);
+            if (sec.birth) { idx = SEC_BIT | (2u * sec.birth_first + i); birth_secondary(&b, sec.in, idx & ~SEC_BIT, g.pe_per_decade, seed, first_id); }
+            else { idx = i; birth(&b, &sh_src, sh_src.energy_kind == 0 ? &sh_mono : nullptr, g.pe_per_decade, seed, first_id + i); }
             x.x = b.x; x.y = b.y; x.z = b.z; w.x = b.wx; w.y = b.wy; w.z = b.wz; E = b.E; Y = b.Y;
             gPE = b.gPE; gKN = b.gKN; L2k = b.L2k; above = b.above; ctr = b.j;
-            if (!sec.in) { c_phot = 1; e_src = (double)E; }               // annihilation photons are not source photons
+            if (!sec.birth) { c_phot = 1; e_src = (double)E; }            // annihilation photons are not source photons
             vol = nav.locate(x, w, nd);
             if (vol < 0) {
                 fate = FATE_ESCAPED;
@@ -324,7 +338,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         x.x = r.x; x.y = r.y; x.z = r.z; w.x = r.wx; w.y = r.wy; w.z = r.wz; E = r.E; Y = r.Y;
         gPE = r.gPE; gKN = r.gKN; L2k = r.L2k; above = (int)(r.tail[0] & 1u); pending = (r.tail[0] & 2u) != 0;
         idx = r.idx; misc = r.misc; ctr = r.ctr; vol = r.vol;
-        if (fate == FATE_ALIVE) { nd = nav.node(vol); if (TRACK) h = pp.hash[idx]; }
+        if (fate == FATE_ALIVE) { nd = nav.node(vol); if (TRACK) h = hash_state(pp, sec, idx); }
     }
 
     // A lane whose photon reaches its interaction point parks there (pending) instead of running the rare, long
@@ -378,7 +392,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
                 const MuParts<R> mp = photon_mu(g, mats[nd.mat], nd.mat, E, gPE, gKN, L2k, above);
                 InteractIO<R> io;
                 io.E = E; io.wx = w.x; io.wy = w.y; io.wz = w.z; io.Y = Y; io.gPE = gPE; io.gKN = gKN; io.L2k = L2k; io.j = ctr; io.above = above;
-                interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, first_id + (sec.in ? sec.in[idx >> 1].idx : idx), sec.in ? 1u + (idx & 1u) : 0u, sec.out != nullptr);
+                interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, photon_id(sec, first_id, idx), photon_tag(idx), sec.out != nullptr);
                 const int ev = io.ev; ctr = io.j;
                 if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = x.x; pv.y = x.y; pv.z = x.z; pv.idx = idx; sec.out[atomicAdd(sec.n_out, 1u)] = pv; }
                 dep_d = (double)io.dep;
@@ -471,7 +485,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         r.tail[0] = (uint32_t)above | (pending ? 2u : 0u);
         GN_CHECK(o < cap && vol >= 0 && vol < g.n_nodes, CHK_STORE_SLOT);
         store_rec(qout, o, r);
-        if (TRACK) pp.hash[idx] = h;
+        if (TRACK) hash_state(pp, sec, idx) = h;
         if (FLAT && sio.keys_out && !key1) {                                 // volume key of a travelling survivor
             const int key = 2 * nav.solid_of(nd).type + (nd.ndau > 0 ? 1 : 0);
             sio.keys_out[o] = (uint8_t)key;
@@ -541,7 +555,7 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         const MuParts<R> mp = photon_mu(g, g.mats[mat], mat, r.E, r.gPE, r.gKN, r.L2k, above);
         InteractIO<R> io;
         io.E = r.E; io.wx = r.wx; io.wy = r.wy; io.wz = r.wz; io.Y = r.Y; io.gPE = r.gPE; io.gKN = r.gKN; io.L2k = r.L2k; io.j = r.ctr; io.above = above;
-        interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, first_id + (sec.in ? sec.in[r.idx >> 1].idx : r.idx), sec.in ? 1u + (r.idx & 1u) : 0u, sec.out != nullptr);
+        interact(&io, mp.pe, mp.c, mp.r, mp.p, mp.tot, g.e_cut, g.pe_per_decade, seed, photon_id(sec, first_id, r.idx), photon_tag(r.idx), sec.out != nullptr);
         int ev = io.ev;
         if (ev == EV_PAIR && sec.out) { PairVtx<R> pv; pv.x = r.x; pv.y = r.y; pv.z = r.z; pv.idx = r.idx; const unsigned ps = atomicAdd(sec.n_out, 1u); GN_CHECK(ps < cap, CHK_PAIR_SLOT); sec.out[ps] = pv; }
         dep_d = (double)io.dep;
@@ -559,9 +573,9 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
             atomicAdd(&sh_cnt[ST_STUCK], 1ull); atomicAdd(&sh_en[EN_STUCK], (double)r.E);
         }
         if (TRACK) {
-            uint64_t h = pp.hash[r.idx];
+            uint64_t h = hash_state(pp, sec, r.idx);
             fnv_word(h, (uint32_t)vol); fnv_word(h, (uint32_t)ev);
-            if (alive) pp.hash[r.idx] = h;
+            if (alive) hash_state(pp, sec, r.idx) = h;
             else history_out(pp, sec, r.idx, h, r.misc >> 8, r.E);
         }
         if (alive) r.tail[0] &= 1u; else r.vol = -1;
@@ -609,7 +623,7 @@ transport_refill(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_i
     __syncthreads();
     Navigator<R, true, FLAT> nav(g, &tab.ctx);
     const int lane = threadIdx.x & 31;
-    const SecIO<R> nosec{nullptr, nullptr, nullptr, nullptr, nullptr};
+    const SecIO<R> nosec = no_secondaries<R>();
 
     bool alive = false, exhausted = false, pending = false;      // pending: parked at its interaction point
     V3<R> x{0, 0, 0}, w{0, 0, 1}; R E = 1, Y = 0, gPE = 0, gKN = 0, L2k = 0;
@@ -762,7 +776,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
     const size_t kb = sorted ? sizeof(KeyCounters) * (TR_MAX_PASSES + 2) : 0;
     const size_t sb = sorted ? ((cap + 255) & ~(size_t)255) + 4 * cap : 0;      // keys + perm
     const size_t pb = secondaries ? cap * sizeof(PairVtx<R>) + 16 : 0;          // pair vertices of a batch + their count
-    const size_t hb2 = (secondaries && track) ? cap * 8 : 0;                    // hash state of a batch of annihilation photons
+    const size_t hb2 = (secondaries && track) ? 2 * cap * 8 : 0;                // hash state of the annihilation photons (two per pair vertex)
     const size_t base = (2 * qb + hb + 512 + cb + kb + sb + 15) & ~(size_t)15;
     bool voxel_sched = false;
     if constexpr (!FLAT) voxel_sched = geo->voxel_sched;
@@ -776,7 +790,8 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
         if (e != cudaSuccess) { cudaGetLastError(); geo->ws_scratch = nullptr; return fail(GN_OUT_OF_MEMORY, std::string("gn_transport_run scratch: ") + cudaGetErrorString(e)); }
         geo->ws_bytes = need;
     }
-    if (!geo->ws_pinned && cudaMallocHost(&geo->ws_pinned, cb) != cudaSuccess) { cudaGetLastError(); geo->ws_pinned = nullptr; return fail(GN_OUT_OF_MEMORY, "gn_transport_run: pinned alloc"); }
+    const size_t npb = sizeof(unsigned) * (TR_MAX_PASSES + 2);     // pinned: the pair count seen after every pass
+    if (!geo->ws_pinned && cudaMallocHost(&geo->ws_pinned, cb + npb) != cudaSuccess) { cudaGetLastError(); geo->ws_pinned = nullptr; return fail(GN_OUT_OF_MEMORY, "gn_transport_run: pinned alloc"); }
     if (!geo->ws_events_ok) {
         bool ok = cudaEventCreate(&geo->ws_events[0]) == cudaSuccess && cudaEventCreate(&geo->ws_events[1]) == cudaSuccess;
         for (int q = 0; q <= TR_LAG; ++q) ok = ok && cudaEventCreateWithFlags(&geo->ws_events[2 + q], cudaEventDisableTiming) == cudaSuccess;
@@ -790,6 +805,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
     DevStats* d_stats = (DevStats*)(scratch + 2 * qb + hb);
     PassCounters* d_ctr = (PassCounters*)(scratch + 2 * qb + hb + 512);
     PassCounters* h_ctr = (PassCounters*)geo->ws_pinned;
+    unsigned* h_np = (unsigned*)((char*)geo->ws_pinned + cb);
     KeyCounters* d_kctr = sorted ? (KeyCounters*)(scratch + 2 * qb + hb + 512 + cb) : nullptr;
     uint8_t* d_keys = sorted ? (uint8_t*)(scratch + 2 * qb + hb + 512 + cb + kb) : nullptr;
     uint32_t* d_perm = sorted ? (uint32_t*)(scratch + 2 * qb + hb + 512 + cb + kb + ((cap + 255) & ~(size_t)255)) : nullptr;
@@ -810,9 +826,15 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
     const GeoView<R>& g = view<R>(geo);
     // one batch of photons through the wavefront: n0 photons born in pass 0 (from the source, or -- sec.in -- at their
     // parents' pair vertices), passes until none is left; ends with a stream synchronise
+    // `sec.birth`: a batch of annihilation photons (pair vertices sec.birth_first ...); otherwise a batch of primaries, into
+    // whose queue the annihilation photons of the pair events seen so far are injected between passes (`injected` counts the
+    // pair vertices used up): they then ride the primaries' passes and share their tail instead of paying their own.
+    unsigned injected = 0;
     auto run_batch = [&](uint32_t n0, uint64_t fid, PerPhotonOut pp, SecIO<R> sec) {
         PhotonRec<R>* in = qb_; PhotonRec<R>* out = qa;
-        const int k_first = sec.in ? K : K0;                      // annihilation photons are born inside the detector: no short first pass
+        const bool sec_batch = sec.birth != 0;
+        const bool inject = secondaries && !sec_batch;
+        const int k_first = sec_batch ? K : K0;                   // annihilation photons are born inside the detector: no short first pass
         cudaMemsetAsync(d_ctr, 0, cb, s);
         if (sorted) cudaMemsetAsync(d_kctr, 0, kb, s);
         cudaEventRecord(ev0, s);
@@ -821,11 +843,42 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
         unsigned ub = n0;
         bool finished = false;
         int n_timed = 0;
+        std::vector<unsigned> inj(inject ? TR_MAX_PASSES + 2 : 0, 0u);       // photons injected into the input queue of pass p
         for (int p = 0; !finished; ++p) {
             if (p > TR_LAG) {
                 e = cudaEventSynchronize(ring[(p - TR_LAG) % (TR_LAG + 1)]);
                 if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pass"); break; }
                 ub = h_ctr[p - TR_LAG].front + h_ctr[p - TR_LAG].back + h_ctr[p - TR_LAG].slow;      // input count of pass p - TR_LAG >= that of pass p
+                if (inject) for (int q = p - TR_LAG; q < p; ++q) ub += inj[q];     // ... plus what was injected since (the copy of counter q predates the injection at q)
+                if (ub == 0) break;
+            }
+            if (inject && p > TR_LAG) {
+                // annihilation photons of the pair vertices recorded so far join the input queue of this pass
+                unsigned seen = h_np[p - TR_LAG];                                   // as the counters: TR_LAG passes old
+                if (ub <= tail || p == TR_MAX_PASSES - 1) {                         // about to run to completion: the exact figures
+                    PassCounters now{};
+                    e = cudaMemcpyAsync(&now, d_ctr + p, sizeof now, cudaMemcpyDeviceToHost, s);
+                    if (e == cudaSuccess) e = cudaMemcpyAsync(&seen, d_npairs, sizeof seen, cudaMemcpyDeviceToHost, s);
+                    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+                    if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pair count"); break; }
+                    ub = now.front + now.back + now.slow;
+                }
+                unsigned avail = seen > injected ? seen - injected : 0u;
+                const bool ending = ub <= tail || p == TR_MAX_PASSES - 1;
+                avail = (unsigned)std::min<uint64_t>(avail, ((uint64_t)cap - std::min<uint64_t>(cap, ub)) / 2);      // as many as the queue has room for
+                if (avail > 0 && (avail >= std::max(256u, ub >> 7) || ending)) {       // enough of them to be worth a source-pass launch of their own
+                    SecIO<R> bs = sec; bs.birth = 1; bs.birth_first = injected;
+                    const unsigned nb = 2u * avail;
+                    launch_pass<R, true, false, FLAT>(track, (nb + TR_THREADS - 1) / TR_THREADS, s, g, src, seed, fid, nb, nullptr, d_ctr + p, nullptr, in, (uint32_t)cap, d_edep, d_stats, pp,
+                                                      K, regroup, bs, sorted ? SortIO{d_kctr + p, d_keys, nullptr} : SortIO{nullptr, nullptr, nullptr});
+                    ++launches;
+                    if (sorted) {                                                    // the work order of this pass again, with the newcomers
+                        cudaMemsetAsync(d_kctr[p].cur, 0, sizeof d_kctr[p].cur, s);
+                        sort_scatter_kernel<<<nav_grid(((int64_t)ub + nb + 3) / 4), NAV_THREADS, 0, s>>>(d_keys, 0, d_kctr[p].tot, d_kctr[p].cur, d_perm, &d_ctr[p].front);
+                        ++launches;
+                    }
+                    ub += nb; injected += avail; inj[p] = nb;
+                }
                 if (ub == 0) break;
             }
             const bool last = p > 0 && (ub <= tail || p == TR_MAX_PASSES - 1);
@@ -876,6 +929,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             e = cudaGetLastError();
             if (e == cudaSuccess && !last) {
                 e = cudaMemcpyAsync(&h_ctr[p + 1], d_ctr + p + 1, sizeof(PassCounters), cudaMemcpyDeviceToHost, s);
+                if (e == cudaSuccess && inject) e = cudaMemcpyAsync(&h_np[p + 1], d_npairs, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
                 if (e == cudaSuccess) e = cudaEventRecord(ring[(p + 1) % (TR_LAG + 1)], s);
             }
             if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pass"); break; }
@@ -911,18 +965,25 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             continue;
         }
         if (secondaries) cudaMemsetAsync(d_npairs, 0, sizeof(unsigned), s);
-        run_batch(n0, fid, pp, SecIO<R>{d_pairs, d_npairs, nullptr, nullptr, nullptr});
+        SecIO<R> sec = no_secondaries<R>();
+        if (secondaries) {
+            sec.out = d_pairs; sec.n_out = d_npairs; sec.in = d_pairs; sec.state_hash = (unsigned long long*)sec_hash;
+            sec.parent_hash = d_hash ? (unsigned long long*)(d_hash + done) : nullptr; sec.parent_nsteps = d_nsteps ? d_nsteps + done : nullptr;
+        }
+        injected = 0;
+        run_batch(n0, fid, pp, sec);
         if (!secondaries || rc != GN_OK) continue;
-        // the annihilation photons of this batch's pair events, at most cap at a time (511 keV: they cannot pair again)
+        // the annihilation photons of the pair vertices that were not injected (pair events of the tail pass, or no room in the
+        // queue), at most cap at a time (511 keV: they cannot pair again)
         unsigned n_pairs = 0;
         e = cudaMemcpyAsync(&n_pairs, d_npairs, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) { rc = cuda_fail(e, "gn_transport_run pair count"); break; }
         const unsigned chunk = (unsigned)(cap / 2);
-        for (unsigned off = 0; off < n_pairs && rc == GN_OK; off += chunk) {
+        for (unsigned off = injected; off < n_pairs && rc == GN_OK; off += chunk) {
             const unsigned np = std::min(chunk, n_pairs - off);
-            run_batch(2u * np, fid, PerPhotonOut{sec_hash, nullptr, nullptr},
-                      SecIO<R>{nullptr, nullptr, d_pairs + off, d_hash ? (unsigned long long*)(d_hash + done) : nullptr, d_nsteps ? d_nsteps + done : nullptr});
+            SecIO<R> bs = sec; bs.birth = 1; bs.birth_first = off;
+            run_batch(2u * np, fid, pp, bs);
         }
     }
     if (rc == GN_OK) {

@@ -75,7 +75,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
             lane_direction(w, g.delta, vl);
             lane_solid(solids, nd.info, vl);
             if (!(nd.info & (NODE_REGULAR | (SLABS ? NODE_SLAB : 0))) || !vl.ok) needgen = true;
-            if (TRACK && !pending && !needgen) h = pp.hash[idx];
+            if (TRACK && !pending && !needgen) h = hash_state(pp, sec, idx);
         }
     }
     int act0 = 32;
@@ -141,7 +141,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
         GN_CHECK(key2 || (key1 ? sh_base[1] + sh_wcount[1][warp] + __popc(bal1 & below) : sh_base[0] + sh_wcount[0][warp] + __popc(bal0 & below)) < cap, CHK_STORE_SLOT);
         if (key2) store_rec(S, sh_base[2] + sh_wcount[2][warp] + __popc(bal2 & below), r);
         else store_rec(qout, key1 ? cap - 1u - (sh_base[1] + sh_wcount[1][warp] + __popc(bal1 & below)) : sh_base[0] + sh_wcount[0][warp] + __popc(bal0 & below), r);
-        if (TRACK && c_steps) pp.hash[idx] = h;
+        if (TRACK && c_steps) hash_state(pp, sec, idx) = h;
     }
     {
         const unsigned s = warp_sum(c_steps);
@@ -198,7 +198,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
         const int above = (int)(r.tail[0] & REC_ABOVE);
         int vol = r.vol;
         uint64_t h = 0;
-        if (TRACK) h = pp.hash[r.idx];
+        if (TRACK) h = hash_state(pp, sec, r.idx);
         NodeRec<R> nd = nav.node(vol);
         const bool cacheable = direction_cacheable(w, g.delta);
         for (int it = 0; it < SLOW_STEPS; ++it) {
@@ -222,7 +222,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
             if (TRACK) { fnv_word(h, (uint32_t)vol_before); fnv_word(h, (uint32_t)ev); if (!alive) history_out(pp, sec, r.idx, h, misc >> 8, r.E); }
             if (!alive || ((nd.info & (NODE_REGULAR | NODE_SLAB)) && cacheable)) break;  // gone, or voxel_pass takes over
         }
-        if (TRACK && alive) pp.hash[r.idx] = h;
+        if (TRACK && alive) hash_state(pp, sec, r.idx) = h;
         r.x = x.x; r.y = x.y; r.z = x.z; r.Y = Y; r.misc = misc; r.vol = vol;
         r.tail[0] = (uint32_t)above | (pending ? REC_PENDING : 0u);
     }
