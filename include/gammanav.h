@@ -59,7 +59,7 @@ typedef struct {
     int32_t first_pass_steps;  /* K0: steps in the pass that also generates the photons (sheds photons that miss early); default 1 */
     int32_t tail_photons;      /* once at most this many photons are left, one last pass runs them to completion; default 148 * 1024 */
     int32_t regroup_percent;   /* a warp ends its pass early once fewer than this % of the lanes it started with still travel
-                                  (the compaction then refills it); default 50 for box-only unrotated geometries, else 75 */
+                                  (the compaction then refills it); default 35 for box-only unrotated geometries, else 90 */
     int32_t secondaries;       /* 1: a pair event deposits E - 2 me c^2 locally and its two back-to-back annihilation photons
                                   (me c^2 each, isotropic axis, Philox stream tags 1 / 2 of the parent's id) are transported
                                   from the vertex; their steps, events, hashes and step counts are added to

@@ -606,7 +606,7 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         for (size_t i = 0; i < V; ++i) { n_regular += (n32[i].info & (NODE_REGULAR | NODE_SLAB)) ? 1 : 0; has_slabs = has_slabs || (n32[i].info & NODE_SLAB); }
         geo->has_slabs = has_slabs;
         geo->voxel_sched = coherent && 2 * n_regular >= V && geo->opts.no_voxel_pass <= 0 && geo->opts.rayleigh <= 0 && geo->opts.pe_table_per_decade <= 0 && n_solids <= 32 && n_mats <= 32 && grids.size() <= 8 && ext < 0x1p50;      // table sizes: MAX_SMEM_* of common.cuh
-        if (regroup_default) geo->opts.regroup_percent = coherent ? 50 : 75;
+        if (regroup_default) geo->opts.regroup_percent = coherent ? 35 : 90;      // swept on configs 2-4 (round 2): 15-50 / 85-95 within 1 %
         if (steps_default && geo->voxel_sched) geo->opts.steps_per_pass = 24;      // the regular-voxel pass is cheap per step: fewer, longer passes (measured)
     }
     Uploader up{geo};
