@@ -273,6 +273,19 @@ int gn_selftest_pipe_peak(int precision, double h_out[4]);
  *   gn_geometry_create
  */
 int gn_host_source_frame(const gn_source* h_src, int precision, double frame_out[9]);
+/*
+ *   gn_host_voxel_tables: the host tables gn_geometry_create would upload for this geometry (same arguments, same code, no
+ *   device touched): counts = {voxel grids, voxel cells, candidate references}; per node its info word (solid index in bits
+ *   0-15; bit 30 identity rotation, 29 regular voxel, 28 regular slab, 31 sibling hints) and link (first daughter / ~grid id
+ *   of a voxelised mother / cell index of a regular voxel or slab); h_hint 4 per node (sibling across the lower / upper z face,
+ *   the start / end phi plane; -1 none); h_grids 11 doubles per grid (mother node, gmin[3], cell width[3], cells[3], first
+ *   cell); h_cell_start (cells + 1 offsets into h_cand) and h_cand (candidate daughters of every cell, ascending).  Any
+ *   output pointer but counts may be NULL; call once for the counts, then with arrays of those sizes.
+ */
+int gn_host_voxel_tables(const double* h_materials, int32_t n_mats, const int32_t* h_solid_type, const double* h_solid_params,
+                         int32_t n_solids, const int32_t* h_placements, int32_t n_places, const double* h_transforms,
+                         int32_t n_transforms, const gn_opts* h_opts, int64_t counts[3], int32_t* h_node_info,
+                         int32_t* h_node_link, int32_t* h_hint, double* h_grids, int32_t* h_cell_start, int32_t* h_cand);
 int gn_host_compose_transforms(const int32_t* h_placements, int32_t n_places, const double* h_transforms, int32_t n_transforms,
                                double* h_M_out, double* h_T_out);
 

@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = ("gn_geometry_create", "gn_geometry_destroy", "gn_geometry_num_places", "gn_geometry_tolerance",
            "gn_geometry_voxel_info", "gn_nav_locate", "gn_nav_compute_step", "gn_nav_compute_step_noalloc", "gn_nav_compute_step_normal", "gn_nav_compute_safety", "gn_transport_run", "gn_nav_query_host",
            "gn_transport_run_host", "gn_free_path_run", "gn_free_path_run_host", "gn_selftest_arith", "gn_selftest_pipe_peak",
-           "gn_host_source_frame", "gn_host_compose_transforms", "gn_last_error", "gn_version")
+           "gn_host_source_frame", "gn_host_compose_transforms", "gn_host_voxel_tables", "gn_last_error", "gn_version")
 
 
 class GammaNavError(RuntimeError):
@@ -78,6 +78,8 @@ def lib():
         L.gn_selftest_pipe_peak.argtypes = [C.c_int, C.c_void_p]
         L.gn_host_source_frame.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.gn_host_compose_transforms.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.gn_host_voxel_tables.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
+                                           C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_free_path_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p]
         L.gn_free_path_run.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         L.gn_transport_run_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
@@ -352,3 +354,25 @@ def host_compose_transforms(geom):
     _check(lib().gn_host_compose_transforms(pl.ctypes.data_as(C.c_void_p), C.c_int32(pl.shape[0]), tr.ctypes.data_as(C.c_void_p), C.c_int32(tr.shape[0]),
                                             M.ctypes.data_as(C.c_void_p), T.ctypes.data_as(C.c_void_p)), "gn_host_compose_transforms")
     return M, T
+
+
+def host_voxel_tables(geom, **opts):
+    """gn_host_voxel_tables: the voxel grids, candidate lists, node flags and sibling hints gn_geometry_create builds for `geom`,
+    as numpy arrays (host only, no device needed)."""
+    L = lib()
+    mats = _np(geom.materials, np.float64); st = _np(geom.solid_type, np.int32); sp = _np(geom.solid_params, np.float64)
+    pl = _np(geom.placements, np.int32); tr = _np(geom.transforms, np.float64)
+    o = Opts(**opts) if opts else None
+    counts = (C.c_int64 * 3)()
+
+    def call(info, link, hint, grids, cell_start, cand):
+        p = lambda a: a.ctypes.data_as(C.c_void_p) if a is not None else None
+        _check(L.gn_host_voxel_tables(p(mats), C.c_int32(mats.shape[0]), p(st), p(sp), C.c_int32(st.shape[0]), p(pl), C.c_int32(pl.shape[0]),
+                                      p(tr), C.c_int32(tr.shape[0]), C.byref(o) if o else None, counts, p(info), p(link), p(hint), p(grids),
+                                      p(cell_start), p(cand)), "gn_host_voxel_tables")
+    call(None, None, None, None, None, None)
+    V, ng, nc, nk = pl.shape[0], counts[0], counts[1], counts[2]
+    info = np.empty(V, np.int32); link = np.empty(V, np.int32); hint = np.empty((V, 4), np.int32)
+    grids = np.empty((max(ng, 1), 11), np.float64); cell_start = np.empty(nc + 1, np.int32); cand = np.empty(max(nk, 1), np.int32)
+    call(info, link, hint, grids, cell_start, cand)
+    return {"info": info, "link": link, "hint": hint, "grids": grids[:ng], "cell_start": cell_start, "cand": cand[:nk]}

@@ -25,9 +25,9 @@ const double kPi = 3.14159265358979323846;
 struct HostSolid { int type; double a, b, c, sphi, dphi; bool sector; double cS, sS, cE, sE; double rbound; };
 
 struct Uploader {
-    gn_geometry* geo; bool ok = true; std::string err;
+    gn_geometry* geo; bool dry = false; bool ok = true; std::string err;
     template <class T> const T* put(const std::vector<T>& v) {
-        if (!ok) return nullptr;
+        if (!ok || dry) return nullptr;
         void* d = nullptr;
         size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(T);
         cudaError_t e = cudaMalloc(&d, bytes);
@@ -187,6 +187,14 @@ int parse_solid(int type, const double* q, HostSolid& out, const char** why) {
 
 struct HostGrid { int n[3]; double gmin[3], w[3]; int cell_base; int mother; };
 
+// gn_host_voxel_tables: the host tables of a geometry (voxel grids, candidate lists, node flags, sibling hints) as
+// gn_geometry_create builds them, kept instead of uploaded -- the same code path with every CUDA call left out
+struct HostTables {
+    std::vector<int> info, link, hint, cell_start, cand;
+    std::vector<HostGrid> grids;
+};
+static thread_local HostTables* g_dry = nullptr;
+
 }  // namespace
 }  // namespace gn
 
@@ -201,8 +209,9 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
     if (n_mats <= 0 || n_solids <= 0 || n_places <= 0 || n_transforms <= 0)
         return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: empty table");
     if (n_solids > NODE_SOLID_MASK + 1) return fail(GN_INVALID_ARGUMENT, "gn_geometry_create: at most 65536 solids (the node record keeps 16 bits for the solid index)");
+    const bool dry = g_dry != nullptr;                             // host tables only (gn_host_voxel_tables): no device is touched
     int dev_count = 0;
-    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) {
+    if (!dry && (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)) {
         cudaGetLastError();
         return fail(GN_CUDA_ERROR, "gn_geometry_create: no CUDA device (this library has no CPU fallback)");
     }
@@ -245,8 +254,8 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
 
     gn_geometry* geo = new gn_geometry();
     geo->n_places = n_places; geo->n_solids = n_solids; geo->n_mats = n_mats;
-    cudaGetDevice(&geo->device);
-    {   // stream-ordered scratch of the query sort: a pool of the handle's own that keeps freed blocks (the device's default
+    if (!dry) cudaGetDevice(&geo->device);
+    if (!dry) {   // stream-ordered scratch of the query sort: a pool of the handle's own that keeps freed blocks (the device's default
         // pool and its release threshold are the application's, not this library's)
         cudaMemPoolProps props{};
         props.allocType = cudaMemAllocationTypePinned; props.handleTypes = cudaMemHandleTypeNone;
@@ -609,6 +618,14 @@ extern "C" int gn_geometry_create(const double* h_materials, int32_t n_mats, con
         if (regroup_default) geo->opts.regroup_percent = coherent ? 35 : 90;      // swept on configs 2-4 (round 2): 15-50 / 85-95 within 1 %
         if (steps_default && geo->voxel_sched) geo->opts.steps_per_pass = 24;      // the regular-voxel pass is cheap per step: fewer, longer passes (measured)
     }
+    if (dry) {
+        g_dry->info.resize(V); g_dry->link.resize(V);
+        for (size_t i = 0; i < V; ++i) { g_dry->info[i] = n32[i].info; g_dry->link[i] = n32[i].link; }
+        g_dry->hint = hint; g_dry->cell_start = cell_start; g_dry->cand = cand; g_dry->grids = grids;
+        delete geo;
+        *out = nullptr;
+        return GN_OK;
+    }
     Uploader up{geo};
     const int* d_dlist = up.put(dlist);
     { std::vector<int> dfirst(V); for (size_t i = 0; i < V; ++i) dfirst[i] = kids[i].x; geo->v32.dfirst = geo->v64.dfirst = up.put(dfirst); }
@@ -689,6 +706,35 @@ extern "C" int gn_geometry_voxel_info(const gn_geometry* geo, int64_t info[4]) {
 namespace gn { const char* last_error_cstr(); }
 extern "C" const char* gn_last_error(void) { return gn::last_error_cstr(); }
 extern "C" const char* gn_version(void) { return "gammanav 0.1 (sm_100a)"; }
+
+// host-only hook (no device needed): the voxel grids, candidate lists, node flags and sibling hints of a geometry, exactly as
+// gn_geometry_create builds them, for tests that check them against brute force
+extern "C" int gn_host_voxel_tables(const double* h_materials, int32_t n_mats, const int32_t* h_solid_type, const double* h_solid_params,
+                                    int32_t n_solids, const int32_t* h_placements, int32_t n_places, const double* h_transforms,
+                                    int32_t n_transforms, const gn_opts* h_opts, int64_t counts[3], int32_t* h_node_info,
+                                    int32_t* h_node_link, int32_t* h_hint, double* h_grids, int32_t* h_cell_start, int32_t* h_cand) {
+    if (!counts) return fail(GN_INVALID_ARGUMENT, "gn_host_voxel_tables: NULL counts");
+    HostTables t;
+    g_dry = &t;
+    gn_geometry* none = nullptr;
+    const int rc = gn_geometry_create(h_materials, n_mats, h_solid_type, h_solid_params, n_solids, h_placements, n_places, h_transforms,
+                                      n_transforms, h_opts, &none);
+    g_dry = nullptr;
+    if (rc != GN_OK) return rc;
+    counts[0] = (int64_t)t.grids.size(); counts[1] = (int64_t)t.cell_start.size() - 1; counts[2] = (int64_t)t.cand.size();
+    if (h_node_info) std::copy(t.info.begin(), t.info.end(), h_node_info);
+    if (h_node_link) std::copy(t.link.begin(), t.link.end(), h_node_link);
+    if (h_hint) std::copy(t.hint.begin(), t.hint.end(), h_hint);
+    if (h_grids) for (size_t i = 0; i < t.grids.size(); ++i) {
+        const HostGrid& G = t.grids[i];
+        double* o = h_grids + 11 * i;
+        o[0] = G.mother; for (int k = 0; k < 3; ++k) { o[1 + k] = G.gmin[k]; o[4 + k] = G.w[k]; o[7 + k] = G.n[k]; }
+        o[10] = G.cell_base;
+    }
+    if (h_cell_start) std::copy(t.cell_start.begin(), t.cell_start.end(), h_cell_start);
+    if (h_cand) std::copy(t.cand.begin(), t.cand.end(), h_cand);
+    return GN_OK;
+}
 
 // host-only hook (no device needed): the composed global -> local transforms the store would hold, M = R_global^T (row-major)
 // and T_global per node, for tests that compare them with an independent composition
