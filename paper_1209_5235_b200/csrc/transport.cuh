@@ -531,8 +531,11 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 #ifndef INTERACT_MIN_BLOCKS
 #define INTERACT_MIN_BLOCKS 6      // 80 registers, 24 warps / SM (1 block: 82 registers -- the same code, but the occupancy is then promised)
 #endif
+#ifndef INTERACT_MIN_BLOCKS_F64
+#define INTERACT_MIN_BLOCKS_F64 3
+#endif
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS, sizeof(R) == 4 ? INTERACT_MIN_BLOCKS : (INTERACT_MIN_BLOCKS + 1) / 2)
+__global__ void __launch_bounds__(TR_THREADS, sizeof(R) == 4 ? INTERACT_MIN_BLOCKS : INTERACT_MIN_BLOCKS_F64)
 interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters* __restrict__ cin, PhotonRec<R>* __restrict__ q, uint32_t cap,
               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = cin->back;

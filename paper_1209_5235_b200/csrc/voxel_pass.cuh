@@ -23,6 +23,12 @@ enum : uint32_t { REC_ABOVE = 1u, REC_PENDING = 2u };      // PhotonRec::tail[0]
 #ifndef GENERAL_MIN_BLOCKS
 #define GENERAL_MIN_BLOCKS 6        // general_pass, fp32: 80 registers, 24 warps / SM
 #endif
+#ifndef VOX_MIN_BLOCKS_F64
+#define VOX_MIN_BLOCKS_F64 6        // voxel_pass, fp64: 80 registers, 24 warps / SM (4 / 5 / 6 / 8 blocks measured on config 2: 2.55 / 2.44 / 2.42 / 2.47 ms)
+#endif
+#ifndef GENERAL_MIN_BLOCKS_F64
+#define GENERAL_MIN_BLOCKS_F64 2
+#endif
 constexpr int SLOW_STEPS = 8;       // general steps a flagged photon may take in one slow_pass
 
 template <class R> __device__ __forceinline__ bool direction_cacheable(const V3<R>& w, R delta) {
@@ -31,7 +37,7 @@ template <class R> __device__ __forceinline__ bool direction_cacheable(const V3<
 }
 
 template <class R, bool TRACK, bool SLABS>
-__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? VOX_MIN_BLOCKS : 4))
+__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? VOX_MIN_BLOCKS : VOX_MIN_BLOCKS_F64))
 voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __restrict__ cout, const PhotonRec<R>* __restrict__ qin,
            PhotonRec<R>* __restrict__ qout, PhotonRec<R>* __restrict__ S, uint32_t cap, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec,
            int K, int regroup_pct, int timed) {
@@ -166,7 +172,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
 // coming voxel_pass -- travelling ones behind its front segment, those that reached their interaction point to its back
 // segment, where interact_pass finds them; there is room, because front + back + flagged never exceeds the photons alive.
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? GENERAL_MIN_BLOCKS : 2))
+__global__ void __launch_bounds__(TR_THREADS, TR_PER_128 * (sizeof(R) == 4 ? GENERAL_MIN_BLOCKS : GENERAL_MIN_BLOCKS_F64))
 general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* __restrict__ S, PhotonRec<R>* __restrict__ q, uint32_t cap,
              DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = ctr->slow;
