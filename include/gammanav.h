@@ -104,7 +104,8 @@ typedef struct {
     double kernel_ms;          /* duration of the whole kernel sequence of the run (source pass, step passes, interaction
                                   passes, tail), CUDA events on the launching stream */
     double step_pass_ms;       /* sum of the launch durations of the lean wavefront step passes (the dominant kernel), one
-                                  CUDA-event pair per launch; only the first 64 such passes of each batch are timed */
+                                  CUDA-event pair per launch; only the first 64 such passes of each batch are timed, and only when
+                                  h_stats_out is not NULL (a caller that asks for no statistics gets no per-pass events) */
     uint64_t n_steps_step_pass;/* steps taken inside exactly those timed passes (later lean passes count in n_steps only) */
     uint64_t n_rayleigh;       /* Rayleigh scatters (gn_opts.rayleigh) */
 } gn_run_stats;

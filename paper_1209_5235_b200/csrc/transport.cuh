@@ -900,7 +900,7 @@ int transport_impl(const gn_geometry* geo, const SourceDev<R>& src, uint64_t see
             } else {
                 // interaction wavefront on the photons parked in the back of the input queue, then the lean step pass; the
                 // first TR_TIMED lean passes of a batch are timed one by one, and only their steps count as lean_steps
-                const bool timed = n_timed < TR_TIMED;
+                const bool timed = n_timed < TR_TIMED && h_stats != nullptr;      // per-pass event timing only for callers that ask for statistics
                 bool voxel = false;
                 if constexpr (!FLAT) voxel = geo->voxel_sched;
                 if (voxel) {
