@@ -173,7 +173,7 @@ int gn_nav_compute_step(const gn_geometry* geo, int precision, const void* d_pos
  *   serialise them (same stream, or an event between them).  Asynchronous on cuda_stream like gn_nav_compute_step.
  */
 #define GN_NOALLOC_MAX_QUERIES (1 << 20)
-#define GN_NOALLOC_SCRATCH_BYTES (256 + 5 * (1 << 20))
+#define GN_NOALLOC_SCRATCH_BYTES (1024 + 5 * (1 << 20))
 int gn_nav_compute_step_noalloc(const gn_geometry* geo, int precision, const void* d_pos, const void* d_dir,
                                 const int32_t* d_vol_in, const void* d_max_step, int64_t n,
                                 void* d_step_out, int32_t* d_next_vol_out, void* cuda_stream);

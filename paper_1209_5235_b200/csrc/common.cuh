@@ -70,15 +70,17 @@ __global__ void __launch_bounds__(NAV_THREADS) sort_keys_kernel(GeoView<R> g, co
     __syncthreads();
     if (threadIdx.x < SORT_KEYS && sh[threadIdx.x]) atomicAdd(&totals[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
 }
+constexpr int SORT_KEYS_MAX = 32;         // the scatter kernel takes the number of keys as an argument (<= this)
+constexpr int SORT_KEYS2 = 2 * SORT_KEYS; // relocation order of ComputeStep queries: volume kind x (boundary is the volume's own / a daughter's)
 static __global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const uint8_t* __restrict__ keys, int64_t n, const unsigned long long* __restrict__ totals,
                                                                    unsigned long long* __restrict__ cursors, uint32_t* __restrict__ perm,
-                                                                   const unsigned* __restrict__ n_ptr) {
-    __shared__ unsigned sh_cnt[SORT_KEYS];
-    __shared__ unsigned long long sh_base[SORT_KEYS];
+                                                                   const unsigned* __restrict__ n_ptr, int nkeys = SORT_KEYS) {
+    __shared__ unsigned sh_cnt[SORT_KEYS_MAX];
+    __shared__ unsigned long long sh_base[SORT_KEYS_MAX];
     if (n_ptr) n = (int64_t)*n_ptr;                                          // count known only on the device (transport passes)
     const int64_t n_tiles = (n + SORT_TILE - 1) / SORT_TILE;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        if (threadIdx.x < SORT_KEYS) sh_cnt[threadIdx.x] = 0;
+        if (threadIdx.x < nkeys) sh_cnt[threadIdx.x] = 0;
         __syncthreads();
         int key[SORT_TILE / NAV_THREADS]; unsigned rank[SORT_TILE / NAV_THREADS];
 #pragma unroll
@@ -88,7 +90,7 @@ static __global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const 
             rank[q] = key[q] >= 0 ? atomicAdd(&sh_cnt[key[q]], 1u) : 0u;
         }
         __syncthreads();
-        if (threadIdx.x < SORT_KEYS) {
+        if (threadIdx.x < nkeys) {
             unsigned long long seg = 0;                                        // start of this key's segment
             for (int k = 0; k < (int)threadIdx.x; ++k) seg += totals[k];
             sh_base[threadIdx.x] = seg + (sh_cnt[threadIdx.x] ? atomicAdd(&cursors[threadIdx.x], (unsigned long long)sh_cnt[threadIdx.x]) : 0ull);

@@ -19,10 +19,10 @@
 namespace gn {
 
 constexpr int64_t NOALLOC_MAX_QUERIES = GN_NOALLOC_MAX_QUERIES;
-constexpr size_t NOALLOC_HEAD = 256;                                   // key totals (16 x u64) + cursors (16 x u64)
+constexpr size_t NOALLOC_HEAD = STEP_SORT_HEAD;                        // totals and cursors of the two work orders (4 x 32 x u64)
 constexpr size_t NOALLOC_BYTES = NOALLOC_HEAD + (size_t)NOALLOC_MAX_QUERIES + 4 * (size_t)NOALLOC_MAX_QUERIES;
 static_assert(NOALLOC_BYTES == GN_NOALLOC_SCRATCH_BYTES, "gammanav.h states the size of the scratch array");
-static_assert(2 * 8 * SORT_KEYS <= NOALLOC_HEAD && NOALLOC_MAX_QUERIES % 64 == 0, "scratch layout");
+static_assert(NOALLOC_HEAD == 1024 && SORT_KEYS2 <= SORT_KEYS_MAX && NOALLOC_MAX_QUERIES % 64 == 0, "scratch layout");
 
 static __device__ __align__(256) unsigned char noalloc_scratch[NOALLOC_BYTES];
 
@@ -57,13 +57,14 @@ static int step_noalloc(const gn_geometry* geo, const void* pos, const void* dir
     unsigned char* scratch = nullptr;
     const int rc = noalloc_scratch_address(geo->device, &scratch);
     if (rc != GN_OK) return rc;
-    unsigned long long* totals = (unsigned long long*)scratch; unsigned long long* cursors = totals + 16;
+    unsigned long long* totals = (unsigned long long*)scratch; unsigned long long* cursors = totals + SORT_KEYS_MAX;
+    unsigned long long* totals2 = cursors + SORT_KEYS_MAX;
     uint8_t* keys = scratch + NOALLOC_HEAD;
     uint32_t* perm = (uint32_t*)(scratch + NOALLOC_HEAD + (size_t)NOALLOC_MAX_QUERIES);
     GN_CUDA(cudaMemsetAsync(scratch, 0, NOALLOC_HEAD, s), "gn_nav_compute_step_noalloc memset");      // the last call's counts
     sort_keys_kernel<R><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), vol, n, keys, totals);
     sort_scatter_kernel<<<nav_grid((n + 3) / 4), NAV_THREADS, 0, s>>>(keys, n, totals, cursors, perm, nullptr);
-    step_kernel<R, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, vol, (const R*)ms, n, (R*)step, next, perm);
+    step_two_wavefronts<R>(geo, pos, dir, vol, ms, n, step, next, perm, keys, totals2, s);
     GN_CUDA(cudaGetLastError(), "gn_nav_compute_step_noalloc launch");
     return GN_OK;
 }
