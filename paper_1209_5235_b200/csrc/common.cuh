@@ -87,7 +87,12 @@ static __global__ void __launch_bounds__(NAV_THREADS) sort_scatter_kernel(const 
         for (int q = 0; q < SORT_TILE / NAV_THREADS; ++q) {
             const int64_t i = tile * SORT_TILE + q * NAV_THREADS + threadIdx.x;
             key[q] = i < n ? keys[i] : -1;
-            rank[q] = key[q] >= 0 ? atomicAdd(&sh_cnt[key[q]], 1u) : 0u;
+            // rank inside the tile: one shared atomic per warp and distinct key (most of a warp shares one or two keys)
+            const unsigned peers = __match_any_sync(0xffffffffu, key[q]);
+            const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+            unsigned base = 0;
+            if (lane == leader && key[q] >= 0) base = atomicAdd(&sh_cnt[key[q]], (unsigned)__popc(peers));
+            rank[q] = __shfl_sync(0xffffffffu, base, leader) + __popc(peers & ((1u << lane) - 1u));
         }
         __syncthreads();
         if (threadIdx.x < nkeys) {
