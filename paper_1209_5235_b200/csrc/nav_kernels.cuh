@@ -27,6 +27,92 @@ __global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_B
     }
 }
 
+// locate on general geometries (tubes, rotations, nested placements) as a level-synchronous wavefront inside each warp.
+// In locate_kernel every lane runs its whole descent; lanes of a warp sit at different depths of the placement tree (config 5:
+// 70 % of the points are in the world volume, the others three to five levels down), so the voxel-cell lookups of a mother run
+// at 2.6 of 32 lanes and the kernel at 14.4 (profiles/r2_compute_step_split.md).  Here a warp owns a tile of up to
+// LOCATE_WTILE consecutive queries and walks the tree one level per round: the queries still descending are kept as a packed
+// list in shared memory (slot in the tile, volume reached); 32 entries at a time, each lane runs Navigator::descend_level on
+// one entry and puts it back (in place: a round writes no further than it has read) if it has further to go.  The lanes of a
+// round all do the same thing -- cell lookup or list walk of one kind of mother, then occupancy tests of candidates -- and a
+// query that is done leaves the list instead of idling in a warp.  No block barrier: a first version with one list per block
+// ran at 24.7 lanes but waited at __syncthreads (10 warps per issue) and gained 5 %.  Same visits, same arithmetic, same
+// answers as locate_kernel (tests/test_gpu_parity.py compares with the oracle bit for bit).  Queries are re-read from global
+// memory at every level (the tile is 7 KB: L1), answers are written as they are found.
+constexpr int LOCATE_WTILE = 256;
+template <class R, bool HAS_DIR>
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : NAV_LOCATE_MIN_BLOCKS_F64)
+locate_levels_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir, int64_t n, int32_t* __restrict__ vol_out, int wtile) {
+    constexpr int WARPS = NAV_THREADS / 32;
+    __shared__ BlockTables<R> tab;
+    __shared__ int32_t sh_vol[WARPS][LOCATE_WTILE];      // per warp: the queries still descending -- volume reached ...
+    __shared__ uint8_t sh_slot[WARPS][LOCATE_WTILE];     // ... and slot in the warp's tile
+    static_assert(LOCATE_WTILE <= 256, "tile slots are stored in a byte");
+    stage_tables(g, tab);
+    __syncthreads();
+    Navigator<R, HAS_DIR, true> nav(g, &tab.ctx);
+    const unsigned lane = threadIdx.x & 31u, below = (1u << lane) - 1u;
+    int32_t* const lv = sh_vol[threadIdx.x >> 5];
+    uint8_t* const ls = sh_slot[threadIdx.x >> 5];
+    const int64_t n_tiles = (n + wtile - 1) / wtile;
+    for (int64_t wt = (int64_t)blockIdx.x * WARPS + (threadIdx.x >> 5); wt < n_tiles; wt += (int64_t)gridDim.x * WARPS) {
+        const int64_t base = wt * wtile;
+        unsigned count = 0;                               // entries in the list (warp-uniform)
+        // the world volume and its own daughters: every query of the tile
+        for (int s = 0; s < wtile; s += 32) {
+            const int64_t i = base + s + lane;
+            bool more = false; int vol = -1;
+            if (i < n) {
+                const V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+                V3<R> w{0, 0, 0};
+                if (HAS_DIR) { w.x = dir[3 * i]; w.y = dir[3 * i + 1]; w.z = dir[3 * i + 2]; }
+                NodeRec<R> nd = nav.node(0);
+                V3<R> p, v;
+                to_local<R, true>(g.rot, 0, nd, x, w, p, v);
+                if (nav.occupied(nd, p, v)) { vol = 0; if (nd.ndau > 0) more = nav.descend_level(vol, nd, x, w); }
+                if (!more) vol_out[i] = vol;
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, more);
+            if (more) { const unsigned o = count + __popc(bal & below); lv[o] = vol; ls[o] = (uint8_t)(s + lane); }
+            count += __popc(bal);
+        }
+        __syncwarp();
+        while (count > 0) {                               // one level of the tree per turn
+            unsigned kept = 0;
+            for (unsigned t0 = 0; t0 < count; t0 += 32) {
+                const unsigned t = t0 + lane;
+                bool more = false; int vol = 0, slot = 0;
+                if (t < count) {
+                    vol = lv[t]; slot = ls[t];
+                    const int64_t i = base + slot;
+                    const V3<R> x{pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+                    V3<R> w{0, 0, 0};
+                    if (HAS_DIR) { w.x = dir[3 * i]; w.y = dir[3 * i + 1]; w.z = dir[3 * i + 2]; }
+                    NodeRec<R> nd = nav.node(vol);
+                    more = nav.descend_level(vol, nd, x, w);
+                    if (!more) vol_out[i] = vol;
+                }
+                __syncwarp();                             // entries t0 .. t0 + 31 are read; kept <= t0: the writes below stay behind
+                const unsigned bal = __ballot_sync(0xffffffffu, more);
+                if (more) { const unsigned o = kept + __popc(bal & below); lv[o] = vol; ls[o] = (uint8_t)slot; }
+                kept += __popc(bal);
+            }
+            __syncwarp();
+            count = kept;
+        }
+    }
+}
+// queries per warp tile: LOCATE_WTILE when the batch fills the chip that way, fewer (a multiple of 32) for small batches
+inline int locate_wtile(int64_t n) {
+    const int64_t warps = 148 * 64;
+    const int64_t per = (n + warps - 1) / warps;
+    return (int)std::min<int64_t>(LOCATE_WTILE, std::max<int64_t>(32, (per + 31) / 32 * 32));
+}
+inline int locate_grid(int64_t n, int wtile) {
+    const int64_t per_block = (int64_t)wtile * (NAV_THREADS / 32);
+    return (int)std::max<int64_t>(1, std::min<int64_t>((n + per_block - 1) / per_block, 148 * 64));
+}
+
 template <class R, bool FLAT>
 __global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_STEP_MIN_BLOCKS : NAV_STEP_MIN_BLOCKS_F64) step_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir,
                                                            const int32_t* __restrict__ vol_in, const R* __restrict__ max_step,
@@ -264,8 +350,14 @@ template <class R> int locate_impl(const gn_geometry* geo, const void* pos, cons
         if (dir) locate_kernel<R, true, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
         else locate_kernel<R, false, false><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
     } else {
+#ifdef GN_LOCATE_FLAT
         if (dir) locate_kernel<R, true, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out);
         else locate_kernel<R, false, true><<<nav_grid(n), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out);
+#else
+        const int wtile = locate_wtile(n);
+        if (dir) locate_levels_kernel<R, true><<<locate_grid(n, wtile), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, (const R*)dir, n, out, wtile);
+        else locate_levels_kernel<R, false><<<locate_grid(n, wtile), NAV_THREADS, 0, s>>>(view<R>(geo), (const R*)pos, nullptr, n, out, wtile);
+#endif
     }
     GN_CUDA(cudaGetLastError(), "gn_nav_locate launch");
     return GN_OK;
