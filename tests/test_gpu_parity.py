@@ -241,6 +241,29 @@ def test_steps_that_end_near_the_edges_of_barrel_sectors(B):
         assert in_sector.mean() > 0.5 and (rnxt[in_sector] >= 3).mean() > 0.3
 
 
+@pytest.mark.parametrize("name", ["detector", "cmslike", "mixed"])
+def test_locate_level_by_level_every_tile_width(B, name):
+    """gn_nav_locate on general geometries walks the placement tree level by level inside each warp, on tiles of 32 ... 256
+    queries per warp chosen from the batch size (locate_levels_kernel): every tile width, single queries,
+    ragged tiles and ragged last warps against the oracle, element by element, with and without directions."""
+    geom = GEOMS[name]()
+    og = oracle.OracleGeometry(geom); g = B.Geometry(geom)
+    rng = np.random.default_rng(77)
+    warps = 148 * 64
+    sizes = [1, 31, 33, 255, 257, warps * 32 + 5, warps * 40 + 3, warps * 100 + 7, warps * 130 + 1, warps * 170 - 3, warps * 200 + 1, warps * 250 + 3]
+    n_max = max(sizes)
+    p = query_points(geom, rng, n_max).astype(np.float32); v = unit(rng, n_max).astype(np.float32)
+    ref = og.locate(p, v, 32); ref0 = og.locate(p, None, 32)
+    assert (ref == -1).any() and len(np.unique(ref)) > 4
+    tp, tv = cuda(p), cuda(v)
+    for n in sizes:
+        o = int(rng.integers(0, n_max - n + 1))                      # a different slice of the same queries each time
+        assert np.array_equal(B.nav_locate(g, tp[o:o + n], tv[o:o + n]).cpu().numpy(), ref[o:o + n]), n
+        assert np.array_equal(B.nav_locate(g, tp[o:o + n], None).cpu().numpy(), ref0[o:o + n]), n
+    pd = p[:warps * 40 + 3].astype(np.float64); vd = v[:warps * 40 + 3].astype(np.float64)
+    assert np.array_equal(B.nav_locate(g, cuda(pd), cuda(vd)).cpu().numpy(), og.locate(pd, vd, 64))
+
+
 def test_nav_edge_cases(B):
     import torch
     geom = GEOMS["slab"]()
