@@ -348,7 +348,7 @@ def run_ours(args):
             B.nav_locate(geo, pos, dirs, out=vol)
             B.nav_compute_step(geo, pos, dirs, vol, out=out)
             ev[1].record(); ev[1].synchronize()
-            # locate_kernel, sort_keys_kernel, sort_scatter_kernel, step_distance_kernel, sort_scatter_kernel, step_relocate_kernel
+            # locate_levels_kernel, sort_keys_kernel, sort_scatter_kernel, step_distance_kernel, sort_scatter_kernel, step_relocate_kernel
             return n, 6, ev[0].elapsed_time(ev[1])
 
     def barrier():
@@ -464,7 +464,7 @@ def run_ours(args):
         voxel = transport and wl.name.startswith(("config3", "config2"))      # geometries of regular voxels / slabs run the voxel schedule (gn_geometry::voxel_sched)
         roofline = {"bound": bound, "achieved": ach, "peak": pk, "unit": un, "frac": fr, "traffic": traffic,
                     "peak_source": peak_src if bound == "hbm" else pipe_src,
-                    "kernel": ("voxel_pass (regular-voxel step pass)" if voxel else "transport_pass<R,0,0,0> (lean wavefront step pass)") if transport else "locate_kernel + query sort + step_distance_kernel + step_relocate_kernel",
+                    "kernel": ("voxel_pass (regular-voxel step pass)" if voxel else "transport_pass<R,0,0,0> (lean wavefront step pass)") if transport else "locate_levels_kernel + query sort + step_distance_kernel + step_relocate_kernel",
                     "algorithmic_bytes_per_unit": abytes, "flops_per_unit": flops_per_unit, "flops_source": flops_src,
                     "hbm_peak_gbs": peak, "pipe_peak_tflops": pipe_tflops, "pipe_peak_source": pipe_src,
                     "frac_hbm": dh, "frac_alu": da,
