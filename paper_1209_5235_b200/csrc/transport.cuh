@@ -540,8 +540,8 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = cin->back;
     if (blockIdx.x * TR_THREADS >= n) return;
-    __shared__ unsigned long long sh_cnt[ST_COUNT];
-    __shared__ double sh_en[4];
+    __shared__ unsigned sh_cnt[ST_COUNT];            // a block counts at most TR_THREADS events: 32-bit shared atomics are single instructions,
+    __shared__ double sh_en[4];                      // 64-bit ones compare-and-swap loops (5 % of this kernel's stall samples, profiles/r2_final.md)
     if (threadIdx.x < ST_COUNT) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
@@ -573,7 +573,7 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         r.ctr = io.j;
         if (alive && (r.misc & 0xffu) >= (uint32_t)g.stuck_limit) {           // stuck guard (C9), after the step's event
             ev = EV_STUCK; alive = false;
-            atomicAdd(&sh_cnt[ST_STUCK], 1ull); atomicAdd(&sh_en[EN_STUCK], (double)r.E);
+            atomicAdd(&sh_cnt[ST_STUCK], 1u); atomicAdd(&sh_en[EN_STUCK], (double)r.E);
         }
         if (TRACK) {
             uint64_t h = hash_state(pp, sec, r.idx);
@@ -589,16 +589,16 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         const unsigned nE = __popc(__ballot_sync(0xffffffffu, ev_done == EV_PE)), nP = __popc(__ballot_sync(0xffffffffu, ev_done == EV_PAIR));
         const unsigned nR = __popc(__ballot_sync(0xffffffffu, ev_done == EV_RAYLEIGH));
         if ((threadIdx.x & 31) == 0) {
-            if (nC) atomicAdd(&sh_cnt[ST_COMPTON], (unsigned long long)nC);
-            if (nX) atomicAdd(&sh_cnt[ST_CUT], (unsigned long long)nX);
-            if (nE) atomicAdd(&sh_cnt[ST_PE], (unsigned long long)nE);
-            if (nP) atomicAdd(&sh_cnt[ST_PAIR], (unsigned long long)nP);
-            if (nR) atomicAdd(&sh_cnt[ST_RAYLEIGH], (unsigned long long)nR);
+            if (nC) atomicAdd(&sh_cnt[ST_COMPTON], nC);
+            if (nX) atomicAdd(&sh_cnt[ST_CUT], nX);
+            if (nE) atomicAdd(&sh_cnt[ST_PE], nE);
+            if (nP) atomicAdd(&sh_cnt[ST_PAIR], nP);
+            if (nR) atomicAdd(&sh_cnt[ST_RAYLEIGH], nR);
         }
     }
     warp_tally(edep, &sh_en[EN_DEPOSITED], vol, dep_d, active);
     __syncthreads();
-    if (threadIdx.x < ST_COUNT && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], sh_cnt[threadIdx.x]);
+    if (threadIdx.x < ST_COUNT && sh_cnt[threadIdx.x]) atomicAdd(&stats->cnt[threadIdx.x], (unsigned long long)sh_cnt[threadIdx.x]);
     if (threadIdx.x >= 16 && threadIdx.x < 20 && sh_en[threadIdx.x - 16] != 0.0) atomicAdd(&stats->en[threadIdx.x - 16], sh_en[threadIdx.x - 16]);
 }
 
