@@ -90,7 +90,7 @@ struct SortIO { KeyCounters* kout; uint8_t* keys_out; const uint32_t* perm_in; }
 template <class R> struct alignas(16) PhotonRec {
     R x, y, z, wx, wy, wz, E, Y, gPE, gKN, L2k;
     int32_t vol; uint32_t idx, ctr, misc;        // misc = zero_steps | nsteps << 8
-    uint32_t tail[sizeof(R) == 4 ? 1 : 2];       // tail[0] = E above the pair threshold (k > 2); rest padding
+    uint32_t tail[sizeof(R) == 4 ? 1 : 2];       // tail[0]: bit 0 = E above the pair threshold (k > 2), bit 1 = parked at an interaction point, bits 8.. = material of vol (written by the step passes for interact_pass); rest padding
 };
 static_assert(sizeof(PhotonRec<float>) == 64 && sizeof(PhotonRec<double>) == 112, "photon record layout");
 
@@ -482,7 +482,7 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
         r.gPE = gPE; r.gKN = gKN; r.L2k = L2k; r.vol = vol; r.idx = idx; r.ctr = ctr; r.misc = misc;
 #pragma unroll
         for (int q = 0; q < (int)(sizeof(r.tail) / 4); ++q) r.tail[q] = 0;
-        r.tail[0] = (uint32_t)above | (pending ? 2u : 0u);
+        r.tail[0] = (uint32_t)above | (pending ? 2u : 0u) | ((uint32_t)nd.mat << 8);      // material of vol: interact_pass needs no node load
         GN_CHECK(o < cap && vol >= 0 && vol < g.n_nodes, CHK_STORE_SLOT);
         store_rec(qout, o, r);
         if (TRACK) hash_state(pp, sec, idx) = h;
@@ -552,9 +552,9 @@ interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters
         GN_CHECK(n <= cap, CHK_LOAD_SLOT);
         PhotonRec<R> r; load_rec(q, cap - 1u - i, r);
         vol = r.vol;
-        GN_CHECK(vol >= 0 && vol < g.n_nodes && g.node[vol].mat < g.n_mats, CHK_VOLUME);
+        GN_CHECK(vol >= 0 && vol < g.n_nodes && (int)(r.tail[0] >> 8) == g.node[vol].mat, CHK_VOLUME);
         const int above = (int)(r.tail[0] & 1u);
-        const int mat = __ldg(&g.node[vol].mat);
+        const int mat = (int)(r.tail[0] >> 8);                                 // written with the record by the pass that parked the photon
         const MuParts<R> mp = photon_mu(g, g.mats[mat], mat, r.E, r.gPE, r.gKN, r.L2k, above);
         InteractIO<R> io;
         io.E = r.E; io.wx = r.wx; io.wy = r.wy; io.wz = r.wz; io.Y = r.Y; io.gPE = r.gPE; io.gKN = r.gKN; io.L2k = r.L2k; io.j = r.ctr; io.above = above;

@@ -16,7 +16,7 @@
 
 namespace gn {
 
-enum : uint32_t { REC_ABOVE = 1u, REC_PENDING = 2u };      // PhotonRec::tail[0]
+enum : uint32_t { REC_ABOVE = 1u, REC_PENDING = 2u, REC_MAT_SHIFT = 8u };      // PhotonRec::tail[0]: flags, material of vol from bit 8
 #ifndef VOX_MIN_BLOCKS
 #define VOX_MIN_BLOCKS 8            // 64 registers: 32 warps / SM (10 blocks = 48 registers spill)
 #endif
@@ -141,7 +141,7 @@ voxel_pass(GeoView<R> g, const PassCounters* __restrict__ cin, PassCounters* __r
         r.gPE = gPE; r.gKN = gKN; r.L2k = L2k; r.vol = vol; r.idx = idx; r.ctr = ctr; r.misc = misc;
 #pragma unroll
         for (int q = 0; q < (int)(sizeof(r.tail) / 4); ++q) r.tail[q] = 0;
-        r.tail[0] = above | (pending ? REC_PENDING : 0u);
+        r.tail[0] = above | (pending ? REC_PENDING : 0u) | ((uint32_t)nd.mat << REC_MAT_SHIFT);
         GN_CHECK(vol >= 0 && vol < g.n_nodes && nd.mat < g.n_mats, CHK_VOLUME);
         GN_CHECK(!key2 || sh_base[2] + sh_wcount[2][warp] + __popc(bal2 & below) < cap, CHK_SLOW_SLOT);
         GN_CHECK(key2 || (key1 ? sh_base[1] + sh_wcount[1][warp] + __popc(bal1 & below) : sh_base[0] + sh_wcount[0][warp] + __popc(bal0 & below)) < cap, CHK_STORE_SLOT);
@@ -230,7 +230,7 @@ general_pass(GeoView<R> g, PassCounters* __restrict__ ctr, const PhotonRec<R>* _
         }
         if (TRACK && alive) hash_state(pp, sec, r.idx) = h;
         r.x = x.x; r.y = x.y; r.z = x.z; r.Y = Y; r.misc = misc; r.vol = vol;
-        r.tail[0] = (uint32_t)above | (pending ? REC_PENDING : 0u);
+        r.tail[0] = (uint32_t)above | (pending ? REC_PENDING : 0u) | ((uint32_t)nd.mat << REC_MAT_SHIFT);
     }
     // ---- append the survivors to the queue: warp-aggregated cursors ------------------------------------------------------
     {
