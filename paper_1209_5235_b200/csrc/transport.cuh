@@ -528,6 +528,9 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 // The interaction wavefront (A6-A9): every photon parked at an interaction point by the previous pass sits in the
 // back segment of the queue (slots cap-1, cap-2, ...); one thread per photon samples the process, updates the record
 // in place (absorbed photons are marked vol = -1) and the warp tallies the deposits.
+#ifndef INTERACT_THREADS
+#define INTERACT_THREADS TR_THREADS     // threads per block of interact_pass (a block waits for its slowest warp)
+#endif
 #ifndef INTERACT_MIN_BLOCKS
 #define INTERACT_MIN_BLOCKS 6      // 80 registers, 24 warps / SM (1 block: 82 registers -- the same code, but the occupancy is then promised)
 #endif
@@ -535,17 +538,17 @@ transport_pass(GeoView<R> g, SourceDev<R> src, uint64_t seed, uint64_t first_id,
 #define INTERACT_MIN_BLOCKS_F64 3
 #endif
 template <class R, bool TRACK>
-__global__ void __launch_bounds__(TR_THREADS, sizeof(R) == 4 ? INTERACT_MIN_BLOCKS : INTERACT_MIN_BLOCKS_F64)
+__global__ void __launch_bounds__(INTERACT_THREADS, ((sizeof(R) == 4 ? INTERACT_MIN_BLOCKS : INTERACT_MIN_BLOCKS_F64) * TR_THREADS + INTERACT_THREADS - 1) / INTERACT_THREADS)
 interact_pass(GeoView<R> g, uint64_t seed, uint64_t first_id, const PassCounters* __restrict__ cin, PhotonRec<R>* __restrict__ q, uint32_t cap,
               double* __restrict__ edep, DevStats* __restrict__ stats, PerPhotonOut pp, SecIO<R> sec) {
     const unsigned n = cin->back;
-    if (blockIdx.x * TR_THREADS >= n) return;
+    if (blockIdx.x * INTERACT_THREADS >= n) return;
     __shared__ unsigned sh_cnt[ST_COUNT];            // a block counts at most TR_THREADS events: 32-bit shared atomics are single instructions,
     __shared__ double sh_en[4];                      // 64-bit ones compare-and-swap loops (5 % of this kernel's stall samples, profiles/r2_final.md)
     if (threadIdx.x < ST_COUNT) sh_cnt[threadIdx.x] = 0;
     if (threadIdx.x < 4) sh_en[threadIdx.x] = 0.0;
     __syncthreads();
-    const unsigned i = blockIdx.x * TR_THREADS + threadIdx.x;
+    const unsigned i = blockIdx.x * INTERACT_THREADS + threadIdx.x;
     const bool active = i < n;
     double dep_d = 0.0; int vol = 0, ev_done = -1;
     if (active) {
@@ -758,8 +761,9 @@ static void launch_pass(bool track, unsigned blocks, cudaStream_t s, const GeoVi
 template <class R>
 static void launch_interact(bool track, unsigned blocks, cudaStream_t s, const GeoView<R>& g, uint64_t seed, uint64_t first_id, const PassCounters* cin,
                             PhotonRec<R>* q, uint32_t cap, double* edep, DevStats* stats, PerPhotonOut pp, SecIO<R> sec) {
-    if (track) interact_pass<R, true><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
-    else interact_pass<R, false><<<blocks, TR_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
+    const unsigned ib = (unsigned)(((uint64_t)blocks * TR_THREADS + INTERACT_THREADS - 1) / INTERACT_THREADS);
+    if (track) interact_pass<R, true><<<ib, INTERACT_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
+    else interact_pass<R, false><<<ib, INTERACT_THREADS, 0, s>>>(g, seed, first_id, cin, q, cap, edep, stats, pp, sec);
 }
 
 template <class R, bool FLAT>
