@@ -40,8 +40,15 @@ __global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_B
 // answers as locate_kernel (tests/test_gpu_parity.py compares with the oracle bit for bit).  Queries are re-read from global
 // memory at every level (the tile is 7 KB: L1), answers are written as they are found.
 constexpr int LOCATE_WTILE = 256;
+// blocks per SM, measured on config 5 (6 / 3: 40 / 80 registers; 8 / 4 spill, fp32 11.70 -> 11.62 ms, fp64 19.59 -> 19.36 ms; fp64 at 5, 6, 8: 20.0, 21.0, 22.1 ms)
+#ifndef NAV_LEVELS_MIN_BLOCKS
+#define NAV_LEVELS_MIN_BLOCKS 6
+#endif
+#ifndef NAV_LEVELS_MIN_BLOCKS_F64
+#define NAV_LEVELS_MIN_BLOCKS_F64 3
+#endif
 template <class R, bool HAS_DIR>
-__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LOCATE_MIN_BLOCKS : NAV_LOCATE_MIN_BLOCKS_F64)
+__global__ void __launch_bounds__(NAV_THREADS, sizeof(R) == 4 ? NAV_LEVELS_MIN_BLOCKS : NAV_LEVELS_MIN_BLOCKS_F64)
 locate_levels_kernel(GeoView<R> g, const R* __restrict__ pos, const R* __restrict__ dir, int64_t n, int32_t* __restrict__ vol_out, int wtile) {
     constexpr int WARPS = NAV_THREADS / 32;
     __shared__ BlockTables<R> tab;
